@@ -1,0 +1,196 @@
+"""Seeded synthetic workloads: the five BASELINE.json configs (codes + frames).
+
+This module serves BOTH the CPU oracle (tests) and the CUDA path (tests, bench.py, smoke).  It holds none of
+the decoder's arithmetic: it draws base matrices, random words, their syndromes and BIAWGN channel LLRs with
+numpy only.  It imports neither `oracle/` nor the CUDA binding.
+
+Conventions (citations are /root/reference/PAPER.md lines, "P:NNN"):
+
+* Base matrix `base_shifts[mb][nb]`, int32: -1 = all-zero ZxZ block, p in [0,Z) = the ZxZ identity with every row
+  cyclically shifted right by p (paper entry i = p+1): check R*Z + r is connected to variable
+  C*Z + ((r + p) mod Z).  Rows are checks, columns are variables.
+* Structure (Fig. 11; BASELINE.json configs): `n_core` dense "core" columns on the left, then a long
+  unshifted diagonal of degree-1 variables: column j >= n_core connects only to row j - n_core + top_rows, shift 0.
+  Each core column has `top_deg` edges to distinct random rows among the `top_rows` top rows and `low_deg` edges to
+  the lower rows, dealt so that every lower row receives exactly 2 core edges (readings S11, S14).
+* Frames: x uniform bits, s = H x mod 2, y = (1 - 2x) + N(0, sigma^2), LLR = 2 y / sigma^2 in fp32 (P:344 with one
+  sigma per frame).  sigma comes from `SIGMA_STAR` (BIAWGN capacity threshold, written by
+  `oracle/make_sigma_table.py`, which calls only `oracle/`) and the config's gap in dB.
+
+These inputs stand in for the paper's unpublished parity-check matrices and QKD data.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Dict, Tuple
+
+import numpy as np
+
+CODE_SEED_BASE = 17020774000  # + config index
+FRAME_SEED_BASE = 17020775000  # + 1000 * config index + frame index (+ 100 * snr point for config 5)
+
+# sigma* with C_BIAWGN(sigma*) = R, i.e. the channel noise std-dev at capacity for rate R.
+# Written by oracle/make_sigma_table.py (numerical integration in oracle/capacity.py); tests/test_capacity.py
+# re-derives them and compares.  Keys are code rates.
+SIGMA_STAR: Dict[float, float] = {
+    0.1: 2.5927695318,
+    0.05: 3.7325617743,
+    0.02: 5.9640225450,
+}
+
+
+@dataclass(frozen=True)
+class CodeSpec:
+    """Shape of one BASELINE.json code family."""
+    name: str
+    nb: int          # base columns
+    mb: int          # base rows
+    Z: int           # lifting size
+    n_core: int      # core (degree > 1) columns
+    top_rows: int    # rows holding the `top_deg` edges of each core column
+    top_deg: int
+    low_deg: int     # edges of each core column into the lower rows
+    rate: float      # design rate 1 - mb/nb
+    seed: int
+
+    @property
+    def n(self) -> int:
+        return self.nb * self.Z
+
+    @property
+    def m(self) -> int:
+        return self.mb * self.Z
+
+
+@dataclass(frozen=True)
+class Config:
+    """One BASELINE.json config: a code, a channel point and the decode arguments."""
+    index: int
+    code: CodeSpec
+    n_frames: int
+    max_iter: int
+    early_stop: int
+    gaps_db: Tuple[float, ...]      # dB above BIAWGN capacity, one entry per SNR point
+    description: str = ""
+
+
+def _spec(name, nb, mb, Z, n_core, top_rows, top_deg, low_deg, rate, idx) -> CodeSpec:
+    return CodeSpec(name, nb, mb, Z, n_core, top_rows, top_deg, low_deg, rate, CODE_SEED_BASE + idx)
+
+
+CONFIGS: Dict[int, Config] = {
+    1: Config(1, _spec("r0.10_80x72_Z32", 80, 72, 32, 16, 8, 3, 8, 0.1, 1), 16, 50, 0, (1.5,),
+              "tiny rate-0.1 code, 16 frames, 50 flooding iterations, early stop off"),
+    2: Config(2, _spec("r0.10_80x72_Z12500", 80, 72, 12500, 16, 8, 3, 8, 0.1, 2), 1, 200, 1, (0.5,),
+              "rate-0.1 n=1e6, 1 frame, max 200 iterations, early stop on"),
+    3: Config(3, _spec("r0.02_100x98_Z10000", 100, 98, 10000, 10, 8, 3, 18, 0.02, 3), 1, 500, 1, (0.3,),
+              "rate-0.02 n=1e6, 1 frame, max 500 iterations, early stop on"),
+    # config 4 is the code of config 3 (same seed) with 64 frames
+    4: Config(4, _spec("r0.02_100x98_Z10000", 100, 98, 10000, 10, 8, 3, 18, 0.02, 3), 64, 500, 1, (0.3,),
+              "batched throughput: config-3 code, 64 frames, max 500 iterations, early stop per frame"),
+    5: Config(5, _spec("r0.05_100x95_Z10000", 100, 95, 10000, 10, 5, 3, 18, 0.05, 5), 32, 300, 1,
+              (0.1, 0.3, 0.5, 0.7, 0.9, 1.1),
+              "rate-0.05 n=1e6, 32 frames per point, 6 SNR points, max 300 iterations, early stop on"),
+}
+
+
+def scaled_spec(spec: CodeSpec, Z: int) -> CodeSpec:
+    """Same base matrix (same seed), different lifting size: used for reduced-size parity cases."""
+    return CodeSpec(f"{spec.name.rsplit('_Z', 1)[0]}_Z{Z}", spec.nb, spec.mb, Z, spec.n_core, spec.top_rows,
+                    spec.top_deg, spec.low_deg, spec.rate, spec.seed)
+
+
+def sigma_for_gap(rate: float, gap_db: float) -> float:
+    """Noise std-dev `gap_db` dB above the BIAWGN capacity threshold of `rate`: sigma^2 = sigma*^2 10^(-gap/10)."""
+    return SIGMA_STAR[rate] * 10.0 ** (-gap_db / 20.0)
+
+
+def make_base_matrix(spec: CodeSpec) -> np.ndarray:
+    """Deterministic base matrix of circulant shifts, int32 [mb][nb], -1 = zero block.
+
+    The *structure* (which cells are non-zero) depends only on spec.seed, the shifts on (spec.seed, Z), so that
+    `scaled_spec` keeps the graph and only re-draws shifts.
+    """
+    rng = np.random.default_rng(spec.seed)
+    nb, mb, nc = spec.nb, spec.mb, spec.n_core
+    n_low = mb - spec.top_rows
+    assert nb - nc == n_low, "one degree-1 column per lower row"
+    assert nc * spec.low_deg == 2 * n_low, "every lower row receives exactly 2 core edges"
+    mask = np.zeros((mb, nb), dtype=bool)
+
+    # top part: top_deg distinct random rows per core column; re-draw until every top row has degree >= 2 (S11)
+    while True:
+        top = np.zeros((spec.top_rows, nc), dtype=bool)
+        for c in range(nc):
+            top[rng.choice(spec.top_rows, size=spec.top_deg, replace=False), c] = True
+        if top.sum(axis=1).min() >= 2:
+            break
+    mask[:spec.top_rows, :nc] = top
+
+    # lower part: shuffle the multiset {each lower row x 2}, deal low_deg sockets per core column, re-draw until
+    # every column's rows are distinct (S14)
+    sockets = np.repeat(np.arange(n_low), 2)
+    while True:
+        perm = rng.permutation(sockets).reshape(nc, spec.low_deg)
+        if all(len(set(perm[c])) == spec.low_deg for c in range(nc)):
+            break
+    for c in range(nc):
+        mask[spec.top_rows + perm[c], c] = True
+
+    base = np.full((mb, nb), -1, dtype=np.int32)
+    srng = np.random.default_rng([spec.seed, spec.Z])
+    base[mask] = srng.integers(0, spec.Z, size=int(mask.sum()), dtype=np.int32)
+    # degree-1 diagonal, unshifted
+    for j in range(nc, nb):
+        base[j - nc + spec.top_rows, j] = 0
+    return base
+
+
+def syndrome_of(base_shifts: np.ndarray, Z: int, x: np.ndarray) -> np.ndarray:
+    """s = H x mod 2 for x uint8 [..., nb*Z] by the lifting rule of P:324: s[R*Z+r] ^= x[C*Z + (r+p) mod Z]."""
+    mb, nb = base_shifts.shape
+    xs = x.reshape(x.shape[:-1] + (nb, Z))
+    s = np.zeros(x.shape[:-1] + (mb, Z), dtype=np.uint8)
+    for R in range(mb):
+        for C in np.nonzero(base_shifts[R] >= 0)[0]:
+            s[..., R, :] ^= np.roll(xs[..., C, :], -int(base_shifts[R, C]), axis=-1)
+    return s.reshape(x.shape[:-1] + (mb * Z,))
+
+
+@dataclass
+class Frames:
+    x: np.ndarray          # uint8 [F][n] transmitted word
+    syndrome: np.ndarray   # uint8 [F][m]
+    llr: np.ndarray        # float32 [F][n]
+    sigma: float
+
+
+def make_frames(base_shifts: np.ndarray, Z: int, sigma: float, n_frames: int, seed_base: int,
+                first_frame: int = 0) -> Frames:
+    """Frames first_frame .. first_frame+n_frames-1; frame f depends only on (seed_base + f)."""
+    mb, nb = base_shifts.shape
+    n = nb * Z
+    x = np.empty((n_frames, n), dtype=np.uint8)
+    llr = np.empty((n_frames, n), dtype=np.float32)
+    for k in range(n_frames):
+        rng = np.random.default_rng(seed_base + first_frame + k)
+        x[k] = rng.integers(0, 2, size=n, dtype=np.uint8)
+        y = (1.0 - 2.0 * x[k].astype(np.float64)) + sigma * rng.standard_normal(n)
+        llr[k] = (2.0 * y / (sigma * sigma)).astype(np.float32)
+    return Frames(x=x, syndrome=syndrome_of(base_shifts, Z, x), llr=llr, sigma=sigma)
+
+
+def frame_seed_base(cfg_index: int, snr_point: int = 0) -> int:
+    return FRAME_SEED_BASE + 1000 * cfg_index + 100 * snr_point
+
+
+def make_config(cfg_index: int, snr_point: int = 0, n_frames: int | None = None, Z: int | None = None,
+                first_frame: int = 0):
+    """(config, base_shifts, Z, frames) for a BASELINE.json config; Z / n_frames override for reduced cases."""
+    cfg = CONFIGS[cfg_index]
+    spec = cfg.code if Z is None else scaled_spec(cfg.code, Z)
+    base = make_base_matrix(spec)
+    sigma = sigma_for_gap(spec.rate, cfg.gaps_db[snr_point])
+    nf = cfg.n_frames if n_frames is None else n_frames
+    frames = make_frames(base, spec.Z, sigma, nf, frame_seed_base(cfg_index, snr_point), first_frame)
+    return cfg, base, spec.Z, frames
