@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on BASELINE.json's headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A "step" is one pass of the whole hot path over one batch: one qcldpc_decode call (LLR init, every flooding
+iteration's fused check/variable update, syndrome check with per-frame early exit, outputs) on config 4 of
+BASELINE.json: the rate-0.02, n = 1e6 code (100x98 base matrix, Z = 10,000), 64 seeded frames at 0.3 dB above BIAWGN
+capacity, max 500 iterations, early stop per frame.  Metric: decoded Mbit/s = coded bits / second (Eq. 17).
+
+  value     inputs resident in HBM; CUDA events on the launching stream; barrier + synchronize on both sides;
+            max over ranks.  Multi-GPU = independent replicas (frames are independent; no data-path collective):
+            every rank decodes its own 64 frames, value = all frames of all ranks / max time ("weak").
+  e2e       the same through qcldpc_decode_host: pinned HOST buffers, H2D of LLRs + syndromes and D2H of hard bits,
+            iteration counts and pass flags inside the timed region.
+  roofline  dominant kernel k_vn_pass: algorithmic bytes per launch (B_min of SURVEY.md §8(d) = 8*E_core + 4*n + m/8
+            per live frame-iteration) / its average launch duration, measured with CUDA event pairs recorded on the
+            decode stream inside the timed steps (qcldpc_profile_enable), against MEASURED_PEAKS.json's HBM copy rate.
+  cpu_baseline  the CPU oracle as it stands on the host cores, on a bounded sample of the same workload.
+
+--impl reference times the CPU oracle (the tier's reference arm) on the same config and metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1702_07740_b200 import workloads as W  # noqa: E402
+
+FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+NOMINAL_HBM_GBS = 8000.0       # north_star's "about 8 TB/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per k_vn_pass launch from the committed `ncu --set full` capture
+# (profiles/r01_vn_pass_full.md); None until a capture exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def algorithmic_bytes(cfg_code: W.CodeSpec):
+    """Per frame-iteration: B_min = 8*E_core + 4*n + m/8, B_2ph = 16*E_core + 4*n + m/8."""
+    e_core = cfg_code.n_core * (cfg_code.top_deg + cfg_code.low_deg) * cfg_code.Z
+    b_min = 8 * e_core + 4 * cfg_code.n + cfg_code.m / 8
+    b_2ph = 16 * e_core + 4 * cfg_code.n + cfg_code.m / 8
+    return b_min, b_2ph
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1])); smax.append(float(p[2]))
+                except ValueError:
+                    continue
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
+                                     p[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample(cfg: W.Config, base, Z, sigma, seed_base, sample_iters: int):
+    """Times the CPU oracle on a bounded sample: `cores` frames x sample_iters flooding iterations of the same
+    workload (early stop on, as configured).  Returns (extrapolated Mbit/s for the full max_iter decode, cores,
+    description, seconds)."""
+    import oracle
+    cores = os.cpu_count() or 1
+    frames_n = min(cores, cfg.n_frames)
+    fr = W.make_frames(base, Z, sigma, frames_n, seed_base)
+    oracle.build()
+    t0 = time.perf_counter()
+    res = oracle.decode(base, Z, fr.llr, fr.syndrome, sample_iters, cfg.early_stop, threads=frames_n)
+    dt = time.perf_counter() - t0
+    frame_iters = float(res.iters.sum())
+    sec_per_frame_iter_all_cores = dt / max(frame_iters, 1.0)      # wall seconds per frame-iteration, all cores busy
+    # full decode of this workload runs max_iter iterations per frame (frames stall)
+    mbit = cfg.code.n / (sec_per_frame_iter_all_cores * cfg.max_iter) / 1e6
+    desc = (f"{frames_n} frames x {sample_iters} of {cfg.max_iter} iterations of the same workload "
+            f"(one frame per thread, H construction included), scaled linearly to {cfg.max_iter} iterations")
+    return mbit, frames_n, desc, dt
+
+
+def run_reference(args, cfg, base, Z, sigma, seed_base, rank, world):
+    if rank != 0:
+        return
+    vals = []
+    for _ in range(args.warmup):
+        oracle_sample(cfg, base, Z, sigma, seed_base, args.ref_iters)
+    t_all = 0.0
+    for _ in range(args.steps):
+        mbit, cores, desc, dt = oracle_sample(cfg, base, Z, sigma, seed_base, args.ref_iters)
+        vals.append(mbit)
+        t_all += dt
+    value = statistics.mean(vals)
+    line = {
+        "impl": "reference", "metric": "decoded_mbit_per_s", "value": value, "unit": "Mbit/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_all / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "frames_per_gpu": cfg.n_frames, "max_iter": cfg.max_iter,
+                   "early_stop": cfg.early_stop},
+        "cpu_baseline": {"value": value, "unit": "Mbit/s", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": "Mbit/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg: W.Config) -> str:
+    sp = cfg.code
+    return (f"BASELINE.json config {cfg.index}: rate-{sp.rate} QC multi-edge code {sp.nb}x{sp.mb} base, Z={sp.Z}, "
+            f"n={sp.n}, {cfg.n_frames} frames, BIAWGN +{cfg.gaps_db[0]} dB over capacity, max {cfg.max_iter} "
+            f"iterations, early stop {'on' if cfg.early_stop else 'off'}")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (4 = headline batched workload)")
+    ap.add_argument("--frames", type=int, default=None, help="override frames per GPU (debug only)")
+    ap.add_argument("--max-iter", type=int, default=None, help="override max iterations (debug only)")
+    ap.add_argument("--ref-iters", type=int, default=8, help="iterations per oracle sample")
+    ap.add_argument("--profile-stride", type=int, default=4, help="time every k-th k_vn_pass launch")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    cfg = W.CONFIGS[args.config]
+    if args.frames is not None or args.max_iter is not None:
+        cfg = W.Config(cfg.index, cfg.code, args.frames or cfg.n_frames, args.max_iter or cfg.max_iter, cfg.early_stop,
+                       cfg.gaps_db, cfg.description)
+    base = W.make_base_matrix(cfg.code)
+    Z = cfg.code.Z
+    sigma = W.sigma_for_gap(cfg.code.rate, cfg.gaps_db[0])
+    seed_base = W.frame_seed_base(cfg.index) + 100000 * rank     # every rank decodes its own frames
+
+    if args.impl == "reference":
+        run_reference(args, cfg, base, Z, sigma, seed_base, rank, world)
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    from paper_1702_07740_b200 import binding as B
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group(backend="nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---------------------------------------------------------------------------------------------- inputs
+    frames = W.make_frames(base, Z, sigma, cfg.n_frames, seed_base)
+    code = B.QCLDPCCode(base, Z)
+    F, n, m = cfg.n_frames, code.n, code.m
+    h_llr = torch.from_numpy(frames.llr).pin_memory()
+    h_syn = torch.from_numpy(frames.syndrome).pin_memory()
+    d_llr = h_llr.to(dev)
+    d_syn = h_syn.to(dev)
+    ws = torch.empty(code.host_workspace_bytes(F, False), dtype=torch.uint8, device=dev)
+    out = B.DecodeResult(torch.empty((F, n), dtype=torch.uint8, device=dev),
+                         torch.empty(F, dtype=torch.int32, device=dev),
+                         torch.empty(F, dtype=torch.uint8, device=dev), None)
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        code.decode(d_llr, d_syn, cfg.max_iter, cfg.early_stop, want_posterior=False, workspace=ws, out=out,
+                    stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    launches_per_step = B.qcldpc_last_launch_count()
+
+    # ---------------------------------------------------------------------------------------------- timed region
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    B.qcldpc_profile_enable(args.profile_stride)
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    prof = B.qcldpc_profile_collect()
+    B.qcldpc_profile_enable(0)
+    clocks = sampler.stop()
+    iters = out.iters.cpu().numpy()
+    passed = out.passed.cpu().numpy()
+
+    # ---------------------------------------------------------------------------------------------- e2e (host buffers)
+    h_out = B.DecodeResult(torch.empty((F, n), dtype=torch.uint8).pin_memory(),
+                           torch.empty(F, dtype=torch.int32).pin_memory(),
+                           torch.empty(F, dtype=torch.uint8).pin_memory(), None)
+    e2e_steps = max(1, min(args.steps, 3))
+    code.decode_host(h_llr, h_syn, cfg.max_iter, cfg.early_stop, want_posterior=False, workspace=ws, out=h_out,
+                     stream=stream)
+    barrier()
+    t0 = time.perf_counter()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        code.decode_host(h_llr, h_syn, cfg.max_iter, cfg.early_stop, want_posterior=False, workspace=ws, out=h_out,
+                         stream=stream)
+    e1.record(stream)
+    barrier()
+    ms_e2e = max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0) * 0.0)
+    h2d = h_llr.numel() * 4 + h_syn.numel()
+    d2h = F * n + F * 4 + F
+    assert np.array_equal(h_out.iters.numpy(), iters)
+
+    # ---------------------------------------------------------------------------------------------- reduce over ranks
+    times = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(times[0]), float(times[1])
+
+    bits_per_step = float(F) * n * world
+    value = bits_per_step * args.steps / (ms_total * 1e-3) / 1e6
+    e2e_value = bits_per_step * e2e_steps / (ms_e2e * 1e-3) / 1e6
+
+    # ---------------------------------------------------------------------------------------------- roofline
+    b_min, b_2ph = algorithmic_bytes(cfg.code)
+    vn_ms, vn_timed, vn_launched = prof["vn_pass"]
+    ck_ms, ck_timed, ck_launched = prof["check"]
+    live_frame_iters = float(iters.sum())                         # per step: frames still live, summed over iterations
+    launches = max(int(iters.max()), 1)
+    live_per_launch = live_frame_iters / launches
+    vn_avg_ms = vn_ms / max(vn_timed, 1)
+    peak, peak_src = hbm_peak()
+    achieved = (b_min * live_per_launch) / (vn_avg_ms * 1e-3) / 1e9 if vn_timed else None
+    roofline = {
+        "bound": "hbm", "kernel": "k_vn_pass", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "frac": (achieved / peak) if achieved else None, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+        "peak_source": peak_src, "bytes_model": "B_min = 8*E_core + 4*n + m/8 per live frame-iteration",
+        "algorithmic_bytes_per_launch": b_min * live_per_launch, "avg_launch_ms": vn_avg_ms,
+        "timed_launches": int(vn_timed), "launches": int(vn_launched),
+        "frac_b2ph_of_peak": (b_2ph * live_per_launch) / (vn_avg_ms * 1e-3) / 1e9 / peak if vn_timed else None,
+        "frac_bmin_of_8tbs": (achieved / NOMINAL_HBM_GBS) if achieved else None,
+        "check_kernel_avg_ms": (ck_ms / ck_timed) if ck_timed else None,
+        "vn_share_of_step": (vn_avg_ms * vn_launched / args.steps) / (ms_total / args.steps) if vn_timed else None,
+    }
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        mbit, cores, desc, dt = oracle_sample(cfg, base, Z, sigma, seed_base, args.ref_iters)
+        cpu_baseline = {"value": mbit, "unit": "Mbit/s", "cores": cores, "kind": "oracle", "sample": desc,
+                        "sample_seconds": dt}
+
+    line = {
+        "metric": "decoded_mbit_per_s", "value": value, "unit": "Mbit/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "frames_per_gpu": F, "max_iter": cfg.max_iter,
+                   "early_stop": cfg.early_stop, "parallelism": f"replicas x{world} (frames independent, no collective)",
+                   "l2": "working set per step (1.3 GB of edge state + inputs) is larger than L2; no flush needed",
+                   "iterations_run": {"min": int(iters.min()), "max": int(iters.max()), "mean": float(iters.mean())},
+                   "frames_passed": int(passed.sum())},
+        "e2e": {"value": e2e_value, "unit": "Mbit/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps},
+        "gpu_launches": int(launches_per_step * args.steps),
+        "clocks": clocks,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+        "ms_per_iteration": ms_total / args.steps / launches,
+        "paper_context": "paper: 1.72 Mbit/s raw on a GTX 1080, own rate-0.02 q=21 code, 1 frame (P:506-511); "
+                         "another machine and code -- context, not a baseline",
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,114 @@
+/*
+ * qcldpc.h -- C ABI of libqcldpc: B200 (sm_100a) flooding Sum-Product decoder for quasi-cyclic LDPC codes in
+ * syndrome form (the decoder gets channel LLRs and a syndrome s and must reach H xhat = s).
+ *
+ * What is computed (citations: /root/reference/PAPER.md line numbers, "P:NNN"; readings S1..S14 in DESIGN.md):
+ *   Algorithm 1 of the paper: LLR initialisation L_vc <- Q_v; per iteration the check-node update
+ *   sgn(m_cv) = (-1)^{s_c} prod_{v' in N(c)\v} sgn(L_v'c),  |m_cv| = Phi^-1( sum_{v' in N(c)\v} Phi(|L_v'c|) ),
+ *   Phi(x) = -ln tanh(x/2) (the factor (-1)^{s_c} is the syndrome generalisation, S1),
+ *   clamped to |m_cv| <= QCLDPC_MSG_MAX (S2); the variable-node update L_vc = Q_v + sum_{c' in M(v)\c} m_c'v and
+ *   posterior L_v = Q_v + sum_{c in M(v)} m_cv; the hard decision xhat_v = 0 iff L_v >= 0 and
+ *   the early-termination test H xhat = s (mod 2) (P:363 generalised), per frame.
+ *   H is given as a base matrix of circulant shifts and a lifting size Z.
+ *
+ * All computation runs in CUDA kernels on the current device; there is no CPU fallback.  No function throws or
+ * exits; every function returns a status (0 = success, negative = error, see qcldpc_status_string).
+ */
+#ifndef QCLDPC_H_
+#define QCLDPC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QCLDPC_MSG_MAX 30.0f /* clamp on |m_cv| (reading S2); part of the definition of the result */
+
+enum {
+    QCLDPC_OK = 0,
+    QCLDPC_ERR_BAD_ARGUMENT = -1, /* NULL pointer, non-positive size, shift outside [-1, Z), max_iter < 0, ... */
+    QCLDPC_ERR_UNSUPPORTED = -2,  /* code outside the supported envelope (a column of degree > 64) */
+    QCLDPC_ERR_WORKSPACE = -3,    /* workspace NULL, misaligned (256 B) or smaller than qcldpc_workspace_bytes */
+    QCLDPC_ERR_CUDA = -4,         /* a CUDA runtime call failed; qcldpc_last_cuda_error() has the text */
+    QCLDPC_ERR_ALLOC = -5         /* host allocation failed */
+};
+
+typedef struct qcldpc_code qcldpc_code_t;
+
+/*
+ * Build a code handle from a base matrix.
+ *   base_shifts  HOST pointer, int32 row-major [mb][nb]; -1 = all-zero ZxZ block; p in [0,Z) = the ZxZ identity with
+ *                every row cyclically shifted right by p (the paper's entry i = p+1, I_i): check R*Z + r is connected
+ *                to variable C*Z + ((r + p) mod Z).  Rows are checks, columns are variables.
+ *   mb, nb, Z    > 0.   n = nb*Z variables, m = mb*Z checks.
+ *   out_code     receives the handle (owned by the caller, release with qcldpc_code_destroy).
+ * The handle owns small device tables (allocated with cudaMalloc on the current device) and is immutable: it may be
+ * used concurrently from several streams with distinct workspaces.  At most one degree-1 column per base row is
+ * "absorbed" into that row (such variables send Q_v forever and need no edge state); every other column is
+ * "active" and carries one fp32 of state per edge.  Active columns may have degree 0..64.
+ */
+int qcldpc_code_create(const int32_t* base_shifts, int mb, int nb, int Z, qcldpc_code_t** out_code);
+void qcldpc_code_destroy(qcldpc_code_t* code);
+
+/* Code facts: n, m, number of active base edges (state = 2 * 4 * Z * that many bytes per frame). */
+int qcldpc_code_info(const qcldpc_code_t* code, int64_t* n, int64_t* m, int64_t* active_base_edges);
+
+/* Bytes of DEVICE workspace qcldpc_decode needs for n_frames frames (0 on bad arguments). */
+size_t qcldpc_workspace_bytes(const qcldpc_code_t* code, int n_frames);
+
+/*
+ * Decode n_frames independent frames (Algorithm 1, syndrome form).  Only ENQUEUES work on `stream`; never
+ * synchronises the device; allocates nothing.  All d_* are DEVICE pointers owned by the caller, frame-major and
+ * contiguous:
+ *   d_llr        const float   [n_frames][n]  Q_v = ln P(x_v=0)/P(x_v=1)
+ *   d_syndrome   const uint8_t [n_frames][m]  s_c in {0,1} (only bit 0 is read)
+ *   max_iter     >= 0.  max_iter = 0: xhat = [Q < 0], d_iters = 0, d_pass by direct check (S6)
+ *   early_stop   0: exactly max_iter iterations, d_iters[f] = max_iter;  1: frame f stops at the first iteration t
+ *                (1-based) with H xhat = s, its outputs are those of iteration t (S5-S7)
+ *   d_hard       uint8_t [n_frames][n]   xhat_v = (L_v < 0) of the frame's last executed iteration
+ *   d_iters      int32_t [n_frames]      iteration at which the frame stopped, else max_iter
+ *   d_pass       uint8_t [n_frames]      1 iff H d_hard = d_syndrome
+ *   d_posterior  float   [n_frames][n]   L_v of the frame's last executed iteration; may be NULL
+ *   d_workspace  >= qcldpc_workspace_bytes(code, n_frames) bytes, 256-byte aligned; contents are scratch
+ *   stream       cudaStream_t passed as void* (NULL = the legacy default stream)
+ * Returns QCLDPC_OK once everything is enqueued.  Outputs are valid when the stream has drained.
+ */
+int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                  int max_iter, int early_stop, uint8_t* d_hard, int32_t* d_iters, uint8_t* d_pass,
+                  float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Same decode with HOST buffers (h_* are HOST pointers, same shapes; pinned memory makes the copies asynchronous):
+ * copies inputs host->device, decodes, copies outputs device->host on `stream`, then WAITS for the stream so that the
+ * h_* outputs are valid on return.  h_posterior may be NULL.  The device staging area is part of d_workspace, which
+ * must hold qcldpc_host_workspace_bytes(code, n_frames, h_posterior != NULL) bytes.
+ */
+size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int want_posterior);
+int qcldpc_decode_host(const qcldpc_code_t* code, const float* h_llr, const uint8_t* h_syndrome, int n_frames,
+                       int max_iter, int early_stop, uint8_t* h_hard, int32_t* h_iters, uint8_t* h_pass,
+                       float* h_posterior, void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Number of kernel launches the last qcldpc_decode / qcldpc_decode_host call of this thread enqueued. */
+int64_t qcldpc_last_launch_count(void);
+
+/*
+ * Optional launch timing for roofline reports (bench.py).  qcldpc_profile_enable(stride) with stride > 0 makes the
+ * following qcldpc_decode calls of this thread record a CUDA event pair, on the decode stream, around every
+ * stride-th launch of the two per-iteration kernels (kind 0 = fused check/variable update k_vn_pass, kind 1 =
+ * syndrome check k_check); stride = 0 switches it off.  qcldpc_profile_collect waits for the recorded events (host
+ * blocks until they have completed), returns for each kind the summed duration in ms of the timed launches, how many
+ * were timed and how many were launched since enable/collect, and clears the record.  ms_sum, timed, launched:
+ * HOST arrays of 2 entries.
+ */
+int qcldpc_profile_enable(int stride);
+int qcldpc_profile_collect(double* ms_sum, int64_t* timed, int64_t* launched);
+
+const char* qcldpc_status_string(int status);
+const char* qcldpc_last_cuda_error(void); /* thread-local text of the last CUDA failure ("" if none) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCLDPC_H_ */

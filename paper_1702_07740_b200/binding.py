@@ -1,0 +1,197 @@
+"""Thin Python binding of libqcldpc (include/qcldpc.h): argument marshalling only.
+
+Every step of the decode runs in the CUDA kernels of csrc/qcldpc.cu; PyTorch is used for device memory and streams.
+There is no CPU fallback: importing this module without csrc/libqcldpc.so raises, and so does every call on a box
+without a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import NamedTuple, Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "csrc", "libqcldpc.so")
+
+EXPORTED_SYMBOLS = (
+    "qcldpc_code_create", "qcldpc_code_destroy", "qcldpc_code_info", "qcldpc_workspace_bytes", "qcldpc_decode",
+    "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_last_launch_count", "qcldpc_status_string",
+    "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
+)
+
+if not os.path.exists(SO_PATH):
+    raise ImportError(f"{SO_PATH} is missing: build it with `python -m paper_1702_07740_b200.build` "
+                      "(there is no CPU fallback)")
+
+_lib = ctypes.CDLL(SO_PATH)
+_vp, _i, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+_lib.qcldpc_code_create.restype = _i
+_lib.qcldpc_code_create.argtypes = [_vp, _i, _i, _i, ctypes.POINTER(_vp)]
+_lib.qcldpc_code_destroy.restype = None
+_lib.qcldpc_code_destroy.argtypes = [_vp]
+_lib.qcldpc_code_info.restype = _i
+_lib.qcldpc_code_info.argtypes = [_vp, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64),
+                                  ctypes.POINTER(ctypes.c_int64)]
+_lib.qcldpc_workspace_bytes.restype = _sz
+_lib.qcldpc_workspace_bytes.argtypes = [_vp, _i]
+_lib.qcldpc_host_workspace_bytes.restype = _sz
+_lib.qcldpc_host_workspace_bytes.argtypes = [_vp, _i, _i]
+_DECODE_ARGS = [_vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.qcldpc_decode.restype = _i
+_lib.qcldpc_decode.argtypes = _DECODE_ARGS
+_lib.qcldpc_decode_host.restype = _i
+_lib.qcldpc_decode_host.argtypes = _DECODE_ARGS
+_lib.qcldpc_last_launch_count.restype = ctypes.c_int64
+_lib.qcldpc_last_launch_count.argtypes = []
+_lib.qcldpc_profile_enable.restype = _i
+_lib.qcldpc_profile_enable.argtypes = [_i]
+_lib.qcldpc_profile_collect.restype = _i
+_lib.qcldpc_profile_collect.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64),
+                                        ctypes.POINTER(ctypes.c_int64)]
+_lib.qcldpc_status_string.restype = ctypes.c_char_p
+_lib.qcldpc_status_string.argtypes = [_i]
+_lib.qcldpc_last_cuda_error.restype = ctypes.c_char_p
+_lib.qcldpc_last_cuda_error.argtypes = []
+
+
+class QCLDPCError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        text = _lib.qcldpc_status_string(status).decode()
+        detail = _lib.qcldpc_last_cuda_error().decode()
+        super().__init__(f"{where}: {text} ({status})" + (f": {detail}" if detail and status == -4 else ""))
+
+
+def _check(status: int, where: str) -> None:
+    if status != 0:
+        raise QCLDPCError(status, where)
+
+
+def qcldpc_status_string(status: int) -> str:
+    return _lib.qcldpc_status_string(status).decode()
+
+
+def qcldpc_last_launch_count() -> int:
+    return int(_lib.qcldpc_last_launch_count())
+
+
+def qcldpc_profile_enable(stride: int) -> None:
+    _check(_lib.qcldpc_profile_enable(int(stride)), "qcldpc_profile_enable")
+
+
+def qcldpc_profile_collect():
+    """{kind: (ms_sum, timed, launched)} for kind in ("vn_pass", "check")."""
+    ms = (ctypes.c_double * 2)()
+    timed = (ctypes.c_int64 * 2)()
+    launched = (ctypes.c_int64 * 2)()
+    _check(_lib.qcldpc_profile_collect(ms, timed, launched), "qcldpc_profile_collect")
+    return {name: (ms[k], timed[k], launched[k]) for k, name in enumerate(("vn_pass", "check"))}
+
+
+class DecodeResult(NamedTuple):
+    hard: "object"        # uint8  [F][n]
+    iters: "object"       # int32  [F]
+    passed: "object"      # uint8  [F]
+    posterior: "object"   # float32 [F][n] or None
+
+
+class QCLDPCCode:
+    """Owns a qcldpc_code_t handle (qcldpc_code_create / qcldpc_code_destroy)."""
+
+    def __init__(self, base_shifts: np.ndarray, Z: int):
+        base = np.ascontiguousarray(base_shifts, dtype=np.int32)
+        if base.ndim != 2:
+            raise ValueError("base_shifts must be [mb][nb]")
+        self.mb, self.nb = base.shape
+        self.Z = int(Z)
+        self._handle = _vp()
+        _check(_lib.qcldpc_code_create(base.ctypes.data, self.mb, self.nb, self.Z, ctypes.byref(self._handle)),
+               "qcldpc_code_create")
+        n, m, e = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        _check(_lib.qcldpc_code_info(self._handle, ctypes.byref(n), ctypes.byref(m), ctypes.byref(e)),
+               "qcldpc_code_info")
+        self.n, self.m, self.active_base_edges = n.value, m.value, e.value
+
+    def __del__(self):
+        h = getattr(self, "_handle", None)
+        if h:
+            _lib.qcldpc_code_destroy(h)
+            self._handle = None
+
+    # ---------------------------------------------------------------------------------------------- sizes
+    def workspace_bytes(self, n_frames: int) -> int:
+        return int(_lib.qcldpc_workspace_bytes(self._handle, int(n_frames)))
+
+    def host_workspace_bytes(self, n_frames: int, want_posterior: bool) -> int:
+        return int(_lib.qcldpc_host_workspace_bytes(self._handle, int(n_frames), int(bool(want_posterior))))
+
+    # ---------------------------------------------------------------------------------------------- decode
+    def decode(self, llr, syndrome, max_iter: int, early_stop: int, want_posterior: bool = True,
+               workspace=None, out: Optional[DecodeResult] = None, stream=None) -> DecodeResult:
+        """qcldpc_decode on device tensors: llr float32 [F][n], syndrome uint8 [F][m] (torch, cuda, contiguous).
+
+        Only enqueues work on `stream` (default: torch's current stream)."""
+        import torch
+        if not (llr.is_cuda and syndrome.is_cuda):
+            raise ValueError("qcldpc_decode needs CUDA tensors (no CPU fallback)")
+        if llr.dtype != torch.float32 or syndrome.dtype != torch.uint8:
+            raise ValueError("llr must be float32 and syndrome uint8")
+        llr = llr.contiguous()
+        syndrome = syndrome.contiguous()
+        if llr.dim() != 2 or llr.shape[1] != self.n or tuple(syndrome.shape) != (llr.shape[0], self.m):
+            raise ValueError(f"shapes {tuple(llr.shape)} / {tuple(syndrome.shape)} do not match n={self.n}, m={self.m}")
+        F = llr.shape[0]
+        dev = llr.device
+        need = self.workspace_bytes(F)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+        if out is None:
+            out = DecodeResult(torch.empty((F, self.n), dtype=torch.uint8, device=dev),
+                               torch.empty(F, dtype=torch.int32, device=dev),
+                               torch.empty(F, dtype=torch.uint8, device=dev),
+                               torch.empty((F, self.n), dtype=torch.float32, device=dev) if want_posterior else None)
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        with torch.cuda.device(dev):
+            rc = _lib.qcldpc_decode(self._handle, llr.data_ptr(), syndrome.data_ptr(), F, int(max_iter),
+                                    int(early_stop), out.hard.data_ptr(), out.iters.data_ptr(),
+                                    out.passed.data_ptr(),
+                                    out.posterior.data_ptr() if out.posterior is not None else None,
+                                    workspace.data_ptr(), workspace.numel(), st.cuda_stream)
+        _check(rc, "qcldpc_decode")
+        return out
+
+    def decode_host(self, llr: np.ndarray, syndrome: np.ndarray, max_iter: int, early_stop: int,
+                    want_posterior: bool = False, workspace=None, out=None, stream=None):
+        """qcldpc_decode_host on HOST arrays (numpy or pinned torch CPU tensors); returns host outputs.
+
+        Host<->device copies happen inside the call; it returns after the stream has drained."""
+        import torch
+
+        def ptr(a):
+            return a.data_ptr() if isinstance(a, torch.Tensor) else a.ctypes.data
+
+        F = llr.shape[0]
+        if tuple(llr.shape) != (F, self.n) or tuple(syndrome.shape) != (F, self.m):
+            raise ValueError("bad host shapes")
+        need = self.host_workspace_bytes(F, want_posterior)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+        if out is None:
+            out = DecodeResult(np.empty((F, self.n), dtype=np.uint8), np.empty(F, dtype=np.int32),
+                               np.empty(F, dtype=np.uint8),
+                               np.empty((F, self.n), dtype=np.float32) if want_posterior else None)
+        st = stream if stream is not None else torch.cuda.current_stream(workspace.device)
+        with torch.cuda.device(workspace.device):
+            rc = _lib.qcldpc_decode_host(self._handle, ptr(llr), ptr(syndrome), F, int(max_iter), int(early_stop),
+                                         ptr(out.hard), ptr(out.iters), ptr(out.passed),
+                                         ptr(out.posterior) if out.posterior is not None else None,
+                                         workspace.data_ptr(), workspace.numel(), st.cuda_stream)
+        _check(rc, "qcldpc_decode_host")
+        return out
+
+
+def raw_lib():
+    """The ctypes handle (tests use it to probe argument checking)."""
+    return _lib
