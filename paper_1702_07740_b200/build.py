@@ -1,32 +1,64 @@
-"""Build step: compiles csrc/qcldpc.cu into csrc/libqcldpc.so for sm_100a with nvcc (in-tree, no JIT cache).
+"""Build step: compiles csrc/*.cu into csrc/libqcldpc.so for sm_100a with nvcc (in-tree, no JIT cache).
 
-`python -m paper_1702_07740_b200.build [--force]`.  nvcc cross-compiles without a GPU.
+`python -m paper_1702_07740_b200.build [--force]`.  nvcc cross-compiles without a GPU.  k_vn_pass is instantiated once
+per register-array size in its own object file (vn_inst.cu with -DVN_DV / -DVN_EXACT); objects build in parallel.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
+OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
-SOURCES = [os.path.join(CSRC, "qcldpc.cu")]
-DEPS = SOURCES + [os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "vn_kernel.cuh"),
+           os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
+# (register array size DV, EXACT): EXACT = every active column has degree DV (the BASELINE.json codes: 11, 21)
+VN_INSTANCES = [(8, 0), (11, 1), (16, 0), (21, 1), (32, 0), (64, 0)]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+
+def _units():
+    units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), [])]
+    for dv, exact in VN_INSTANCES:
+        units.append((os.path.join(CSRC, "vn_inst.cu"), os.path.join(OBJDIR, f"vn_dv{dv}.o"),
+                      [f"-DVN_DV={dv}", f"-DVN_EXACT={exact}"]))
+    return units
+
+
+def _stale(target: str, deps) -> bool:
+    return (not os.path.exists(target)) or any(os.path.getmtime(d) > os.path.getmtime(target) for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    stale = (not os.path.exists(SO_PATH)) or any(os.path.getmtime(d) > os.path.getmtime(SO_PATH) for d in DEPS)
-    if force or stale:
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", SO_PATH] + SOURCES
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    os.makedirs(OBJDIR, exist_ok=True)
+    todo = [(src, obj, defs) for src, obj, defs in _units() if force or _stale(obj, [src] + HEADERS)]
+
+    def compile_one(unit):
+        src, obj, defs = unit
+        cmd = [nvcc] + NVCC_FLAGS + defs + ["-c", "-o", obj, src]
+        return cmd, subprocess.run(cmd, capture_output=True, text=True)
+
+    if todo:
+        with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 1)) as pool:
+            for cmd, res in pool.map(compile_one, todo):
+                if verbose or res.returncode != 0:
+                    sys.stderr.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+                if res.returncode != 0:
+                    raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    objs = [obj for _, obj, _ in _units()]
+    if todo or force or _stale(SO_PATH, objs):
+        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", SO_PATH] + objs
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
         if res.returncode != 0:
-            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+            raise RuntimeError("link failed: " + " ".join(cmd))
     return SO_PATH
 
 

@@ -21,9 +21,7 @@
 //   k_check    a3  check-centric: decides the absorbed degree-1 variables (L_j = Q_j + m_cj), xhat parity vs s_c,
 //              per-frame count of unsatisfied checks (integer atomics only); optional posterior write
 //   k_flags    a3  per-frame early exit: freezes d_iters / d_pass / done
-#include "../../include/qcldpc.h"
-
-#include <cuda_runtime.h>
+#include "common.cuh"
 
 #include <algorithm>
 #include <cstdio>
@@ -31,26 +29,19 @@
 #include <new>
 #include <vector>
 
+namespace qc {
+// one object file per instantiation of k_vn_pass (vn_inst.cu)
+void launch_vn_dv8(const VnLaunch&);
+void launch_vn_dv11(const VnLaunch&);
+void launch_vn_dv16(const VnLaunch&);
+void launch_vn_dv21(const VnLaunch&);
+void launch_vn_dv32(const VnLaunch&);
+void launch_vn_dv64(const VnLaunch&);
+}  // namespace qc
+
+using namespace qc;
+
 namespace {
-
-constexpr int kMaxDv = 64;       // largest supported active-column degree
-constexpr int kThreads = 128;    // threads per CTA in every kernel
-constexpr float kLog2e = 1.4426950408889634f;
-constexpr float kLn2 = 0.6931471805599453f;
-
-struct EdgeDesc { int shift; int row; int pbeg; int np; };        // one active base edge (own column side)
-struct PartnerDesc { int edge; int delta; };                      // other active edge of the same row; delta = (p' - p) mod Z
-struct ColDesc { int col; int ebeg; int dv; int pad; };           // active column: original column, first edge, degree
-struct RowDesc { int ebeg; int ne; int abs_col; int abs_shift; }; // base row: its active edges, absorbed column or -1
-struct RowEdge { int edge; int shift; int col; int pad; };        // active edge seen from its row
-
-// Tables small enough travel as __grid_constant__ kernel parameters (constant bank, uniform loads); larger codes
-// read the same tables from global memory.
-constexpr int kInlEdges = 256, kInlPartners = 512, kInlCols = 64, kInlRows = 128;
-struct VnTablesInline { EdgeDesc edge[kInlEdges]; PartnerDesc partner[kInlPartners]; ColDesc col[kInlCols]; };
-struct VnTablesGlobal { const EdgeDesc* edge; const PartnerDesc* partner; const ColDesc* col; };
-struct CnTablesInline { RowDesc row[kInlRows]; RowEdge redge[kInlEdges]; };
-struct CnTablesGlobal { const RowDesc* row; const RowEdge* redge; };
 
 thread_local char g_cuda_error[512] = "";
 thread_local int64_t g_launches = 0;
@@ -71,39 +62,20 @@ struct qcldpc_code {
     int64_t n, m;
     int n_act_cols, n_act_edges, n_partners, max_dv, bucket;
     bool uniform_dv, inline_ok;
-    std::vector<EdgeDesc> edge;
+    std::vector<PairDesc> pair;
     std::vector<PartnerDesc> partner;
+    std::vector<GenDesc> gen;
     std::vector<ColDesc> col;
     std::vector<RowDesc> row;
     std::vector<RowEdge> redge;
     // device copies
-    EdgeDesc* d_edge = nullptr; PartnerDesc* d_partner = nullptr; ColDesc* d_col = nullptr;
+    PairDesc* d_pair = nullptr; PartnerDesc* d_partner = nullptr; GenDesc* d_gen = nullptr; ColDesc* d_col = nullptr;
     RowDesc* d_row = nullptr; RowEdge* d_redge = nullptr;
     VnTablesInline vn_inl; CnTablesInline cn_inl;
+    VnLauncher launcher = nullptr;
 };
 
 namespace {
-
-// ---------------------------------------------------------------------------------------------------------------
-// device helpers
-// ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-
-// q(L) = sgn(L) exp(-|L|); sgn(x) = -1 iff x < 0, so -0.0 counts as + (reading S3)
-__device__ __forceinline__ float q_of_llr(float L) {
-    float q = ex2_approx(-fabsf(L) * kLog2e);
-    return __uint_as_float(__float_as_uint(q) | (L < 0.0f ? 0x80000000u : 0u));
-}
-// |m| = ln den - ln num, clamped (S2).  num = 0 -> +inf -> clamp.
-__device__ __forceinline__ float mag_of(float num, float den) {
-    return fminf(kLn2 * (lg2_approx(den) - lg2_approx(num)), QCLDPC_MSG_MAX);
-}
-__device__ __forceinline__ void boxplus_acc(float a, float& num, float& den) {
-    const float n2 = fmaf(a, den, num);
-    den = fmaf(a, num, den);
-    num = n2;
-}
 
 struct InitArgs {
     const float* llr; const uint8_t* syn; float* q0; float* t; uint8_t* hard; float* post;
@@ -143,87 +115,6 @@ __global__ void __launch_bounds__(kThreads) k_init_t(const __grid_constant__ Tab
     }
     const unsigned s = a.syn[(int64_t)f * a.m + c] & 1u;
     a.t[(int64_t)f * a.m + c] = __uint_as_float(__float_as_uint(t) ^ (s << 31));
-}
-
-struct VnArgs {
-    const float* llr; const float* qold; float* qnew; const float* t; uint8_t* hard; float* post; const int* done;
-    int Z, tiles; int64_t n, m, EZ;
-};
-
-// a1 + a2: fused check-node / variable-node update, one thread per U active variables.
-// DV: register array size (>= every column degree).  EXACT: every active column has degree DV (no predicates).
-template <int DV, int U, bool EXACT, class Tables>
-__global__ void __launch_bounds__(kThreads) k_vn_pass(const __grid_constant__ Tables tab, const VnArgs a) {
-    const int f = blockIdx.y;
-    if (a.done[f]) return;                                   // frame already stopped: its state stays frozen
-    const int ca = blockIdx.x / a.tiles;                     // block-uniform active column
-    const int tile = blockIdx.x - ca * a.tiles;
-    const ColDesc cd = tab.col[ca];
-    const int Z = a.Z;
-    const int dv = EXACT ? DV : cd.dv;
-    const float* __restrict__ qold = a.qold + (int64_t)f * a.EZ;
-    float* __restrict__ qnew = a.qnew + (int64_t)f * a.EZ;
-    const float* __restrict__ tf = a.t + (int64_t)f * a.m;
-
-    int i[U];
-    bool valid[U];
-    float Q[U];
-    float msg[U][DV];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const int ii = tile * (kThreads * U) + u * kThreads + threadIdx.x;
-        valid[u] = ii < Z;
-        i[u] = valid[u] ? ii : Z - 1;                        // clamp: loads stay in bounds, stores are guarded
-        Q[u] = __ldg(a.llr + (int64_t)f * a.n + (int64_t)cd.col * Z + i[u]);
-    }
-
-    // check-node side: for every edge (c,v) of this variable, combine the other inputs of check c
-#pragma unroll
-    for (int k = 0; k < DV; ++k) {
-        if (EXACT || k < dv) {
-            const EdgeDesc ed = tab.edge[cd.ebeg + k];
-            const float* trow = tf + (int64_t)ed.row * Z;
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                int r = i[u] - ed.shift; r += (r < 0) ? Z : 0;          // check index inside the block row
-                const float tt = __ldg(trow + r);
-                unsigned sg = __float_as_uint(tt) & 0x80000000u;
-                float num = fabsf(tt), den = 1.0f;
-                for (int j = 0; j < ed.np; ++j) {
-                    const PartnerDesc pd = tab.partner[ed.pbeg + j];
-                    int ip = i[u] + pd.delta; ip -= (ip >= Z) ? Z : 0;  // partner variable index in its column
-                    const float qa = __ldg(qold + (int64_t)pd.edge * Z + ip);
-                    sg ^= __float_as_uint(qa) & 0x80000000u;
-                    boxplus_acc(fabsf(qa), num, den);
-                }
-                msg[u][k] = __uint_as_float(__float_as_uint(mag_of(num, den)) | sg);
-            }
-        } else {
-#pragma unroll
-            for (int u = 0; u < U; ++u) msg[u][k] = 0.0f;
-        }
-    }
-
-    // variable-node side: L_v = Q_v + sum m, L_vc by direct exclusion via prefix + suffix sums
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        float suf[DV + 1];
-        suf[DV] = 0.0f;
-#pragma unroll
-        for (int k = DV - 1; k >= 0; --k) suf[k] = suf[k + 1] + msg[u][k];
-        float run = Q[u];
-#pragma unroll
-        for (int k = 0; k < DV; ++k) {
-            const float Lvc = run + suf[k + 1];
-            run += msg[u][k];
-            if ((EXACT || k < dv) && valid[u]) qnew[(int64_t)(cd.ebeg + k) * Z + i[u]] = q_of_llr(Lvc);
-        }
-        if (valid[u]) {
-            const int64_t v = (int64_t)f * a.n + (int64_t)cd.col * Z + i[u];
-            a.hard[v] = run < 0.0f ? 1 : 0;                  // 0 iff L_v >= 0
-            if (a.post) a.post[v] = run;
-        }
-    }
 }
 
 struct CnArgs {
@@ -354,12 +245,6 @@ Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
     return w;
 }
 
-template <int DV, int U, bool EXACT>
-void launch_vn(const qcldpc_code* code, const VnArgs& a, dim3 grid, cudaStream_t st) {
-    if (code->inline_ok) k_vn_pass<DV, U, EXACT, VnTablesInline><<<grid, kThreads, 0, st>>>(code->vn_inl, a);
-    else k_vn_pass<DV, U, false, VnTablesGlobal><<<grid, kThreads, 0, st>>>(VnTablesGlobal{code->d_edge, code->d_partner, code->d_col}, a);
-}
-
 // Register-array size used for a code: the exact degree when every active column has the same degree and a
 // specialisation exists (the BASELINE.json codes: 11 and 21), else the next bucket.
 int vn_bucket(int max_dv, bool uniform) {
@@ -368,19 +253,16 @@ int vn_bucket(int max_dv, bool uniform) {
     for (int b : buckets) if (max_dv <= b) return b;
     return -1;
 }
-int vn_unroll(int bucket) { return bucket > 21 ? 1 : 2; }   // variables per thread
-
-int dispatch_vn(const qcldpc_code* code, const VnArgs& a, dim3 grid, cudaStream_t st) {
-    switch (code->bucket) {
-        case 8:  launch_vn<8, 2, false>(code, a, grid, st); break;
-        case 11: launch_vn<11, 2, true>(code, a, grid, st); break;
-        case 16: launch_vn<16, 2, false>(code, a, grid, st); break;
-        case 21: launch_vn<21, 2, true>(code, a, grid, st); break;
-        case 32: launch_vn<32, 1, false>(code, a, grid, st); break;
-        case 64: launch_vn<64, 1, false>(code, a, grid, st); break;
-        default: return QCLDPC_ERR_UNSUPPORTED;
+VnLauncher vn_launcher(int bucket) {
+    switch (bucket) {
+        case 8: return launch_vn_dv8;
+        case 11: return launch_vn_dv11;
+        case 16: return launch_vn_dv16;
+        case 21: return launch_vn_dv21;
+        case 32: return launch_vn_dv32;
+        case 64: return launch_vn_dv64;
+        default: return nullptr;
     }
-    return QCLDPC_OK;
 }
 
 void launch_check(const qcldpc_code* code, const CnArgs& a, dim3 grid, cudaStream_t st) {
@@ -419,18 +301,20 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
                 absorbed_by[C] = R;
             }
     // active columns and their edges, in increasing (column, row) order
+    struct HostEdge { int shift, row, col_k; };
+    std::vector<HostEdge> edges;
     std::vector<int> edge_of_cell((size_t)mb * nb, -1);
     code->max_dv = 0;
     bool uniform = true;
     int first_dv = -1;
     for (int C = 0; C < nb; ++C) {
         if (absorbed_by[C] >= 0) continue;
-        ColDesc cd{C, (int)code->edge.size(), 0, 0};
+        ColDesc cd{C, (int)edges.size(), 0, 0, 0, 0, 0, 0};
         for (int R = 0; R < mb; ++R) {
             const int p = base[(size_t)R * nb + C];
             if (p < 0) continue;
-            edge_of_cell[(size_t)R * nb + C] = (int)code->edge.size();
-            code->edge.push_back(EdgeDesc{p, R, 0, 0});
+            edge_of_cell[(size_t)R * nb + C] = (int)edges.size();
+            edges.push_back(HostEdge{p, R, cd.dv});
             ++cd.dv;
         }
         code->col.push_back(cd);
@@ -438,10 +322,13 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
         if (first_dv < 0) first_dv = cd.dv;
         uniform = uniform && cd.dv == first_dv;
     }
-    if (code->max_dv > kMaxDv) { delete code; return QCLDPC_ERR_UNSUPPORTED; }
     code->n_act_cols = (int)code->col.size();
-    code->n_act_edges = (int)code->edge.size();
-    // row view and partner lists
+    code->n_act_edges = (int)edges.size();
+    if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Z >= ((int64_t)1 << 31)) {
+        delete code;
+        return QCLDPC_ERR_UNSUPPORTED;
+    }
+    // row view
     for (int R = 0; R < mb; ++R) {
         code->row[R].ebeg = (int)code->redge.size();
         for (int C = 0; C < nb; ++C) {
@@ -450,27 +337,48 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
         }
         code->row[R].ne = (int)code->redge.size() - code->row[R].ebeg;
     }
-    for (int e = 0; e < code->n_act_edges; ++e) {
-        EdgeDesc& ed = code->edge[e];
-        const RowDesc& rd = code->row[ed.row];
-        ed.pbeg = (int)code->partner.size();
-        for (int k = 0; k < rd.ne; ++k) {
-            const RowEdge& re = code->redge[rd.ebeg + k];
-            if (re.edge == e) continue;
-            code->partner.push_back(PartnerDesc{re.edge, ((re.shift - ed.shift) % Z + Z) % Z});
+    // per edge: the pair descriptor; rows with 0 or >= 2 other active edges get a partner list (GenDesc)
+    for (size_t ci = 0; ci < code->col.size(); ++ci) {
+        ColDesc& cd = code->col[ci];
+        cd.gbeg = (int)code->gen.size();
+        for (int k = 0; k < cd.dv; ++k) {
+            const int e = cd.ebeg + k;
+            const HostEdge& he = edges[e];
+            const RowDesc& rd = code->row[he.row];
+            PairDesc pd{he.shift, he.row * Z, -1, 0};
+            const int np = rd.ne - 1;
+            if (np == 1) {
+                for (int j = 0; j < rd.ne; ++j) {
+                    const RowEdge& re = code->redge[rd.ebeg + j];
+                    if (re.edge == e) continue;
+                    pd.p_off = re.edge * Z;
+                    pd.delta = ((re.shift - he.shift) % Z + Z) % Z;
+                }
+            } else {
+                GenDesc gd{k, (int)code->partner.size(), np, 0};
+                for (int j = 0; j < rd.ne; ++j) {
+                    const RowEdge& re = code->redge[rd.ebeg + j];
+                    if (re.edge == e) continue;
+                    code->partner.push_back(PartnerDesc{re.edge * Z, ((re.shift - he.shift) % Z + Z) % Z});
+                }
+                code->gen.push_back(gd);
+            }
+            code->pair.push_back(pd);
         }
-        ed.np = (int)code->partner.size() - ed.pbeg;
+        cd.ng = (int)code->gen.size() - cd.gbeg;
     }
     code->n_partners = (int)code->partner.size();
     code->uniform_dv = uniform && code->n_act_cols > 0;
     code->bucket = vn_bucket(code->max_dv, code->uniform_dv);
+    code->launcher = vn_launcher(code->bucket);
     code->inline_ok = code->n_act_edges <= kInlEdges && code->n_partners <= kInlPartners &&
-                      code->n_act_cols <= kInlCols && mb <= kInlRows;
+                      code->n_act_cols <= kInlCols && (int)code->gen.size() <= kInlGen && mb <= kInlRows;
     if (code->inline_ok) {
         memset(&code->vn_inl, 0, sizeof(code->vn_inl));
         memset(&code->cn_inl, 0, sizeof(code->cn_inl));
-        std::copy(code->edge.begin(), code->edge.end(), code->vn_inl.edge);
+        std::copy(code->pair.begin(), code->pair.end(), code->vn_inl.pair);
         std::copy(code->partner.begin(), code->partner.end(), code->vn_inl.partner);
+        std::copy(code->gen.begin(), code->gen.end(), code->vn_inl.gen);
         std::copy(code->col.begin(), code->col.end(), code->vn_inl.col);
         std::copy(code->row.begin(), code->row.end(), code->cn_inl.row);
         std::copy(code->redge.begin(), code->redge.end(), code->cn_inl.redge);
@@ -483,8 +391,9 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
         if (!vec.empty()) e = cudaMemcpy(*dptr, vec.data(), vec.size() * sizeof(vec[0]), cudaMemcpyHostToDevice);
         return e;
     };
-    cudaError_t e = upload(code->edge, &code->d_edge);
+    cudaError_t e = upload(code->pair, &code->d_pair);
     if (e == cudaSuccess) e = upload(code->partner, &code->d_partner);
+    if (e == cudaSuccess) e = upload(code->gen, &code->d_gen);
     if (e == cudaSuccess) e = upload(code->col, &code->d_col);
     if (e == cudaSuccess) e = upload(code->row, &code->d_row);
     if (e == cudaSuccess) e = upload(code->redge, &code->d_redge);
@@ -495,7 +404,7 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
 
 void qcldpc_code_destroy(qcldpc_code_t* code) {
     if (!code) return;
-    cudaFree(code->d_edge); cudaFree(code->d_partner); cudaFree(code->d_col);
+    cudaFree(code->d_pair); cudaFree(code->d_partner); cudaFree(code->d_gen); cudaFree(code->d_col);
     cudaFree(code->d_row); cudaFree(code->d_redge);
     delete code;
 }
@@ -534,27 +443,28 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
     InitArgs ia{d_llr, d_syndrome, w.qbuf[0], w.t, d_hard, d_posterior, Z, tiles1, code->n, code->m, EZ};
     if (code->n_act_cols > 0) {
         k_init_q<VnTablesGlobal><<<dim3(tiles1 * code->n_act_cols, n_frames), kThreads, 0, st>>>(
-            VnTablesGlobal{code->d_edge, code->d_partner, code->d_col}, ia);
+            VnTablesGlobal{code->d_pair, code->d_partner, code->d_gen, code->d_col}, ia);
         ++g_launches;
     }
     k_init_t<CnTablesGlobal><<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(
         CnTablesGlobal{code->d_row, code->d_redge}, ia);
     ++g_launches;
 
-    const int vn_u = vn_unroll(code->bucket);
-    const int tiles_vn = (Z + kThreads * vn_u - 1) / (kThreads * vn_u);
-    const dim3 grid_vn(tiles_vn * code->n_act_cols, n_frames);
+    const dim3 grid_vn(tiles1 * code->n_act_cols, n_frames);
+    if (code->n_act_cols > 0 && !code->launcher) return QCLDPC_ERR_UNSUPPORTED;
     const dim3 grid_cn(tiles1 * code->mb, n_frames);
     CnArgs ca{d_llr, d_syndrome, w.qbuf[0], w.qbuf[1], d_hard, nullptr, w.done, d_iters, w.unsat,
               Z, tiles1, 0, 1, 1, code->n, code->m, EZ};
 
     for (int t = 1; t <= max_iter; ++t) {
         if (code->n_act_cols > 0) {
-            VnArgs va{d_llr, w.qbuf[(t - 1) & 1], w.qbuf[t & 1], w.t, d_hard, d_posterior, w.done,
-                      Z, tiles_vn, code->n, code->m, EZ};
+            VnLaunch vl{code->inline_ok ? &code->vn_inl : nullptr,
+                        VnTablesGlobal{code->d_pair, code->d_partner, code->d_gen, code->d_col},
+                        VnArgs{d_llr, w.qbuf[(t - 1) & 1], w.qbuf[t & 1], w.t, d_hard, d_posterior, w.done,
+                               Z, tiles1, code->n, code->m, EZ},
+                        grid_vn, st};
             const int pk = prof_begin(0, st);
-            const int rc = dispatch_vn(code, va, grid_vn, st);
-            if (rc != QCLDPC_OK) return rc;
+            code->launcher(vl);
             prof_end(pk, st);
             ++g_launches;
         }
