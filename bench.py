@@ -13,7 +13,7 @@ capacity, max 500 iterations, early stop per frame.  Metric: decoded Mbit/s = co
             every rank decodes its own 64 frames, value = all frames of all ranks / max time ("weak").
   e2e       the same through qcldpc_decode_host: pinned HOST buffers, H2D of LLRs + syndromes and D2H of hard bits,
             iteration counts and pass flags inside the timed region.
-  roofline  dominant kernel k_vn_pass: algorithmic bytes per launch (B_min of SURVEY.md §8(d) = 8*E_core + 4*n + m/8
+  roofline  dominant kernel k_pass: algorithmic bytes per launch (B_min of SURVEY.md §8(d) = 8*E_core + 4*n + m/8
             per live frame-iteration) / its average launch duration, measured with CUDA event pairs recorded on the
             decode stream inside the timed steps (qcldpc_profile_enable), against MEASURED_PEAKS.json's HBM copy rate.
   cpu_baseline  the CPU oracle as it stands on the host cores, on a bounded sample of the same workload.
@@ -41,7 +41,7 @@ from paper_1702_07740_b200 import workloads as W  # noqa: E402
 
 FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 NOMINAL_HBM_GBS = 8000.0       # north_star's "about 8 TB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per k_vn_pass launch from the committed `ncu --set full` capture
+# dram__bytes_read.sum + dram__bytes_write.sum per k_pass launch from the committed `ncu --set full` capture
 # (profiles/r01_vn_pass_full.md); None until a capture exists.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = None
 
@@ -179,7 +179,7 @@ def main():
     ap.add_argument("--frames", type=int, default=None, help="override frames per GPU (debug only)")
     ap.add_argument("--max-iter", type=int, default=None, help="override max iterations (debug only)")
     ap.add_argument("--ref-iters", type=int, default=8, help="iterations per oracle sample")
-    ap.add_argument("--profile-stride", type=int, default=4, help="time every k-th k_vn_pass launch")
+    ap.add_argument("--profile-stride", type=int, default=4, help="time every k-th k_pass launch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
@@ -293,8 +293,8 @@ def main():
 
     # ---------------------------------------------------------------------------------------------- roofline
     b_min, b_2ph = algorithmic_bytes(cfg.code)
-    vn_ms, vn_timed, vn_launched = prof["vn_pass"]
-    ck_ms, ck_timed, ck_launched = prof["check"]
+    vn_ms, vn_timed, vn_launched = prof["pass"]
+    ck_ms, ck_timed, ck_launched = prof["cand"]
     live_frame_iters = float(iters.sum())                         # per step: frames still live, summed over iterations
     launches = max(int(iters.max()), 1)
     live_per_launch = live_frame_iters / launches
@@ -302,15 +302,15 @@ def main():
     peak, peak_src = hbm_peak()
     achieved = (b_min * live_per_launch) / (vn_avg_ms * 1e-3) / 1e9 if vn_timed else None
     roofline = {
-        "bound": "hbm", "kernel": "k_vn_pass", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "bound": "hbm", "kernel": "k_pass", "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": (achieved / peak) if achieved else None, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
         "peak_source": peak_src, "bytes_model": "B_min = 8*E_core + 4*n + m/8 per live frame-iteration",
         "algorithmic_bytes_per_launch": b_min * live_per_launch, "avg_launch_ms": vn_avg_ms,
         "timed_launches": int(vn_timed), "launches": int(vn_launched),
         "frac_b2ph_of_peak": (b_2ph * live_per_launch) / (vn_avg_ms * 1e-3) / 1e9 / peak if vn_timed else None,
         "frac_bmin_of_8tbs": (achieved / NOMINAL_HBM_GBS) if achieved else None,
-        "check_kernel_avg_ms": (ck_ms / ck_timed) if ck_timed else None,
-        "vn_share_of_step": (vn_avg_ms * vn_launched / args.steps) / (ms_total / args.steps) if vn_timed else None,
+        "cand_kernel_avg_ms": (ck_ms / ck_timed) if ck_timed else None,
+        "pass_share_of_step": (vn_avg_ms * vn_launched / args.steps) / (ms_total / args.steps) if vn_timed else None,
     }
 
     if rank != 0:

@@ -96,8 +96,8 @@ int64_t qcldpc_last_launch_count(void);
 /*
  * Optional launch timing for roofline reports (bench.py).  qcldpc_profile_enable(stride) with stride > 0 makes the
  * following qcldpc_decode calls of this thread record a CUDA event pair, on the decode stream, around every
- * stride-th launch of the two per-iteration kernels (kind 0 = fused check/variable update k_vn_pass, kind 1 =
- * syndrome check k_check); stride = 0 switches it off.  qcldpc_profile_collect waits for the recorded events (host
+ * stride-th launch of the two per-iteration kernels (kind 0 = fused check/variable update k_pass, kind 1 =
+ * early-exit check k_cand); stride = 0 switches it off.  qcldpc_profile_collect waits for the recorded events (host
  * blocks until they have completed), returns for each kind the summed duration in ms of the timed launches, how many
  * were timed and how many were launched since enable/collect, and clears the record.  ms_sum, timed, launched:
  * HOST arrays of 2 entries.

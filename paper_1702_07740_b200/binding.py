@@ -82,12 +82,12 @@ def qcldpc_profile_enable(stride: int) -> None:
 
 
 def qcldpc_profile_collect():
-    """{kind: (ms_sum, timed, launched)} for kind in ("vn_pass", "check")."""
+    """{kind: (ms_sum, timed, launched)} for kind in ("pass", "cand")."""
     ms = (ctypes.c_double * 2)()
     timed = (ctypes.c_int64 * 2)()
     launched = (ctypes.c_int64 * 2)()
     _check(_lib.qcldpc_profile_collect(ms, timed, launched), "qcldpc_profile_collect")
-    return {name: (ms[k], timed[k], launched[k]) for k, name in enumerate(("vn_pass", "check"))}
+    return {name: (ms[k], timed[k], launched[k]) for k, name in enumerate(("pass", "cand"))}
 
 
 class DecodeResult(NamedTuple):
@@ -116,7 +116,7 @@ class QCLDPCCode:
 
     def __del__(self):
         h = getattr(self, "_handle", None)
-        if h:
+        if h and _lib is not None:          # _lib is None while the interpreter shuts down
             _lib.qcldpc_code_destroy(h)
             self._handle = None
 

@@ -10,69 +10,96 @@
 
 namespace qc {
 
-constexpr int kMaxDv = 64;       // largest supported active-column degree
-constexpr int kThreads = 128;    // threads per CTA in every kernel
+constexpr int kMaxDv = 64;          // largest supported active-column degree
+constexpr int kThreads = 128;       // threads per CTA in every kernel
+constexpr int kMaxV = 2;            // variables per thread in k_pass (tile = kThreads * V consecutive variables)
+constexpr int kHalo = kThreads * kMaxV;   // every cyclic run of Z floats is stored with this many wrapped copies behind it
+constexpr int kMaxPartners = 2048;  // partner entries (other edges of the gen rows) per active column
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kMsgMax2 = QCLDPC_MSG_MAX * kLog2e;   // the clamp S2 in log2 units
 
-// ---- code tables (built once by qcldpc_code_create) -----------------------------------------------------------
-// Active edge seen from its own variable.  Check index r = (i - shift) mod Z; static term at t[t_off + r].
-// If the row has exactly one other active edge ("pair row", every lower row of the BASELINE.json codes) that
-// partner's message sits at q[p_off + (i + delta) mod Z]; otherwise p_off = -1 and a GenDesc lists the partners.
-struct PairDesc { int shift; int t_off; int p_off; int delta; };
-struct GenDesc { int k; int pbeg; int np; int pad; };             // k: edge index inside the column
-struct PartnerDesc { int off; int delta; };                       // q[off + (i + delta) mod Z]
-struct ColDesc { int col; int ebeg; int dv; int gbeg; int ng; int pad0, pad1, pad2; };
-struct RowDesc { int ebeg; int ne; int abs_col; int abs_shift; }; // base row: active edges, absorbed column or -1
-struct RowEdge { int edge; int shift; int col; int pad; };        // active edge seen from its row
+// ---- layout -----------------------------------------------------------------------------------------------------
+// Messages live in base-2 units: L' = L * log2(e).  Edge state of active edge e = (c,v), variable index i:
+//     w[e * Zs + i] = sgn(L_vc) * 2^-|L'_vc|          (sign in the IEEE sign bit; S3: -0 never occurs)
+// Zs = round_up(Z + kHalo, 32): the run [0,Z) is followed by a copy of its first kHalo entries, so that a tile of
+// consecutive variables reads its cyclically shifted window [a, a + tile) with a < Z WITHOUT a per-element wrap.
+// Edges of "gen" rows (see below) carry the hard decision xhat_v of their variable in mantissa bit 0 (the reader
+// masks it off: the magnitude never depends on it).
+// Static per check c of base row R, index r:
+//     t[R * Zs + r] = (-1)^{s_c} * sgn(Q_j) * 2^-|Q'_j|   for the absorbed degree-1 variable j of c, or
+//                     (-1)^{s_c} * 0                       if the row has none                   (same halo).
 
-// Tables small enough travel as __grid_constant__ kernel parameters (constant bank, uniform loads); larger codes
-// read the same tables from global memory.
-constexpr int kInlEdges = 256, kInlPartners = 512, kInlCols = 32, kInlGen = 96, kInlRows = 128;
-struct VnTablesInline {
-    PairDesc pair[kInlEdges]; PartnerDesc partner[kInlPartners]; GenDesc gen[kInlGen]; ColDesc col[kInlCols];
-};
-struct VnTablesGlobal { const PairDesc* pair; const PartnerDesc* partner; const GenDesc* gen; const ColDesc* col; };
-struct CnTablesInline { RowDesc row[kInlRows]; RowEdge redge[kInlEdges]; };
-struct CnTablesGlobal { const RowDesc* row; const RowEdge* redge; };
+// ---- code tables (built once by qcldpc_code_create, read from global memory in each block's preamble) -----------
+// A base row is a PAIR row if it has an absorbed variable and exactly two active edges (every lower row of the
+// BASELINE.json codes); every other row is a GEN row.  Inside an active column the gen edges come first.
+struct EdgeDesc { int shift; int t_off; int p_off; int delta; };  // t at t[t_off + (i - shift) mod Z]; pair edge:
+                                                                  // partner at w[p_off + (i + delta) mod Z], else p_off = -1
+struct GenDesc { int pbeg; int np; int counter; int pad; };       // partners [pbeg, pbeg+np) relative to the column's
+                                                                  // first partner; counter: this edge reports the row's parity
+struct PartnerDesc { int off; int delta; };                       // w[off + (i + delta) mod Z]
+struct ColDesc { int col; int ebeg; int dv; int ng; int gbeg; int pbeg; int np; int pad; };
+struct RowDesc { int ebeg; int ne; int abs_col; int abs_shift; int gen; int pad0, pad1, pad2; };
+struct RowEdge { int edge; int shift; int col; int ca; };         // active edge seen from its row (ca = active column)
+
+struct PassTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc* partner; const ColDesc* col; };
+struct CheckTables { const RowDesc* row; const RowEdge* redge; };
 
 // ---- kernel arguments -------------------------------------------------------------------------------------------
-struct VnArgs {
-    const float* llr; const float* qold; float* qnew; const float* t; uint8_t* hard; float* post; const int* done;
-    int Z, tiles; int64_t n, m, EZ;
+struct PassArgs {
+    const float* llr;          // [F][n]
+    float* qb[3];              // the three edge-state buffers [F][E][Zs]
+    const float* t;            // [F][mb][Zs]
+    const uint8_t* hard_in;    // xhat of the input iteration, active columns only [F][A][Zs]
+    uint8_t* hard_out;
+    uint8_t* d_hard;           // FINAL: outputs
+    float* d_post;
+    const int* done;           // [F]
+    const int32_t* iters;      // [F]  (FINAL: the iteration whose decisions are formed)
+    int* topbad;               // [F]  slot of the input iteration: set to 1 if a parity of a row without absorbed variable fails
+    int in_buf, out_buf;       // regular pass: qb[in_buf] -> qb[out_buf]
+    int Z, Zs, tiles;
+    int64_t n, EZs, mZs, AZs;  // per-frame strides
 };
 
-struct VnLaunch {
-    const VnTablesInline* inl;    // host pointer, or nullptr -> use `glob`
-    VnTablesGlobal glob;
-    VnArgs args;
-    dim3 grid;
-    cudaStream_t stream;
-};
-using VnLauncher = void (*)(const VnLaunch&);
+struct PassLaunch { PassTables tab; PassArgs args; dim3 grid; cudaStream_t stream; int V; bool final_mode; };
+using PassLauncher = void (*)(const PassLaunch&);
 
-// ---- device helpers -----------------------------------------------------------------------------------------------
+// ---- device helpers ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-// q(L) = sgn(L) exp(-|L|); sgn(x) = -1 iff x < 0, so -0.0 counts as + (reading S3)
-__device__ __forceinline__ float q_of_llr(float L) {
-    const float q = ex2_approx(-fabsf(L) * kLog2e);
-    return __uint_as_float(__float_as_uint(q) | (L < 0.0f ? 0x80000000u : 0u));
+// LLR in base-2 units; "+ 0.0f" turns -0.0 into +0.0 so that the sign bit alone is "L < 0" from here on (S3)
+__device__ __forceinline__ float llr_to_log2(float Q) { return Q * kLog2e + 0.0f; }
+// w(L') = sgn(L') 2^-|L'|
+__device__ __forceinline__ float w_of(float L2) {
+    const float q = ex2_approx(-fabsf(L2));
+    return __uint_as_float(__float_as_uint(q) | (__float_as_uint(L2) & 0x80000000u));
 }
-// |m| = ln den - ln num, clamped (S2).  num = 0 -> +inf -> clamp.
+// |m'| = lg2 den - lg2 num, clamped (S2).  num = 0 -> +inf -> clamp.
 __device__ __forceinline__ float mag_of(float num, float den) {
-    return fminf(kLn2 * (lg2_approx(den) - lg2_approx(num)), QCLDPC_MSG_MAX);
+    return fminf(lg2_approx(den) - lg2_approx(num), kMsgMax2);
 }
-// (num/den) [+] a = (num + a den) / (den + a num): Moebius addition of q = exp(-|L|) values, fraction kept apart
+// (num/den) [+] a = (num + a den) / (den + a num): the check-node rule on q = 2^-|L'| values, fraction kept apart
 __device__ __forceinline__ void boxplus_acc(float a, float& num, float& den) {
     const float n2 = fmaf(a, den, num);
     den = fmaf(a, num, den);
     num = n2;
 }
+// base + boff bytes as ONE 32x32+64 multiply-add (IMAD.WIDE.U32 with multiplier 1; a multiplier of 4 is split by ptxas
+// into LEA + LEA.HI.X); boff is an unsigned byte offset < 2^32
+template <class T>
+__device__ __forceinline__ T* byte_ptr(T* base, unsigned boff) {
+    unsigned long long r;
+    asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(boff), "l"((unsigned long long)base));
+    return reinterpret_cast<T*>(r);
+}
 __device__ __forceinline__ unsigned sign_of(float x) { return __float_as_uint(x) & 0x80000000u; }
-__device__ __forceinline__ float with_sign(float mag, unsigned sg) { return __uint_as_float(__float_as_uint(mag) | sg); }
+// XOR, not OR: the approximate lg2/rcp can make a magnitude that should be +0 come out as -tiny, and the result must
+// stay an odd function of the signs (the syndrome <-> codeword equivalence is bit-exact, tests P5)
+__device__ __forceinline__ float with_sign(float mag, unsigned sg) { return __uint_as_float(__float_as_uint(mag) ^ sg); }
 #endif
 
 }  // namespace qc

@@ -1,42 +1,42 @@
 // libqcldpc -- B200 (sm_100a) flooding Sum-Product decoder for QC-LDPC codes in syndrome form.
 // C ABI: include/qcldpc.h.  Design notes: DESIGN.md.  Citations "P:NNN" are /root/reference/PAPER.md lines.
 //
-// Arithmetic domain.  Edge state is stored as  q_vc = sgn(L_vc) * exp(-|L_vc|)  (sign in the IEEE sign bit).
-// With tanh(|L|/2) = (1-q)/(1+q) the paper's check-node rule
+// Arithmetic domain.  Edge state is stored as  w_vc = sgn(L_vc) * 2^-|L'_vc|,  L' = L log2(e)  (sign in the IEEE sign
+// bit).  With tanh(|L|/2) = (1-q)/(1+q), q = e^-|L|, the paper's check-node rule
 //     |m_cv| = Phi^-1( sum_{v'} Phi(|L_v'c|) ) = 2 atanh( prod_{v'} tanh(|L_v'c|/2) )
 // becomes a Moebius ("velocity") addition of the q's,  q_a [+] q_b = (q_a + q_b) / (1 + q_a q_b),
 // and |m_cv| = -ln( [+]_{v' in N(c)\v} q_v'c ).  Keeping numerator and denominator apart,
-//     (num, den) <- (num + a*den, den + a*num),   |m_cv| = ln den - ln num,
+//     (num, den) <- (num + a*den, den + a*num),   |m'_cv| = lg2 den - lg2 num,
 // needs no division, no cancellation (all terms are >= 0) and one ex2 + two lg2 per edge and iteration.
 // Degree-1 variables that are absorbed into their row contribute a constant q, folded together with the
 // syndrome sign (-1)^{s_c} (reading S1) into one static float per check, t_c.
 //
-// Kernels (one thread per unit, frames on blockIdx.y so that the sweep is frame-major and a frame's working set
-// stays in the 126 MB L2 while it is being processed):
-//   k_init_q   a0  q^(0) = q(Q_v) on every active edge; hard/posterior of active variables at t = 0
-//   k_init_t   a0  t_c from the absorbed variable's LLR and the syndrome bit
-//   k_vn_pass  a1+a2  fused check-node + variable-node update, VN-centric: the thread of active variable v gathers,
-//              for each of its edges (c,v), the q of the OTHER edges of c (+ t_c), forms m_cv, then L_v, xhat_v and
-//              all L_vc by prefix/suffix sums (direct exclusion, no total-minus-self), and writes q^(t) (ping-pong)
-//   k_check    a3  check-centric: decides the absorbed degree-1 variables (L_j = Q_j + m_cj), xhat parity vs s_c,
-//              per-frame count of unsatisfied checks (integer atomics only); optional posterior write
-//   k_flags    a3  per-frame early exit: freezes d_iters / d_pass / done
+// Kernels:
+//   k_init_cols a0  w^(0) = w(Q_v) on every active edge (+ halo), decisions at t = 0 of the active variables
+//   k_init_rows a0  t_c from the absorbed variable's LLR and the syndrome bit (+ halo)
+//   k_pass      a1+a2  (pass_kernel.cuh) fused check-node + variable-node update of one iteration, VN-centric; also
+//               forms, from bit-0 tags, the parity of the rows WITHOUT absorbed variable at the previous iteration:
+//               a necessary condition for H xhat = s that costs no extra memory traffic
+//   k_cand      a3  early exit: for the frames that pass that filter, the full check (decisions of the absorbed
+//               variables L_j = Q_j + m_cj and every parity) on the still intact state of that iteration; persistent
+//               grid, returns at once when there is no candidate.  Freezes d_iters / d_pass / done per frame.
+//   k_pass<FINAL>, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
+// Edge state is triple-buffered: pass t reads w^(t-1) and writes w^(t) over w^(t-2), so that when the check of
+// iteration t-1 runs (after pass t), w^(t-2) -- the input of iteration t-1 -- is still there.
 #include "common.cuh"
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 namespace qc {
-// one object file per instantiation of k_vn_pass (vn_inst.cu)
-void launch_vn_dv8(const VnLaunch&);
-void launch_vn_dv11(const VnLaunch&);
-void launch_vn_dv16(const VnLaunch&);
-void launch_vn_dv21(const VnLaunch&);
-void launch_vn_dv32(const VnLaunch&);
-void launch_vn_dv64(const VnLaunch&);
+// one object file per instantiation family of k_pass (pass_inst.cu)
+void launch_pass_dv11_ng3(const PassLaunch&);
+void launch_pass_dv21_ng3(const PassLaunch&);
+void launch_pass_generic(const PassLaunch&);
 }  // namespace qc
 
 using namespace qc;
@@ -58,50 +58,55 @@ thread_local Profile g_prof;
 }  // namespace
 
 struct qcldpc_code {
-    int mb, nb, Z;
+    int mb, nb, Z, Zs, V, tiles;
     int64_t n, m;
-    int n_act_cols, n_act_edges, n_partners, max_dv, bucket;
-    bool uniform_dv, inline_ok;
-    std::vector<PairDesc> pair;
-    std::vector<PartnerDesc> partner;
+    int n_act_cols, n_act_edges, max_dv;
+    bool filter_rows;                     // some row has no absorbed variable (the early-exit filter exists)
+    std::vector<EdgeDesc> edge;
     std::vector<GenDesc> gen;
+    std::vector<PartnerDesc> partner;
     std::vector<ColDesc> col;
     std::vector<RowDesc> row;
     std::vector<RowEdge> redge;
-    // device copies
-    PairDesc* d_pair = nullptr; PartnerDesc* d_partner = nullptr; GenDesc* d_gen = nullptr; ColDesc* d_col = nullptr;
+    EdgeDesc* d_edge = nullptr; GenDesc* d_gen = nullptr; PartnerDesc* d_partner = nullptr; ColDesc* d_col = nullptr;
     RowDesc* d_row = nullptr; RowEdge* d_redge = nullptr;
-    VnTablesInline vn_inl; CnTablesInline cn_inl;
-    VnLauncher launcher = nullptr;
+    PassLauncher launcher = nullptr;
+    int n_sm = 148;
 };
 
 namespace {
 
 struct InitArgs {
-    const float* llr; const uint8_t* syn; float* q0; float* t; uint8_t* hard; float* post;
-    int Z, tiles; int64_t n, m, EZ;
+    const float* llr; const uint8_t* syn; float* q0; float* t; uint8_t* hard0; uint8_t* d_hard; float* d_post;
+    int Z, Zs, tiles; int64_t n, m, EZs, mZs, AZs;
 };
 
-// a0: q^(0) on every active edge, decisions at t = 0 for active variables
-template <class Tables>
-__global__ void __launch_bounds__(kThreads) k_init_q(const __grid_constant__ Tables tab, const InitArgs a) {
+// a0: w^(0) on every active edge, decisions at t = 0 for active variables.  One thread per (active column, index).
+__global__ void __launch_bounds__(kThreads) k_init_cols(const PassTables tab, const InitArgs a) {
     const int f = blockIdx.y;
     const int ca = blockIdx.x / a.tiles;
     const int i = (blockIdx.x - ca * a.tiles) * kThreads + threadIdx.x;
     if (i >= a.Z) return;
     const ColDesc cd = tab.col[ca];
-    const int64_t v = (int64_t)cd.col * a.Z + i;
-    const float Q = __ldg(a.llr + (int64_t)f * a.n + v);
-    const float q = q_of_llr(Q);
-    float* q0 = a.q0 + (int64_t)f * a.EZ;
-    for (int k = 0; k < cd.dv; ++k) q0[(int64_t)(cd.ebeg + k) * a.Z + i] = q;
-    a.hard[(int64_t)f * a.n + v] = Q < 0.0f ? 1 : 0;
-    if (a.post) a.post[(int64_t)f * a.n + v] = Q;
+    const int64_t v = (int64_t)f * a.n + (int64_t)cd.col * a.Z + i;
+    const float Q = __ldg(a.llr + v);
+    const float Q2 = llr_to_log2(Q);
+    const unsigned xh = __float_as_uint(Q2) >> 31;
+    const unsigned wb = __float_as_uint(w_of(Q2));
+    float* q0 = a.q0 + (int64_t)f * a.EZs + (int64_t)cd.ebeg * a.Zs;
+    const bool halo = i < kHalo;
+    for (int k = 0; k < cd.dv; ++k) {
+        const float w = __uint_as_float(k < cd.ng ? ((wb & 0xfffffffeu) | xh) : wb);
+        q0[(int64_t)k * a.Zs + i] = w;
+        if (halo) q0[(int64_t)k * a.Zs + a.Z + i] = w;
+    }
+    a.hard0[(int64_t)f * a.AZs + (int64_t)ca * a.Zs + i] = (uint8_t)xh;
+    a.d_hard[v] = (uint8_t)xh;
+    if (a.d_post) a.d_post[v] = Q;
 }
 
-// a0: t_c = (-1)^{s_c} sgn(Q_j) exp(-|Q_j|) for the absorbed variable j of check c, or (-1)^{s_c} * 0
-template <class Tables>
-__global__ void __launch_bounds__(kThreads) k_init_t(const __grid_constant__ Tables tab, const InitArgs a) {
+// a0: t_c = (-1)^{s_c} sgn(Q_j) 2^-|Q'_j| for the absorbed variable j of check c, or (-1)^{s_c} * 0
+__global__ void __launch_bounds__(kThreads) k_init_rows(const CheckTables tab, const InitArgs a) {
     const int f = blockIdx.y;
     const int R = blockIdx.x / a.tiles;
     const int r = (blockIdx.x - R * a.tiles) * kThreads + threadIdx.x;
@@ -111,88 +116,141 @@ __global__ void __launch_bounds__(kThreads) k_init_t(const __grid_constant__ Tab
     float t = 0.0f;
     if (rd.abs_col >= 0) {
         int j = r + rd.abs_shift; j -= (j >= a.Z) ? a.Z : 0;
-        t = q_of_llr(__ldg(a.llr + (int64_t)f * a.n + (int64_t)rd.abs_col * a.Z + j));
+        t = w_of(llr_to_log2(__ldg(a.llr + (int64_t)f * a.n + (int64_t)rd.abs_col * a.Z + j)));
     }
     const unsigned s = a.syn[(int64_t)f * a.m + c] & 1u;
-    a.t[(int64_t)f * a.m + c] = __uint_as_float(__float_as_uint(t) ^ (s << 31));
+    const float ts = __uint_as_float(__float_as_uint(t) ^ (s << 31));
+    float* tf = a.t + (int64_t)f * a.mZs + (int64_t)R * a.Zs;
+    tf[r] = ts;
+    if (r < kHalo) tf[a.Z + r] = ts;
 }
 
-struct CnArgs {
-    const float* llr; const uint8_t* syn; const float* qbuf0; const float* qbuf1; uint8_t* hard; float* post;
-    const int* done; const int32_t* iters; int* unsat;
-    int Z, tiles, t_fixed, count, skip_done; int64_t n, m, EZ;
+struct CheckArgs {
+    const float* llr; const uint8_t* syn;
+    const float* qb[3];
+    const uint8_t* hardbuf[2];   // candidate mode: xhat of iteration t in hardbuf[t & 1], active columns [F][A][Zs]
+    uint8_t* d_hard; float* d_post;
+    int* done; int32_t* iters; uint8_t* pass;
+    const int* topbad;           // slot of the iteration being checked
+    int* topbad_clear;           // the other slot
+    int* fullbad; int* unsat; unsigned* ticket;
+    int n_frames, mb, Z, Zs, tiles, t; int64_t n, m, EZs, AZs;
 };
 
-// a3: one thread per check: decision of the absorbed degree-1 variable, parity of the hard decisions against s_c
-template <class Tables>
-__global__ void __launch_bounds__(kThreads) k_check(const __grid_constant__ Tables tab, const CnArgs a) {
-    const int f = blockIdx.y;
-    if (a.skip_done && a.done[f]) return;
-    const int t = a.t_fixed >= 0 ? a.t_fixed : a.iters[f];  // iteration whose decisions are being formed
-    const int R = blockIdx.x / a.tiles;
-    const int r = (blockIdx.x - R * a.tiles) * kThreads + threadIdx.x;
+// a3: parity of check (R, r) of frame f for the decisions of iteration T: decides the absorbed degree-1 variable from
+// the messages of iteration T-1 (L_j = Q_j + m_cj), XORs the hard decisions against s_c.
+// FINAL: decisions of the active variables come from d_hard, the absorbed variable's outputs are written.
+template <bool FINAL>
+__device__ __forceinline__ unsigned check_one(const CheckTables& tab, const CheckArgs& a, int f, int R, int r, int T) {
+    const RowDesc rd = tab.row[R];
     const int Z = a.Z;
-    unsigned bad = 0;
-    if (r < Z) {
-        const RowDesc rd = tab.row[R];
-        // m^(t) is formed from the messages of iteration t-1: the buffer k_vn_pass(t) read from
-        const float* __restrict__ qprev = (((t - 1) & 1) ? a.qbuf1 : a.qbuf0) + (int64_t)f * a.EZ;
-        const uint8_t* hard = a.hard + (int64_t)f * a.n;
-        unsigned par = a.syn[(int64_t)f * a.m + (int64_t)R * Z + r] & 1u;
-        unsigned sg = par << 31;
-        float num = 0.0f, den = 1.0f;
-        for (int k = 0; k < rd.ne; ++k) {
-            const RowEdge re = tab.redge[rd.ebeg + k];
-            int iv = r + re.shift; iv -= (iv >= Z) ? Z : 0;
-            par ^= hard[(int64_t)re.col * Z + iv] & 1u;
-            if (rd.abs_col >= 0 && t > 0) {
-                const float qa = __ldg(qprev + (int64_t)re.edge * Z + iv);
-                sg ^= __float_as_uint(qa) & 0x80000000u;
-                boxplus_acc(fabsf(qa), num, den);
-            }
+    const float* __restrict__ qprev = a.qb[(T + 2) % 3] + (int64_t)f * a.EZs;     // w^(T-1)
+    unsigned par = a.syn[(int64_t)f * a.m + (int64_t)R * Z + r] & 1u;
+    unsigned sg = par << 31;
+    float num = 0.0f, den = 1.0f;
+    for (int k = 0; k < rd.ne; ++k) {
+        const RowEdge re = tab.redge[rd.ebeg + k];
+        int iv = r + re.shift; iv -= (iv >= Z) ? Z : 0;
+        if (FINAL) par ^= a.d_hard[(int64_t)f * a.n + (int64_t)re.col * Z + iv] & 1u;
+        else par ^= a.hardbuf[T & 1][(int64_t)f * a.AZs + (int64_t)re.ca * a.Zs + iv] & 1u;
+        if (rd.abs_col >= 0 && T > 0) {
+            unsigned wb = __float_as_uint(__ldg(qprev + (int64_t)re.edge * a.Zs + iv));
+            sg ^= wb & 0x80000000u;
+            wb &= rd.gen ? 0x7ffffffeu : 0x7fffffffu;         // gen edges carry a tag in bit 0
+            boxplus_acc(__uint_as_float(wb), num, den);
         }
-        if (rd.abs_col >= 0) {
-            int j = r + rd.abs_shift; j -= (j >= Z) ? Z : 0;
-            const int64_t v = (int64_t)f * a.n + (int64_t)rd.abs_col * Z + j;
-            const float Qj = __ldg(a.llr + v);
-            const float mcj = t > 0 ? __uint_as_float(__float_as_uint(mag_of(num, den)) | sg) : 0.0f;
-            const float Lj = Qj + mcj;                       // degree-1 variable: L_j = Q_j + m_cj
-            const unsigned xj = Lj < 0.0f ? 1u : 0u;
-            a.hard[v] = (uint8_t)xj;
-            if (a.post) a.post[v] = Lj;
-            par ^= xj;
+    }
+    if (rd.abs_col >= 0) {
+        int j = r + rd.abs_shift; j -= (j >= Z) ? Z : 0;
+        const int64_t v = (int64_t)f * a.n + (int64_t)rd.abs_col * Z + j;
+        const float Qj = __ldg(a.llr + v);
+        float Lj = llr_to_log2(Qj);
+        if (T > 0) Lj += with_sign(mag_of(num, den), sg);   // L'_j = Q'_j + m'_cj
+        const unsigned xj = __float_as_uint(Lj) >> 31;
+        if (FINAL) {
+            a.d_hard[v] = (uint8_t)xj;
+            if (a.d_post) a.d_post[v] = T > 0 ? Lj * kLn2 : Qj;
         }
-        bad = par;
+        par ^= xj;
     }
-    if (a.count) {
-        const int nbad = __syncthreads_count(bad != 0);
-        if (threadIdx.x == 0 && nbad) atomicAdd(a.unsat + f, nbad);
-    }
+    return par;
 }
 
-// a3: per-frame early exit.  mode 0: iteration t of an early-stop run; mode 1: final pass/fail of a fixed-length run
-__global__ void k_flags(int* done, int* unsat, int32_t* iters, uint8_t* pass, int n_frames, int t, int final_only) {
+// a4: one thread per check of every frame, on the frame's frozen state (iteration d_iters[f]); counts failed parities
+__global__ void __launch_bounds__(kThreads) k_check_final(const CheckTables tab, const CheckArgs a) {
+    const int f = blockIdx.y;
+    const int R = blockIdx.x / a.tiles;
+    const int r = (blockIdx.x - R * a.tiles) * kThreads + threadIdx.x;
+    unsigned bad = 0;
+    if (r < a.Z) bad = check_one<true>(tab, a, f, R, r, a.iters[f]);
+    const int nbad = __syncthreads_count(bad != 0);
+    if (threadIdx.x == 0 && nbad) atomicAdd(a.unsat + f, nbad);
+}
+
+__global__ void k_flags_final(int* unsat, uint8_t* pass, int n_frames) {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= n_frames) return;
-    if (final_only) {
-        pass[f] = unsat[f] == 0 ? 1 : 0;
-        iters[f] = t;
-    } else if (!done[f]) {
-        if (unsat[f] == 0) { done[f] = 1; iters[f] = t; pass[f] = 1; }
-    }
+    pass[f] = unsat[f] == 0 ? 1 : 0;
     unsat[f] = 0;
 }
 
-__global__ void k_reset(int* done, int* unsat, int32_t* iters, uint8_t* pass, int n_frames, int max_iter) {
+// a3: early exit for iteration t (runs after pass t+1).  Persistent grid.  A frame is a candidate if it is still live
+// and no row without absorbed variable failed its parity (topbad, formed by pass t+1 from the bit-0 tags).  Every
+// block walks the candidates in the same order; the last block to finish freezes the frames whose full check passed.
+__global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const CheckArgs a) {
+    __shared__ unsigned s_last;
+    const int units = a.mb * a.tiles;
+    if (blockIdx.x == 0)
+        for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.topbad_clear[f] = 0;
+    bool any = false;
+    for (int f0 = 0; f0 < a.n_frames; f0 += kThreads) {
+        const int f = f0 + threadIdx.x;
+        const int c = (f < a.n_frames && !a.done[f] && !a.topbad[f]) ? 1 : 0;
+        if (!__syncthreads_or(c)) continue;
+        any = true;
+        const int fend = min(f0 + kThreads, a.n_frames);
+        for (int g = f0; g < fend; ++g) {
+            if (a.done[g] || a.topbad[g]) continue;                      // block-uniform
+            for (int u = blockIdx.x; u < units; u += gridDim.x) {
+                // some block already found a failed parity of this frame: skip the rest of it
+                if (__syncthreads_or(threadIdx.x == 0 ? *((volatile int*)(a.fullbad + g)) : 0)) break;
+                const int R = u / a.tiles;
+                const int r = (u - R * a.tiles) * kThreads + threadIdx.x;
+                unsigned bad = 0;
+                if (r < a.Z) bad = check_one<false>(tab, a, g, R, r, a.t);
+                if (__syncthreads_or(bad != 0) && threadIdx.x == 0) a.fullbad[g] = 1;
+            }
+        }
+    }
+    if (!any) return;                                                    // the same decision in every block
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int f = threadIdx.x; f < a.n_frames; f += kThreads) {
+        if (!a.done[f] && !a.topbad[f]) {
+            if (*((volatile int*)(a.fullbad + f)) == 0) { a.done[f] = 1; a.iters[f] = a.t; a.pass[f] = 1; }
+            a.fullbad[f] = 0;
+        }
+    }
+    if (threadIdx.x == 0) *a.ticket = 0;
+}
+
+__global__ void k_reset(int* done, int* unsat, int* topbad2, int* fullbad, unsigned* ticket, int32_t* iters,
+                        uint8_t* pass, int n_frames, int max_iter) {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f == 0) *ticket = 0;
     if (f >= n_frames) return;
-    done[f] = 0; unsat[f] = 0; iters[f] = max_iter; pass[f] = 0;
+    done[f] = 0; unsat[f] = 0; topbad2[f] = 0; topbad2[n_frames + f] = 0; fullbad[f] = 0;
+    iters[f] = max_iter; pass[f] = 0;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
-// kind 0 = k_vn_pass, 1 = k_check.  Returns the pair index to close with prof_end, or -1.
+// kind 0 = k_pass, 1 = k_cand.  Returns the pair index to close with prof_end, or -1.
 int prof_begin(int kind, cudaStream_t st) {
     Profile& p = g_prof;
     if (p.stride <= 0) return -1;
@@ -225,7 +283,7 @@ int cuda_fail(cudaError_t e, const char* what) {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Workspace {
-    float* qbuf[2]; float* t; int* done; int* unsat;
+    float* qbuf[3]; float* t; uint8_t* hardbuf[2]; int* done; int* unsat; int* topbad; int* fullbad; unsigned* ticket;
     size_t bytes;
 };
 
@@ -233,41 +291,20 @@ Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
     Workspace w;
     char* p = static_cast<char*>(base);
     size_t off = 0;
-    const size_t qbytes = align_up((size_t)n_frames * code->n_act_edges * code->Z * sizeof(float), 256);
-    const size_t tbytes = align_up((size_t)n_frames * code->m * sizeof(float), 256);
+    const size_t qbytes = align_up((size_t)n_frames * code->n_act_edges * code->Zs * sizeof(float), 256);
+    const size_t tbytes = align_up((size_t)n_frames * code->mb * code->Zs * sizeof(float), 256);
+    const size_t hbytes = align_up((size_t)n_frames * code->n_act_cols * code->Zs, 256);
     const size_t fbytes = align_up((size_t)n_frames * sizeof(int), 256);
-    w.qbuf[0] = reinterpret_cast<float*>(p + off); off += qbytes;
-    w.qbuf[1] = reinterpret_cast<float*>(p + off); off += qbytes;
+    for (int b = 0; b < 3; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
     w.t = reinterpret_cast<float*>(p + off); off += tbytes;
+    for (int b = 0; b < 2; ++b) { w.hardbuf[b] = reinterpret_cast<uint8_t*>(p + off); off += hbytes; }
     w.done = reinterpret_cast<int*>(p + off); off += fbytes;
     w.unsat = reinterpret_cast<int*>(p + off); off += fbytes;
+    w.topbad = reinterpret_cast<int*>(p + off); off += 2 * fbytes;     // two slots of n_frames ints, contiguous
+    w.fullbad = reinterpret_cast<int*>(p + off); off += fbytes;
+    w.ticket = reinterpret_cast<unsigned*>(p + off); off += 256;
     w.bytes = off;
     return w;
-}
-
-// Register-array size used for a code: the exact degree when every active column has the same degree and a
-// specialisation exists (the BASELINE.json codes: 11 and 21), else the next bucket.
-int vn_bucket(int max_dv, bool uniform) {
-    if (uniform && (max_dv == 11 || max_dv == 21)) return max_dv;
-    const int buckets[] = {8, 16, 32, 64};
-    for (int b : buckets) if (max_dv <= b) return b;
-    return -1;
-}
-VnLauncher vn_launcher(int bucket) {
-    switch (bucket) {
-        case 8: return launch_vn_dv8;
-        case 11: return launch_vn_dv11;
-        case 16: return launch_vn_dv16;
-        case 21: return launch_vn_dv21;
-        case 32: return launch_vn_dv32;
-        case 64: return launch_vn_dv64;
-        default: return nullptr;
-    }
-}
-
-void launch_check(const qcldpc_code* code, const CnArgs& a, dim3 grid, cudaStream_t st) {
-    if (code->inline_ok) k_check<CnTablesInline><<<grid, kThreads, 0, st>>>(code->cn_inl, a);
-    else k_check<CnTablesGlobal><<<grid, kThreads, 0, st>>>(CnTablesGlobal{code->d_row, code->d_redge}, a);
 }
 
 }  // namespace
@@ -286,45 +323,55 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
     qcldpc_code* code = new (std::nothrow) qcldpc_code();
     if (!code) return QCLDPC_ERR_ALLOC;
     code->mb = mb; code->nb = nb; code->Z = Z;
+    code->Zs = (int)align_up((size_t)Z + kHalo, 32);
     code->n = (int64_t)nb * Z; code->m = (int64_t)mb * Z;
+    const int Zs = code->Zs;
+    auto cell = [&](int R, int C) { return base[(size_t)R * nb + C]; };
 
     // column degrees; absorb at most one degree-1 column per row (the lowest-numbered one)
-    std::vector<int> deg(nb, 0), absorbed_by(nb, -1);
+    std::vector<int> deg(nb, 0), absorbed_by(nb, -1), n_active(mb, 0);
     for (int R = 0; R < mb; ++R)
-        for (int C = 0; C < nb; ++C) deg[C] += base[(size_t)R * nb + C] >= 0;
-    code->row.assign(mb, RowDesc{0, 0, -1, 0});
+        for (int C = 0; C < nb; ++C) deg[C] += cell(R, C) >= 0;
+    code->row.assign(mb, RowDesc{0, 0, -1, 0, 0, 0, 0, 0});
     for (int R = 0; R < mb; ++R)
         for (int C = 0; C < nb; ++C)
-            if (base[(size_t)R * nb + C] >= 0 && deg[C] == 1 && code->row[R].abs_col < 0) {
+            if (cell(R, C) >= 0 && deg[C] == 1 && code->row[R].abs_col < 0) {
                 code->row[R].abs_col = C;
-                code->row[R].abs_shift = base[(size_t)R * nb + C];
+                code->row[R].abs_shift = cell(R, C);
                 absorbed_by[C] = R;
             }
-    // active columns and their edges, in increasing (column, row) order
-    struct HostEdge { int shift, row, col_k; };
+    for (int R = 0; R < mb; ++R)
+        for (int C = 0; C < nb; ++C) n_active[R] += (cell(R, C) >= 0 && absorbed_by[C] < 0);
+    code->filter_rows = false;
+    for (int R = 0; R < mb; ++R) {
+        code->row[R].gen = !(code->row[R].abs_col >= 0 && n_active[R] == 2);
+        code->filter_rows = code->filter_rows || (code->row[R].abs_col < 0 && n_active[R] > 0);
+    }
+
+    // active columns and their edges: column by column, gen edges first, then pair edges, each in row order
+    struct HostEdge { int shift, row; };
     std::vector<HostEdge> edges;
-    std::vector<int> edge_of_cell((size_t)mb * nb, -1);
+    std::vector<int> edge_of_cell((size_t)mb * nb, -1), act_index(nb, -1);
     code->max_dv = 0;
-    bool uniform = true;
-    int first_dv = -1;
     for (int C = 0; C < nb; ++C) {
         if (absorbed_by[C] >= 0) continue;
         ColDesc cd{C, (int)edges.size(), 0, 0, 0, 0, 0, 0};
-        for (int R = 0; R < mb; ++R) {
-            const int p = base[(size_t)R * nb + C];
-            if (p < 0) continue;
-            edge_of_cell[(size_t)R * nb + C] = (int)edges.size();
-            edges.push_back(HostEdge{p, R, cd.dv});
-            ++cd.dv;
-        }
+        for (int pass = 0; pass < 2; ++pass)
+            for (int R = 0; R < mb; ++R) {
+                if (cell(R, C) < 0 || (code->row[R].gen != 0) != (pass == 0)) continue;
+                edge_of_cell[(size_t)R * nb + C] = (int)edges.size();
+                edges.push_back(HostEdge{cell(R, C), R});
+                ++cd.dv;
+                cd.ng += pass == 0;
+            }
+        act_index[C] = (int)code->col.size();
         code->col.push_back(cd);
         code->max_dv = std::max(code->max_dv, cd.dv);
-        if (first_dv < 0) first_dv = cd.dv;
-        uniform = uniform && cd.dv == first_dv;
     }
     code->n_act_cols = (int)code->col.size();
     code->n_act_edges = (int)edges.size();
-    if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Z >= ((int64_t)1 << 31)) {
+    if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Zs >= ((int64_t)1 << 31) ||
+        (int64_t)mb * Zs >= ((int64_t)1 << 31)) {
         delete code;
         return QCLDPC_ERR_UNSUPPORTED;
     }
@@ -333,57 +380,58 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
         code->row[R].ebeg = (int)code->redge.size();
         for (int C = 0; C < nb; ++C) {
             const int e = edge_of_cell[(size_t)R * nb + C];
-            if (e >= 0) code->redge.push_back(RowEdge{e, base[(size_t)R * nb + C], C, 0});
+            if (e >= 0) code->redge.push_back(RowEdge{e, cell(R, C), C, act_index[C]});
         }
         code->row[R].ne = (int)code->redge.size() - code->row[R].ebeg;
     }
-    // per edge: the pair descriptor; rows with 0 or >= 2 other active edges get a partner list (GenDesc)
-    for (size_t ci = 0; ci < code->col.size(); ++ci) {
-        ColDesc& cd = code->col[ci];
+    // per edge: where its partners are
+    bool partners_ok = true;
+    int max_np = 0;
+    for (ColDesc& cd : code->col) {
         cd.gbeg = (int)code->gen.size();
+        cd.pbeg = (int)code->partner.size();
         for (int k = 0; k < cd.dv; ++k) {
             const int e = cd.ebeg + k;
             const HostEdge& he = edges[e];
             const RowDesc& rd = code->row[he.row];
-            PairDesc pd{he.shift, he.row * Z, -1, 0};
-            const int np = rd.ne - 1;
-            if (np == 1) {
+            EdgeDesc ed{he.shift, he.row * Zs, -1, 0};
+            if (!rd.gen) {
                 for (int j = 0; j < rd.ne; ++j) {
                     const RowEdge& re = code->redge[rd.ebeg + j];
                     if (re.edge == e) continue;
-                    pd.p_off = re.edge * Z;
-                    pd.delta = ((re.shift - he.shift) % Z + Z) % Z;
+                    ed.p_off = re.edge * Zs;
+                    ed.delta = ((re.shift - he.shift) % Z + Z) % Z;
                 }
             } else {
-                GenDesc gd{k, (int)code->partner.size(), np, 0};
+                GenDesc gd{(int)code->partner.size() - cd.pbeg, rd.ne - 1, 0, 0};
+                gd.counter = (rd.abs_col < 0 && code->redge[rd.ebeg].edge == e) ? 1 : 0;
                 for (int j = 0; j < rd.ne; ++j) {
                     const RowEdge& re = code->redge[rd.ebeg + j];
                     if (re.edge == e) continue;
-                    code->partner.push_back(PartnerDesc{re.edge * Z, ((re.shift - he.shift) % Z + Z) % Z});
+                    code->partner.push_back(PartnerDesc{re.edge * Zs, ((re.shift - he.shift) % Z + Z) % Z});
                 }
                 code->gen.push_back(gd);
             }
-            code->pair.push_back(pd);
+            code->edge.push_back(ed);
         }
-        cd.ng = (int)code->gen.size() - cd.gbeg;
+        cd.np = (int)code->partner.size() - cd.pbeg;
+        max_np = std::max(max_np, cd.np);
+        partners_ok = partners_ok && cd.np <= kMaxPartners;
     }
-    code->n_partners = (int)code->partner.size();
-    code->uniform_dv = uniform && code->n_act_cols > 0;
-    code->bucket = vn_bucket(code->max_dv, code->uniform_dv);
-    code->launcher = vn_launcher(code->bucket);
-    code->inline_ok = code->n_act_edges <= kInlEdges && code->n_partners <= kInlPartners &&
-                      code->n_act_cols <= kInlCols && (int)code->gen.size() <= kInlGen && mb <= kInlRows;
-    if (code->inline_ok) {
-        memset(&code->vn_inl, 0, sizeof(code->vn_inl));
-        memset(&code->cn_inl, 0, sizeof(code->cn_inl));
-        std::copy(code->pair.begin(), code->pair.end(), code->vn_inl.pair);
-        std::copy(code->partner.begin(), code->partner.end(), code->vn_inl.partner);
-        std::copy(code->gen.begin(), code->gen.end(), code->vn_inl.gen);
-        std::copy(code->col.begin(), code->col.end(), code->vn_inl.col);
-        std::copy(code->row.begin(), code->row.end(), code->cn_inl.row);
-        std::copy(code->redge.begin(), code->redge.end(), code->cn_inl.redge);
+    if (!partners_ok) { delete code; return QCLDPC_ERR_UNSUPPORTED; }
+
+    // kernel choice: exact instantiations for the column shapes of the BASELINE.json codes, else the generic one
+    bool uniform = code->n_act_cols > 0;
+    for (const ColDesc& cd : code->col) uniform = uniform && cd.dv == code->col[0].dv && cd.ng == code->col[0].ng;
+    code->launcher = launch_pass_generic;
+    code->V = 1;
+    if (uniform && max_np <= 128 && code->col[0].ng == 3 && (code->col[0].dv == 11 || code->col[0].dv == 21)) {
+        code->launcher = code->col[0].dv == 11 ? launch_pass_dv11_ng3 : launch_pass_dv21_ng3;
+        const char* v = getenv("QCLDPC_V");                  // tuning knob: variables per thread (1 or 2)
+        if (v && atoi(v) == 2) code->V = 2;
     }
-    // device copies (always made: the init kernels and large codes read them from global memory)
+    code->tiles = (Z + kThreads * code->V - 1) / (kThreads * code->V);
+
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
         const size_t bytes = std::max<size_t>(vec.size(), 1) * sizeof(vec[0]);
         cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dptr), bytes);
@@ -391,12 +439,15 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
         if (!vec.empty()) e = cudaMemcpy(*dptr, vec.data(), vec.size() * sizeof(vec[0]), cudaMemcpyHostToDevice);
         return e;
     };
-    cudaError_t e = upload(code->pair, &code->d_pair);
-    if (e == cudaSuccess) e = upload(code->partner, &code->d_partner);
+    cudaError_t e = upload(code->edge, &code->d_edge);
     if (e == cudaSuccess) e = upload(code->gen, &code->d_gen);
+    if (e == cudaSuccess) e = upload(code->partner, &code->d_partner);
     if (e == cudaSuccess) e = upload(code->col, &code->d_col);
     if (e == cudaSuccess) e = upload(code->row, &code->d_row);
     if (e == cudaSuccess) e = upload(code->redge, &code->d_redge);
+    int dev = 0;
+    if (e == cudaSuccess) e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&code->n_sm, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) { qcldpc_code_destroy(code); return cuda_fail(e, "qcldpc_code_create: table upload"); }
     *out_code = code;
     return QCLDPC_OK;
@@ -404,7 +455,7 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
 
 void qcldpc_code_destroy(qcldpc_code_t* code) {
     if (!code) return;
-    cudaFree(code->d_pair); cudaFree(code->d_partner); cudaFree(code->d_gen); cudaFree(code->d_col);
+    cudaFree(code->d_edge); cudaFree(code->d_gen); cudaFree(code->d_partner); cudaFree(code->d_col);
     cudaFree(code->d_row); cudaFree(code->d_redge);
     delete code;
 }
@@ -433,62 +484,64 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
         return QCLDPC_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const Workspace w = carve(code, n_frames, d_workspace);
-    const int Z = code->Z;
-    const int64_t EZ = (int64_t)code->n_act_edges * Z;
+    const int Z = code->Z, Zs = code->Zs;
+    const int64_t EZs = (int64_t)code->n_act_edges * Zs, mZs = (int64_t)code->mb * Zs;
+    const int64_t AZs = (int64_t)code->n_act_cols * Zs;
     const int tiles1 = (Z + kThreads - 1) / kThreads;
     const int fblocks = (n_frames + 127) / 128;
+    const PassTables ptab{code->d_edge, code->d_gen, code->d_partner, code->d_col};
+    const CheckTables ctab{code->d_row, code->d_redge};
 
-    k_reset<<<fblocks, 128, 0, st>>>(w.done, w.unsat, d_iters, d_pass, n_frames, max_iter);
+    k_reset<<<fblocks, 128, 0, st>>>(w.done, w.unsat, w.topbad, w.fullbad, w.ticket, d_iters, d_pass, n_frames, max_iter);
     ++g_launches;
-    InitArgs ia{d_llr, d_syndrome, w.qbuf[0], w.t, d_hard, d_posterior, Z, tiles1, code->n, code->m, EZ};
+    const InitArgs ia{d_llr, d_syndrome, w.qbuf[0], w.t, w.hardbuf[0], d_hard, d_posterior,
+                      Z, Zs, tiles1, code->n, code->m, EZs, mZs, AZs};
     if (code->n_act_cols > 0) {
-        k_init_q<VnTablesGlobal><<<dim3(tiles1 * code->n_act_cols, n_frames), kThreads, 0, st>>>(
-            VnTablesGlobal{code->d_pair, code->d_partner, code->d_gen, code->d_col}, ia);
+        k_init_cols<<<dim3(tiles1 * code->n_act_cols, n_frames), kThreads, 0, st>>>(ptab, ia);
         ++g_launches;
     }
-    k_init_t<CnTablesGlobal><<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(
-        CnTablesGlobal{code->d_row, code->d_redge}, ia);
+    k_init_rows<<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(ctab, ia);
     ++g_launches;
 
-    const dim3 grid_vn(tiles1 * code->n_act_cols, n_frames);
-    if (code->n_act_cols > 0 && !code->launcher) return QCLDPC_ERR_UNSUPPORTED;
-    const dim3 grid_cn(tiles1 * code->mb, n_frames);
-    CnArgs ca{d_llr, d_syndrome, w.qbuf[0], w.qbuf[1], d_hard, nullptr, w.done, d_iters, w.unsat,
-              Z, tiles1, 0, 1, 1, code->n, code->m, EZ};
+    PassLaunch pl{ptab,
+                  PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
+                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, code->n, EZs, mZs, AZs},
+                  dim3(code->tiles * code->n_act_cols, n_frames), st, code->V, false};
+    CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
+                 d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
+                 n_frames, code->mb, Z, Zs, tiles1, 0, code->n, code->m, EZs, AZs};
+    const int cand_blocks = std::max(1, std::min(code->n_sm * 4, code->mb * tiles1));
 
     for (int t = 1; t <= max_iter; ++t) {
         if (code->n_act_cols > 0) {
-            VnLaunch vl{code->inline_ok ? &code->vn_inl : nullptr,
-                        VnTablesGlobal{code->d_pair, code->d_partner, code->d_gen, code->d_col},
-                        VnArgs{d_llr, w.qbuf[(t - 1) & 1], w.qbuf[t & 1], w.t, d_hard, d_posterior, w.done,
-                               Z, tiles1, code->n, code->m, EZ},
-                        grid_vn, st};
+            pl.args.in_buf = (t - 1) % 3; pl.args.out_buf = t % 3;
+            pl.args.hard_in = w.hardbuf[(t - 1) & 1]; pl.args.hard_out = w.hardbuf[t & 1];
+            pl.args.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
             const int pk = prof_begin(0, st);
-            code->launcher(vl);
+            code->launcher(pl);
             prof_end(pk, st);
             ++g_launches;
         }
-        if (early_stop) {
-            ca.t_fixed = t;
+        if (early_stop && t >= 2) {
+            // early exit for iteration t-1: its filter bits were formed by pass t, its input state w^(t-2) is intact
+            ca.t = t - 1;
+            ca.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
+            ca.topbad_clear = w.topbad + (size_t)(t & 1) * n_frames;
             const int pk = prof_begin(1, st);
-            launch_check(code, ca, grid_cn, st);
+            k_cand<<<cand_blocks, kThreads, 0, st>>>(ctab, ca);
             prof_end(pk, st);
-            k_flags<<<fblocks, 128, 0, st>>>(w.done, w.unsat, d_iters, d_pass, n_frames, t, 0);
-            g_launches += 2;
+            ++g_launches;
         }
     }
-    if (!early_stop || max_iter == 0) {
-        // fixed-length run: one check of the final decisions gives d_pass (and the absorbed variables' outputs)
-        ca.t_fixed = max_iter; ca.post = d_posterior; ca.skip_done = 0;
-        launch_check(code, ca, grid_cn, st);
-        k_flags<<<fblocks, 128, 0, st>>>(w.done, w.unsat, d_iters, d_pass, n_frames, max_iter, 1);
-        g_launches += 2;
-    } else if (d_posterior) {
-        // early-stop run: posteriors of the absorbed variables from each frame's frozen state (iteration d_iters[f])
-        ca.t_fixed = -1; ca.post = d_posterior; ca.skip_done = 0; ca.count = 0;
-        launch_check(code, ca, grid_cn, st);
+    // outputs from each frame's frozen state: iteration d_iters[f] (= max_iter for the frames that did not stop)
+    if (code->n_act_cols > 0 && max_iter > 0) {
+        pl.final_mode = true;
+        code->launcher(pl);
         ++g_launches;
     }
+    k_check_final<<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(ctab, ca);
+    k_flags_final<<<fblocks, 128, 0, st>>>(w.unsat, d_pass, n_frames);
+    g_launches += 2;
     CUDA_TRY(cudaGetLastError());
     return QCLDPC_OK;
 }
