@@ -46,6 +46,26 @@ NOMINAL_HBM_GBS = 8000.0       # north_star's "about 8 TB/s"
 NCU_TRAFFIC_BYTES_PER_LAUNCH = None
 
 
+def decoded_mbit_per_s(block_length_bits: float, n_frames: float, seconds: float) -> float:
+    """The metric: raw decode throughput in coded Mbit/s = block length x frames / time (Eq. 17: for one frame
+    time = latency per iteration x iterations).  Pinned to Table II's printed numbers in tests/test_golden.py."""
+    return block_length_bits * n_frames / seconds / 1e6
+
+
+def rank_seed_base(cfg_index: int, rank: int) -> int:
+    """Replicas: every rank decodes its own frames of the same code."""
+    return W.frame_seed_base(cfg_index) + 100000 * rank
+
+
+def max_over_ranks(values_ms, dist, device):
+    """Element-wise MAX of per-rank times over all ranks (dist = torch.distributed or None for one process)."""
+    import torch
+    t = torch.tensor(list(values_ms), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
 def algorithmic_bytes(cfg_code: W.CodeSpec):
     """Per frame-iteration: B_min = 8*E_core + 4*n + m/8, B_2ph = 16*E_core + 4*n + m/8."""
     e_core = cfg_code.n_core * (cfg_code.top_deg + cfg_code.low_deg) * cfg_code.Z
@@ -131,7 +151,7 @@ def oracle_sample(cfg: W.Config, base, Z, sigma, seed_base, sample_iters: int):
     frame_iters = float(res.iters.sum())
     sec_per_frame_iter_all_cores = dt / max(frame_iters, 1.0)      # wall seconds per frame-iteration, all cores busy
     # full decode of this workload runs max_iter iterations per frame (frames stall)
-    mbit = cfg.code.n / (sec_per_frame_iter_all_cores * cfg.max_iter) / 1e6
+    mbit = decoded_mbit_per_s(cfg.code.n, 1, sec_per_frame_iter_all_cores * cfg.max_iter)
     desc = (f"{frames_n} frames x {sample_iters} of {cfg.max_iter} iterations of the same workload "
             f"(one frame per thread, H construction included), scaled linearly to {cfg.max_iter} iterations")
     return mbit, frames_n, desc, dt
@@ -178,7 +198,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (4 = headline batched workload)")
     ap.add_argument("--frames", type=int, default=None, help="override frames per GPU (debug only)")
     ap.add_argument("--max-iter", type=int, default=None, help="override max iterations (debug only)")
-    ap.add_argument("--ref-iters", type=int, default=8, help="iterations per oracle sample")
+    ap.add_argument("--ref-iters", type=int, default=40, help="iterations per oracle sample")
     ap.add_argument("--profile-stride", type=int, default=4, help="time every k-th k_pass launch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -194,7 +214,7 @@ def main():
     base = W.make_base_matrix(cfg.code)
     Z = cfg.code.Z
     sigma = W.sigma_for_gap(cfg.code.rate, cfg.gaps_db[0])
-    seed_base = W.frame_seed_base(cfg.index) + 100000 * rank     # every rank decodes its own frames
+    seed_base = rank_seed_base(cfg.index, rank)
 
     if args.impl == "reference":
         run_reference(args, cfg, base, Z, sigma, seed_base, rank, world)
@@ -282,14 +302,10 @@ def main():
     assert np.array_equal(h_out.iters.numpy(), iters)
 
     # ---------------------------------------------------------------------------------------------- reduce over ranks
-    times = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(times[0]), float(times[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], dist, dev)
 
-    bits_per_step = float(F) * n * world
-    value = bits_per_step * args.steps / (ms_total * 1e-3) / 1e6
-    e2e_value = bits_per_step * e2e_steps / (ms_e2e * 1e-3) / 1e6
+    value = decoded_mbit_per_s(n, F * world * args.steps, ms_total * 1e-3)
+    e2e_value = decoded_mbit_per_s(n, F * world * e2e_steps, ms_e2e * 1e-3)
 
     # ---------------------------------------------------------------------------------------------- roofline
     b_min, b_2ph = algorithmic_bytes(cfg.code)
