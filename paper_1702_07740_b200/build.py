@@ -19,6 +19,7 @@ HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh
            os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
 # (symbol, DV, NG, EXACT): EXACT = every active column has degree DV with NG gen edges (the BASELINE.json codes:
 # 11 or 21 edges, 3 of them into the top rows); the generic instantiation takes any column of degree <= 64
+PCAP = int(os.environ.get("QCLDPC_PCAP", "4"))   # partner slots per gen edge held in registers (tuning knob)
 PASS_INSTANCES = [("launch_pass_dv11_ng3", 11, 3, 1), ("launch_pass_dv21_ng3", 21, 3, 1),
                   ("launch_pass_generic", 64, 64, 0)]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -29,7 +30,8 @@ def _units():
     units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), [])]
     for name, dv, ng, exact in PASS_INSTANCES:
         units.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJDIR, f"{name}.o"),
-                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_EXACT={exact}"]))
+                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={PCAP}",
+                       f"-DPASS_EXACT={exact}"]))
     return units
 
 

@@ -5,7 +5,9 @@
 // of check c from the previous iteration, plus the static term t_c.  Both are cyclic runs in i; thanks to the halo
 // behind every run (common.cuh) the window a tile reads is contiguous, so its start is block-uniform: the preamble
 // computes it once per edge into shared memory and the per-thread cost of an access is one 64-bit multiply-add.
-//   phase 1  every load of the pair rows, back to back (2*dv*V independent loads in flight per thread)
+//   phase 1  every load, back to back: the partners of the gen rows (EXACT: NG x PCAP predicated slots per thread, so
+//            that they are in flight together with everything else instead of one dependent round trip per gen
+//            edge), t of every row, the partner of every pair row
 //   phase 2  gen rows (the few rows that are not "two active edges + one absorbed variable"): fold the partners into
 //            one equivalent q; the row's counter edge also forms the parity of the PREVIOUS iteration's hard
 //            decisions from the bit-0 tags (rows without absorbed variable only: the cheap early-exit filter)
@@ -19,15 +21,17 @@
 
 namespace qc {
 
-template <bool EXACT> struct PassCaps { static constexpr int kPartners = EXACT ? 128 : kMaxPartners; };
-
-template <int DV, int NG, bool EXACT, int V, bool FINAL>
+// EXACT: every active column has DV edges, the first NG of them gen edges; the first PCAP partners of each gen edge
+// sit in fixed (compile-time) slots, the rare rest (row degree > PCAP + 1) is folded in a slow loop afterwards.
+template <int DV, int NG, int PCAP, bool EXACT, int V, bool FINAL>
 __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const PassArgs a) {
     constexpr int UNR = EXACT ? DV : 1;
-    constexpr int UNG = EXACT ? (NG > 0 ? NG : 1) : 1;
+    constexpr int NGS = NG > 0 ? NG : 1;
+    constexpr int UNG = EXACT ? NGS : 1;
+    static_assert(!EXACT || NGS * PCAP <= kThreads, "one preamble thread per partner slot");
     __shared__ int2 s_eo[DV];
-    __shared__ GenDesc s_gd[NG > 0 ? NG : 1];
-    __shared__ int s_po[PassCaps<EXACT>::kPartners];
+    __shared__ GenDesc s_gd[NGS];
+    __shared__ int s_po[EXACT ? NGS * PCAP : kMaxPartners];
 
     const int f = blockIdx.y;
     int in_buf;
@@ -57,11 +61,25 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
         s_eo[tid] = make_int2(qo < 0 ? -1 : 4 * qo, 4 * (d.t_off + r0));    // byte offsets
     }
     if (tid < ng) s_gd[tid] = tab.gen[cd.gbeg + tid];
+    if (EXACT) {
+        if (tid < NG * PCAP) {                               // slot (g, jj): partner jj of gen edge g, or -1
+            const int g = tid / PCAP, jj = tid - g * PCAP;
+            const GenDesc gd = tab.gen[cd.gbeg + g];
+            int po = -1;
+            if (jj < gd.np) {
+                const PartnerDesc p = tab.partner[cd.pbeg + gd.pbeg + jj];
+                int x = i0 + p.delta; x -= (x >= Z) ? Z : 0;
+                po = 4 * (p.off + x);
+            }
+            s_po[tid] = po;
+        }
+    } else {
 #pragma unroll 1
-    for (int j = tid; j < cd.np; j += kThreads) {
-        const PartnerDesc p = tab.partner[cd.pbeg + j];
-        int x = i0 + p.delta; x -= (x >= Z) ? Z : 0;
-        s_po[j] = 4 * (p.off + x);
+        for (int j = tid; j < cd.np; j += kThreads) {
+            const PartnerDesc p = tab.partner[cd.pbeg + j];
+            int x = i0 + p.delta; x -= (x >= Z) ? Z : 0;
+            s_po[j] = 4 * (p.off + x);
+        }
     }
     __syncthreads();
 
@@ -78,7 +96,20 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
         xb[v] = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] : 0u;
     }
 
-    // phase 1: all loads of the pair rows (and t of every row)
+    // phase 1: all loads.  Gen partners first (EXACT: fixed slots, predicated off where the row is shorter)
+    float pw[EXACT ? NGS : 1][EXACT ? PCAP : 1][V];
+    if (EXACT) {
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+#pragma unroll
+            for (int j = 0; j < PCAP; ++j) {
+                const int po = s_po[g * PCAP + j];
+#pragma unroll
+                for (int v = 0; v < V; ++v)
+                    pw[g][j][v] = (po != -1) ? __ldg(byte_ptr(qP, po) + v * kThreads) : 0.0f;
+            }
+        }
+    }
     float tv[DV][V], wv[DV][V];
 #pragma unroll UNR
     for (int k = 0; k < (EXACT ? DV : dv); ++k) {
@@ -101,14 +132,38 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
         unsigned xa[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) { num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
-#pragma unroll 4
-        for (int j = 0; j < gd.np; ++j) {
-            const int po = s_po[gd.pbeg + j];
+        if (EXACT) {
+            // an empty slot holds +0.0: the identity of both the XOR and the fold
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-                const unsigned wb = __float_as_uint(__ldg(byte_ptr(qP, po) + v * kThreads));
-                xa[v] ^= wb;
-                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+            for (int j = 0; j < PCAP; ++j) {
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const unsigned wb = __float_as_uint(pw[EXACT ? g : 0][EXACT ? j : 0][v]);
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
+            }
+#pragma unroll 1
+            for (int j = PCAP; j < gd.np; ++j) {             // rows of degree > PCAP + 1: rare, slow path
+                const PartnerDesc p = tab.partner[cd.pbeg + gd.pbeg + j];
+                int x = i0 + p.delta; x -= (x >= Z) ? Z : 0;
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const unsigned wb = __float_as_uint(__ldg(qP + p.off + x + v * kThreads));
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
+            }
+        } else {
+#pragma unroll 4
+            for (int j = 0; j < gd.np; ++j) {
+                const int po = s_po[gd.pbeg + j];
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const unsigned wb = __float_as_uint(__ldg(byte_ptr(qP, po) + v * kThreads));
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
             }
         }
 #pragma unroll
@@ -182,14 +237,14 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
     }
 }
 
-template <int DV, int NG, bool EXACT>
+template <int DV, int NG, int PCAP, bool EXACT>
 void launch_pass(const PassLaunch& L) {
     if (L.V == 2 && EXACT) {
-        if (L.final_mode) k_pass<DV, NG, EXACT, 2, true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
-        else k_pass<DV, NG, EXACT, 2, false><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
+        if (L.final_mode) k_pass<DV, NG, PCAP, EXACT, 2, true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
+        else k_pass<DV, NG, PCAP, EXACT, 2, false><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
     } else {
-        if (L.final_mode) k_pass<DV, NG, EXACT, 1, true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
-        else k_pass<DV, NG, EXACT, 1, false><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
+        if (L.final_mode) k_pass<DV, NG, PCAP, EXACT, 1, true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
+        else k_pass<DV, NG, PCAP, EXACT, 1, false><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
     }
 }
 
