@@ -41,9 +41,9 @@ from paper_1702_07740_b200 import workloads as W  # noqa: E402
 
 FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 NOMINAL_HBM_GBS = 8000.0       # north_star's "about 8 TB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per k_pass launch from the committed `ncu --set full` capture
-# (profiles/r01_vn_pass_full.md); None until a capture exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum per k_pass launch on config 4 (64 live frames) from the committed
+# `ncu --set full` capture (profiles/r01b_k_pass_full.md: 824.6 + 524.5 Mbyte); reported only for that workload.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1349.1e6
 
 
 def decoded_mbit_per_s(block_length_bits: float, n_frames: float, seconds: float) -> float:
@@ -319,7 +319,8 @@ def main():
     achieved = (b_min * live_per_launch) / (vn_avg_ms * 1e-3) / 1e9 if vn_timed else None
     roofline = {
         "bound": "hbm", "kernel": "k_pass", "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": (achieved / peak) if achieved else None, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+        "frac": (achieved / peak) if achieved else None,
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if (cfg.index == 4 and F == 64 and live_per_launch == 64) else None,
         "peak_source": peak_src, "bytes_model": "B_min = 8*E_core + 4*n + m/8 per live frame-iteration",
         "algorithmic_bytes_per_launch": b_min * live_per_launch, "avg_launch_ms": vn_avg_ms,
         "timed_launches": int(vn_timed), "launches": int(vn_launched),
