@@ -1,8 +1,8 @@
 """Build step: compiles csrc/*.cu into csrc/libqcldpc.so for sm_100a with nvcc (in-tree, no JIT cache).
 
-`python -m paper_1702_07740_b200.build [--force]`.  nvcc cross-compiles without a GPU.  k_pass is instantiated once
-per column shape in its own object file (pass_inst.cu with -DPASS_DV / -DPASS_NG / -DPASS_EXACT); objects build in
-parallel.
+`python -m paper_1702_07740_b200.build [--force]`.  nvcc cross-compiles without a GPU.  The fused pass is instantiated
+once per exact column shape in its own object file (pass_inst.cu with -DPASS_DV / -DPASS_NG / -DPASS_PCAP), the generic
+kernel in pass_generic.cu; objects build in parallel.
 """
 from __future__ import annotations
 
@@ -15,23 +15,22 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"),
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
-# (symbol, DV, NG, EXACT): EXACT = every active column has degree DV with NG gen edges (the BASELINE.json codes:
-# 11 or 21 edges, 3 of them into the top rows); the generic instantiation takes any column of degree <= 64
+# (symbol, DV, NG): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
+# 11 or 21 edges, 3 of them into the top rows); pass_generic.cu takes any column of degree <= 64
 PCAP = int(os.environ.get("QCLDPC_PCAP", "4"))   # partner slots per gen edge held in registers (tuning knob)
-PASS_INSTANCES = [("launch_pass_dv11_ng3", 11, 3, 1), ("launch_pass_dv21_ng3", 21, 3, 1),
-                  ("launch_pass_generic", 64, 64, 0)]
+PASS_INSTANCES = [("launch_pass_dv11_ng3", 11, 3), ("launch_pass_dv21_ng3", 21, 3)]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def _units():
-    units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), [])]
-    for name, dv, ng, exact in PASS_INSTANCES:
+    units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), []),
+             (os.path.join(CSRC, "pass_generic.cu"), os.path.join(OBJDIR, "pass_generic.o"), [])]
+    for name, dv, ng in PASS_INSTANCES:
         units.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJDIR, f"{name}.o"),
-                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={PCAP}",
-                       f"-DPASS_EXACT={exact}"]))
+                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={PCAP}"]))
     return units
 
 

@@ -62,8 +62,28 @@ struct PassArgs {
     int64_t n, EZs, mZs, AZs;  // per-frame strides
 };
 
-struct PassLaunch { PassTables tab; PassArgs args; dim3 grid; cudaStream_t stream; int V; bool final_mode; };
+// Codes whose active columns all have the same shape (DV edges, the first NG of them gen edges; at most kMaxExactCols
+// columns): the column descriptors travel in the kernel parameters (pass_exact.cuh).  Offsets are in floats.
+constexpr int kMaxExactCols = 16;
+template <int DV, int NG, int PCAP>
+struct ExactCol {
+    int col, ebeg;                                   // base column; first active edge
+    int shift[DV], t_off[DV];                        // edge k: t at t[t_off + (i - shift) mod Z]
+    int p_off[DV], delta[DV];                        // pair edge k >= NG: partner at w[p_off + (i + delta) mod Z]
+    int g_off[(NG > 0 ? NG : 1) * PCAP], g_delta[(NG > 0 ? NG : 1) * PCAP];   // gen edge g, slot j: partner or off = -1
+    int g_np[NG > 0 ? NG : 1], g_counter[NG > 0 ? NG : 1], g_pbeg[NG > 0 ? NG : 1];   // all partners: partner[g_pbeg + j], j < g_np
+};
+template <int DV, int NG, int PCAP>
+struct ExactTable { ExactCol<DV, NG, PCAP> c[kMaxExactCols]; };
+struct HostTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc* partner; const ColDesc* col; int n_cols; };
+
+struct PassLaunch {
+    PassTables tab; PassArgs args; dim3 grid; cudaStream_t stream; int V; bool final_mode;
+    const void* exact;         // HOST: the ExactTable of the instantiation (exact families only)
+    int n_cols, n_frames;
+};
 using PassLauncher = void (*)(const PassLaunch&);
+using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only
 
 // ---- device helpers ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__

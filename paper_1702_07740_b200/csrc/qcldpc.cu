@@ -37,6 +37,8 @@ namespace qc {
 void launch_pass_dv11_ng3(const PassLaunch&);
 void launch_pass_dv21_ng3(const PassLaunch&);
 void launch_pass_generic(const PassLaunch&);
+size_t launch_pass_dv11_ng3_table(const HostTables&, void*);
+size_t launch_pass_dv21_ng3_table(const HostTables&, void*);
 }  // namespace qc
 
 using namespace qc;
@@ -58,7 +60,7 @@ thread_local Profile g_prof;
 }  // namespace
 
 struct qcldpc_code {
-    int mb, nb, Z, Zs, V, tiles;
+    int mb, nb, Z, Zs, tiles;             // tiles = ceil(Z / kThreads)
     int64_t n, m;
     int n_act_cols, n_act_edges, max_dv;
     bool filter_rows;                     // some row has no absorbed variable (the early-exit filter exists)
@@ -71,6 +73,7 @@ struct qcldpc_code {
     EdgeDesc* d_edge = nullptr; GenDesc* d_gen = nullptr; PartnerDesc* d_partner = nullptr; ColDesc* d_col = nullptr;
     RowDesc* d_row = nullptr; RowEdge* d_redge = nullptr;
     PassLauncher launcher = nullptr;
+    std::vector<char> exact;              // kernel-parameter table of the exact family (empty: generic kernel)
     int n_sm = 148;
 };
 
@@ -424,13 +427,16 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
     bool uniform = code->n_act_cols > 0;
     for (const ColDesc& cd : code->col) uniform = uniform && cd.dv == code->col[0].dv && cd.ng == code->col[0].ng;
     code->launcher = launch_pass_generic;
-    code->V = 1;
-    if (uniform && max_np <= 128 && code->col[0].ng == 3 && (code->col[0].dv == 11 || code->col[0].dv == 21)) {
+    if (uniform && code->n_act_cols <= kMaxExactCols && code->col[0].ng == 3 &&
+        (code->col[0].dv == 11 || code->col[0].dv == 21)) {
         code->launcher = code->col[0].dv == 11 ? launch_pass_dv11_ng3 : launch_pass_dv21_ng3;
-        const char* v = getenv("QCLDPC_V");                  // tuning knob: variables per thread (1 or 2)
-        if (v && atoi(v) == 2) code->V = 2;
+        const ExactBuilder fill = code->col[0].dv == 11 ? launch_pass_dv11_ng3_table : launch_pass_dv21_ng3_table;
+        const HostTables ht{code->edge.data(), code->gen.data(), code->partner.data(), code->col.data(),
+                            code->n_act_cols};
+        code->exact.resize(fill(ht, nullptr));
+        fill(ht, code->exact.data());
     }
-    code->tiles = (Z + kThreads * code->V - 1) / (kThreads * code->V);
+    code->tiles = (Z + kThreads - 1) / kThreads;
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
         const size_t bytes = std::max<size_t>(vec.size(), 1) * sizeof(vec[0]);
@@ -503,10 +509,20 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
     k_init_rows<<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(ctab, ia);
     ++g_launches;
 
+    // exact families: two variables per thread (1 KB windows) once the grid still fills the chip several times over;
+    // small batches keep one variable per thread (more CTAs in flight).  QCLDPC_V=1|2 overrides (tuning knob).
+    int V = 1;
+    if (!code->exact.empty()) {
+        const int64_t ctas_v2 = (int64_t)((Z + 2 * kThreads - 1) / (2 * kThreads)) * code->n_act_cols * n_frames;
+        if (ctas_v2 >= (int64_t)4 * 8 * code->n_sm) V = 2;
+        const char* v = getenv("QCLDPC_V");
+        if (v && (atoi(v) == 1 || atoi(v) == 2)) V = atoi(v);
+    }
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, code->n, EZs, mZs, AZs},
-                  dim3(code->tiles * code->n_act_cols, n_frames), st, code->V, false};
+                  dim3(code->tiles * code->n_act_cols, n_frames), st, V, false,
+                  code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
                  d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
                  n_frames, code->mb, Z, Zs, tiles1, 0, code->n, code->m, EZs, AZs};
