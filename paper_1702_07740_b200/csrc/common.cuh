@@ -85,8 +85,27 @@ struct PassLaunch {
 using PassLauncher = void (*)(const PassLaunch&);
 using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only
 
+// Programmatic dependent launch: the per-iteration kernels (the fused pass, k_cand) are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization, so the CTAs of launch k+1 are placed on the SMs while launch k
+// drains, run their parameter-only preamble and block in pdl_wait() until launch k has completed and its writes are
+// visible.  Every such kernel calls pdl_launch() first and pdl_wait() before its first access to global memory that
+// a predecessor writes -- in EVERY CTA, so completion of launch k+1 implies completion of launch k (the chain is
+// transitive).
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---- device helpers ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }

@@ -15,16 +15,8 @@ __global__ void __launch_bounds__(kThreads) k_pass_exact(const __grid_constant__
                                                          const __grid_constant__ PassArgs a,
                                                          const PartnerDesc* __restrict__ partner) {
     constexpr int NGS = NG > 0 ? NG : 1;
+    pdl_launch();
     const int f = blockIdx.z;
-    int in_buf;
-    if (FINAL) {
-        const int Tit = a.iters[f];
-        if (Tit <= 0) return;                                // t = 0: k_init_cols wrote the outputs
-        in_buf = (Tit - 1) % 3;
-    } else {
-        if (a.done[f]) return;                               // frame already stopped: its state stays frozen
-        in_buf = a.in_buf;
-    }
     const int ca = blockIdx.y;                               // block-uniform active column
     const ExactCol<DV, NG, PCAP>& cd = T.c[ca];
     const int Z = a.Z, Zs = a.Zs;
@@ -44,6 +36,16 @@ __global__ void __launch_bounds__(kThreads) k_pass_exact(const __grid_constant__
         const int sl = tid - (kThreads - NG * PCAP);
         int x = i0 + cd.g_delta[sl]; x -= (x >= Z) ? Z : 0;
         s_po[sl] = cd.g_off[sl] >= 0 ? 4 * (cd.g_off[sl] + x) : -1;
+    }
+    pdl_wait();                                              // from here on: memory the previous launch wrote
+    int in_buf;
+    if (FINAL) {
+        const int Tit = a.iters[f];
+        if (Tit <= 0) return;                                // t = 0: k_init_cols wrote the outputs
+        in_buf = (Tit - 1) % 3;
+    } else {
+        if (a.done[f]) return;                               // frame already stopped: its state stays frozen
+        in_buf = a.in_buf;
     }
     __syncthreads();
 

@@ -43,8 +43,12 @@ size_t PASS_CAT(PASS_NAME, _table)(const HostTables& h, void* out) {
 template <int V, bool FINAL>
 static void launch_exact(const PassLaunch& L) {
     const dim3 grid((L.args.Z + kThreads * V - 1) / (kThreads * V), L.n_cols, L.n_frames);
-    k_pass_exact<PASS_DV, PASS_NG, PASS_PCAP, V, FINAL><<<grid, kThreads, 0, L.stream>>>(
-        *static_cast<const Table*>(L.exact), L.args, L.tab.partner);
+    if (FINAL)
+        k_pass_exact<PASS_DV, PASS_NG, PASS_PCAP, V, FINAL><<<grid, kThreads, 0, L.stream>>>(
+            *static_cast<const Table*>(L.exact), L.args, L.tab.partner);
+    else
+        launch_pdl(k_pass_exact<PASS_DV, PASS_NG, PASS_PCAP, V, FINAL>, grid, dim3(kThreads), 0, L.stream,
+                   *static_cast<const Table*>(L.exact), L.args, L.tab.partner);
 }
 
 void PASS_NAME(const PassLaunch& L) {

@@ -28,6 +28,8 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
     __shared__ GenDesc s_gd[kMaxDv];
     __shared__ int s_po[kMaxPartners];
 
+    pdl_launch();
+    pdl_wait();
     const int f = blockIdx.y;
     int in_buf;
     if (FINAL) {
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
 
 inline void launch_pass_any(const PassLaunch& L) {
     if (L.final_mode) k_pass<true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
-    else k_pass<false><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
+    else launch_pdl(k_pass<false>, L.grid, dim3(kThreads), 0, L.stream, L.tab, L.args);
 }
 
 }  // namespace qc

@@ -202,6 +202,8 @@ __global__ void k_flags_final(int* unsat, uint8_t* pass, int n_frames) {
 // block walks the candidates in the same order; the last block to finish freezes the frames whose full check passed.
 __global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const CheckArgs a) {
     __shared__ unsigned s_last;
+    pdl_launch();
+    pdl_wait();
     const int units = a.mb * a.tiles;
     if (blockIdx.x == 0)
         for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.topbad_clear[f] = 0;
@@ -544,7 +546,7 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
             ca.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
             ca.topbad_clear = w.topbad + (size_t)(t & 1) * n_frames;
             const int pk = prof_begin(1, st);
-            k_cand<<<cand_blocks, kThreads, 0, st>>>(ctab, ca);
+            launch_pdl(k_cand, dim3(cand_blocks), dim3(kThreads), 0, st, ctab, ca);
             prof_end(pk, st);
             ++g_launches;
         }
