@@ -80,6 +80,19 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
                   float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * qcldpc_decode with the paper's early-termination scheduling (the parity test is "enabled only after"
+ * an expected number of iterations, which the paper takes from a per-SNR table of average iteration counts):
+ *   check_from_iter  >= 1.  With early_stop = 1 the test H xhat = s runs at iterations t >= check_from_iter only; a
+ *                    frame cannot stop earlier, d_iters[f] >= check_from_iter for every frame that stops.
+ *                    check_from_iter = 1 is qcldpc_decode (test at every iteration, reading S5).  No effect when
+ *                    early_stop = 0.  The caller supplies the number (the paper's table is not published).
+ * Everything else as qcldpc_decode.  Before check_from_iter the per-iteration early-exit kernel is not launched.
+ */
+int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                     int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                     uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Same decode with HOST buffers (h_* are HOST pointers, same shapes; pinned memory makes the copies asynchronous):
  * copies inputs host->device, decodes, copies outputs device->host on `stream`, then WAITS for the stream so that the
  * h_* outputs are valid on return.  h_posterior may be NULL.  The device staging area is part of d_workspace, which

@@ -41,10 +41,10 @@ def _load():
         lib.oracle_build_h_coo.restype = ctypes.c_int64
         lib.oracle_build_h_coo.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                            ctypes.c_void_p, ctypes.c_void_p]
-        lib.oracle_decode.restype = ctypes.c_int
-        lib.oracle_decode.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+        lib.oracle_decode_from.restype = ctypes.c_int
+        lib.oracle_decode_from.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
-                                      ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                      ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                       ctypes.c_void_p]
         _lib = lib
@@ -79,7 +79,7 @@ class OracleResult(NamedTuple):
 
 def decode(base_shifts: np.ndarray, Z: int, llr: np.ndarray, syndrome: np.ndarray, max_iter: int,
            early_stop: int, msg_max: float = MSG_MAX, precision: int = 64, want_messages: bool = False,
-           threads: Optional[int] = None) -> OracleResult:
+           threads: Optional[int] = None, check_from: int = 1) -> OracleResult:
     """Run the oracle on frames llr float32 [F][n], syndrome uint8 [F][m]."""
     base = np.ascontiguousarray(base_shifts, dtype=np.int32)
     mb, nb = base.shape
@@ -98,8 +98,8 @@ def decode(base_shifts: np.ndarray, Z: int, llr: np.ndarray, syndrome: np.ndarra
     E = int((base >= 0).sum()) * Z
     msg = np.zeros((F, E), dtype=np.float64) if want_messages else None
     lib = _load()
-    rc = lib.oracle_decode(base.ctypes.data, mb, nb, Z, llr.ctypes.data, syndrome.ctypes.data, F, int(max_iter),
-                           int(early_stop), float(msg_max), int(precision), int(threads or 0),
+    rc = lib.oracle_decode_from(base.ctypes.data, mb, nb, Z, llr.ctypes.data, syndrome.ctypes.data, F, int(max_iter),
+                           int(early_stop), int(check_from), float(msg_max), int(precision), int(threads or 0),
                            hard.ctypes.data, iters.ctypes.data,
                            passed.ctypes.data, post.ctypes.data, msg.ctypes.data if msg is not None else None)
     if rc != 0:

@@ -147,12 +147,14 @@ double oracle_phi(double x) { return log1p(2.0 / expm1(x)); }
  *   msg_cv double[n_frames][E] (may be NULL): the CN->VN messages m_cv of the last executed iteration in
  *   check-major edge order (the order of oracle_build_h_coo).
  * precision: 64 = double (definition), 32 = float diagnostic (outputs still widened to double).
+ * check_from: the early-termination test (early_stop != 0) runs at iterations t >= check_from only (the
+ * paper enables it after the expected iteration count); 1 = every iteration.
  * Frames are independent and run one per OpenMP thread (n_threads <= 0: the OpenMP default).  Returns 0, or <0 on bad arguments / allocation failure.
  */
-int oracle_decode(const int32_t *base, int mb, int nb, int Z,
-                  const float *llr, const uint8_t *syndrome, int n_frames, int max_iter, int early_stop,
-                  double msg_max, int precision, int n_threads,
-                  uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv) {
+int oracle_decode_from(const int32_t *base, int mb, int nb, int Z,
+                       const float *llr, const uint8_t *syndrome, int n_frames, int max_iter, int early_stop,
+                       int check_from, double msg_max, int precision, int n_threads,
+                       uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv) {
     if (!base || !llr || !syndrome || !hard || !iters || !pass) return -1;
     if (mb <= 0 || nb <= 0 || Z <= 0 || n_frames < 0 || max_iter < 0) return -1;
     if (precision != 64 && precision != 32) return -1;
@@ -168,8 +170,8 @@ int oracle_decode(const int32_t *base, int mb, int nb, int Z,
         double *post = posterior ? posterior + (int64_t)f * h.n : NULL;
         double *mo = msg_cv ? msg_cv + (int64_t)f * h.E : NULL;
         int r = (precision == 64)
-            ? decode_frame_f64(&h, q, s, max_iter, early_stop, msg_max, hard + (int64_t)f * h.n, iters + f, pass + f, post, mo)
-            : decode_frame_f32(&h, q, s, max_iter, early_stop, msg_max, hard + (int64_t)f * h.n, iters + f, pass + f, post, mo);
+            ? decode_frame_f64(&h, q, s, max_iter, early_stop, check_from, msg_max, hard + (int64_t)f * h.n, iters + f, pass + f, post, mo)
+            : decode_frame_f32(&h, q, s, max_iter, early_stop, check_from, msg_max, hard + (int64_t)f * h.n, iters + f, pass + f, post, mo);
         if (r != 0) {
 #pragma omp atomic write
             fail = 1;
@@ -177,4 +179,13 @@ int oracle_decode(const int32_t *base, int mb, int nb, int Z,
     }
     free_h(&h);
     return fail ? -2 : 0;
+}
+
+/* The early-termination test at every iteration (reading S5). */
+int oracle_decode(const int32_t *base, int mb, int nb, int Z,
+                  const float *llr, const uint8_t *syndrome, int n_frames, int max_iter, int early_stop,
+                  double msg_max, int precision, int n_threads,
+                  uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv) {
+    return oracle_decode_from(base, mb, nb, Z, llr, syndrome, n_frames, max_iter, early_stop, 1, msg_max, precision,
+                              n_threads, hard, iters, pass, posterior, msg_cv);
 }

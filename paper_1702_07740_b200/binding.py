@@ -17,6 +17,7 @@ SO_PATH = os.path.join(_HERE, "csrc", "libqcldpc.so")
 
 EXPORTED_SYMBOLS = (
     "qcldpc_code_create", "qcldpc_code_destroy", "qcldpc_code_info", "qcldpc_workspace_bytes", "qcldpc_decode",
+    "qcldpc_decode_ex",
     "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
 )
@@ -41,6 +42,8 @@ _lib.qcldpc_host_workspace_bytes.argtypes = [_vp, _i, _i]
 _DECODE_ARGS = [_vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.qcldpc_decode.restype = _i
 _lib.qcldpc_decode.argtypes = _DECODE_ARGS
+_lib.qcldpc_decode_ex.restype = _i
+_lib.qcldpc_decode_ex.argtypes = [_vp, _vp, _vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.qcldpc_decode_host.restype = _i
 _lib.qcldpc_decode_host.argtypes = _DECODE_ARGS
 _lib.qcldpc_last_launch_count.restype = ctypes.c_int64
@@ -129,10 +132,11 @@ class QCLDPCCode:
 
     # ---------------------------------------------------------------------------------------------- decode
     def decode(self, llr, syndrome, max_iter: int, early_stop: int, want_posterior: bool = True,
-               workspace=None, out: Optional[DecodeResult] = None, stream=None) -> DecodeResult:
-        """qcldpc_decode on device tensors: llr float32 [F][n], syndrome uint8 [F][m] (torch, cuda, contiguous).
+               workspace=None, out: Optional[DecodeResult] = None, stream=None,
+               check_from_iter: int = 1) -> DecodeResult:
+        """qcldpc_decode_ex on device tensors: llr float32 [F][n], syndrome uint8 [F][m] (torch, cuda, contiguous).
 
-        Only enqueues work on `stream` (default: torch's current stream)."""
+        Only enqueues work on `stream` (default: torch's current stream).  check_from_iter = 1 is qcldpc_decode."""
         import torch
         if not (llr.is_cuda and syndrome.is_cuda):
             raise ValueError("qcldpc_decode needs CUDA tensors (no CPU fallback)")
@@ -154,12 +158,12 @@ class QCLDPCCode:
                                torch.empty((F, self.n), dtype=torch.float32, device=dev) if want_posterior else None)
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         with torch.cuda.device(dev):
-            rc = _lib.qcldpc_decode(self._handle, llr.data_ptr(), syndrome.data_ptr(), F, int(max_iter),
-                                    int(early_stop), out.hard.data_ptr(), out.iters.data_ptr(),
-                                    out.passed.data_ptr(),
-                                    out.posterior.data_ptr() if out.posterior is not None else None,
-                                    workspace.data_ptr(), workspace.numel(), st.cuda_stream)
-        _check(rc, "qcldpc_decode")
+            rc = _lib.qcldpc_decode_ex(self._handle, llr.data_ptr(), syndrome.data_ptr(), F, int(max_iter),
+                                       int(early_stop), int(check_from_iter), out.hard.data_ptr(),
+                                       out.iters.data_ptr(), out.passed.data_ptr(),
+                                       out.posterior.data_ptr() if out.posterior is not None else None,
+                                       workspace.data_ptr(), workspace.numel(), st.cuda_stream)
+        _check(rc, "qcldpc_decode_ex")
         return out
 
     def decode_host(self, llr: np.ndarray, syndrome: np.ndarray, max_iter: int, early_stop: int,

@@ -137,7 +137,7 @@ struct CheckArgs {
     const int* topbad;           // slot of the iteration being checked
     int* topbad_clear;           // the other slot
     int* fullbad; int* unsat; unsigned* ticket;
-    int n_frames, mb, Z, Zs, tiles, t; int64_t n, m, EZs, AZs;
+    int n_frames, mb, Z, Zs, tiles, t, check_from; int64_t n, m, EZs, AZs;
 };
 
 // a3: parity of check (R, r) of frame f for the decisions of iteration T: decides the absorbed degree-1 variable from
@@ -207,6 +207,7 @@ __global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const 
     const int units = a.mb * a.tiles;
     if (blockIdx.x == 0)
         for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.topbad_clear[f] = 0;
+    if (a.t < a.check_from) return;                                      // launched only to clear the filter slot
     bool any = false;
     for (int f0 = 0; f0 < a.n_frames; f0 += kThreads) {
         const int f = f0 + threadIdx.x;
@@ -484,7 +485,15 @@ size_t qcldpc_workspace_bytes(const qcldpc_code_t* code, int n_frames) {
 int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                   int max_iter, int early_stop, uint8_t* d_hard, int32_t* d_iters, uint8_t* d_pass,
                   float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream) {
+    return qcldpc_decode_ex(code, d_llr, d_syndrome, n_frames, max_iter, early_stop, 1, d_hard, d_iters, d_pass,
+                            d_posterior, d_workspace, workspace_bytes, stream);
+}
+
+int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                     int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                     uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream) {
     g_launches = 0;
+    if (check_from_iter < 1) return QCLDPC_ERR_BAD_ARGUMENT;
     if (!code || !d_llr || !d_syndrome || !d_hard || !d_iters || !d_pass) return QCLDPC_ERR_BAD_ARGUMENT;
     if (n_frames <= 0 || n_frames > 65535 || max_iter < 0) return QCLDPC_ERR_BAD_ARGUMENT;
     if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255) ||
@@ -527,7 +536,7 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
                   code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
                  d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
-                 n_frames, code->mb, Z, Zs, tiles1, 0, code->n, code->m, EZs, AZs};
+                 n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
     const int cand_blocks = std::max(1, std::min(code->n_sm * 4, code->mb * tiles1));
 
     for (int t = 1; t <= max_iter; ++t) {
@@ -540,8 +549,9 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
             prof_end(pk, st);
             ++g_launches;
         }
-        if (early_stop && t >= 2) {
+        if (early_stop && t >= 2 && t - 1 >= check_from_iter - 1) {
             // early exit for iteration t-1: its filter bits were formed by pass t, its input state w^(t-2) is intact
+            // (the launch for iteration check_from_iter - 1 only clears the filter slot of the first checked one)
             ca.t = t - 1;
             ca.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
             ca.topbad_clear = w.topbad + (size_t)(t & 1) * n_frames;

@@ -37,11 +37,12 @@ def B():
     return binding
 
 
-def gpu_decode(B, base, Z, llr, syn, max_iter, early_stop, want_posterior=True):
+def gpu_decode(B, base, Z, llr, syn, max_iter, early_stop, want_posterior=True, check_from_iter=1):
     code = B.QCLDPCCode(base, Z)
     d_llr = torch.from_numpy(np.ascontiguousarray(llr, dtype=np.float32)).cuda()
     d_syn = torch.from_numpy(np.ascontiguousarray(syn, dtype=np.uint8)).cuda()
-    out = code.decode(d_llr, d_syn, max_iter, early_stop, want_posterior=want_posterior)
+    out = code.decode(d_llr, d_syn, max_iter, early_stop, want_posterior=want_posterior,
+                      check_from_iter=check_from_iter)
     torch.cuda.synchronize()
     post = out.posterior.cpu().numpy() if out.posterior is not None else None
     return out.hard.cpu().numpy(), out.iters.cpu().numpy(), out.passed.cpu().numpy(), post
@@ -94,6 +95,22 @@ def test_config1_early_stop_matches_oracle(oracle_lib, B):
     np.testing.assert_array_equal(hard[ok], ref.hard[ok])
     assert rel_err(post[ok], ref.posterior[ok]).max() <= TOL
     np.testing.assert_array_equal(W.syndrome_of(base, Z, hard[ok]), fr.syndrome[ok])
+
+
+@pytest.mark.parametrize("check_from", [2, 7, 13, 50, 60])
+def test_config1_check_from_iter_matches_oracle(oracle_lib, B, check_from):
+    """Early-termination scheduling: the test runs at iterations >= check_from only."""
+    cfg, base, Z, fr = W.make_config(1)
+    ref = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from=check_from)
+    hard, iters, passed, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1,
+                                           check_from_iter=check_from)
+    np.testing.assert_array_equal(passed, ref.passed)
+    np.testing.assert_array_equal(iters, ref.iters)
+    stopped = ref.iters < cfg.max_iter
+    assert (iters[stopped] >= check_from).all()
+    ok = ref.passed.astype(bool)
+    np.testing.assert_array_equal(hard[ok], ref.hard[ok])
+    assert rel_err(post[ok], ref.posterior[ok]).max() <= TOL
 
 
 # ----------------------------------------------------------------------- reduced-Z versions of configs 2, 3, 5

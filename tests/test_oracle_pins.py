@@ -278,3 +278,31 @@ def test_degree1_variable_posterior(oracle_lib):
     for f in range(2):
         want = fr.llr[f, d1].astype(np.float64) + r.msg_cv[f, edge_of[d1]]
         np.testing.assert_array_equal(r.posterior[f, d1], want)
+
+
+def test_check_from_iter_semantics(oracle_lib):
+    """Early-termination scheduling: with the test enabled from iteration T0 on, a frame that first
+    satisfies H xhat = s at t1 stops at max(t1, first passing t >= T0); the decisions of a stopped frame satisfy the
+    syndrome; T0 = 1 is the plain decode; T0 > max_iter never stops but still reports pass from the last decisions."""
+    cfg, base, Z, fr = W.make_config(1)
+    plain = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1)
+    same = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from=1)
+    np.testing.assert_array_equal(plain.iters, same.iters)
+    np.testing.assert_array_equal(plain.hard, same.hard)
+    for T0 in (5, 12, 30):
+        r = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from=T0)
+        stopped = r.iters < cfg.max_iter
+        assert (r.iters[stopped] >= T0).all()
+        assert (r.iters >= plain.iters).all()
+        # the state at iteration t does not depend on when the test runs: same as a fixed-count decode
+        for f in np.nonzero(stopped)[0][:3]:
+            fixed = oracle_lib.decode(base, Z, fr.llr[f], fr.syndrome[f], int(r.iters[f]), 0)
+            np.testing.assert_array_equal(fixed.hard[0], r.hard[f])
+            np.testing.assert_array_equal(fixed.posterior[0], r.posterior[f])
+        np.testing.assert_array_equal(W.syndrome_of(base, Z, r.hard[r.passed.astype(bool)]),
+                                      fr.syndrome[r.passed.astype(bool)])
+    never = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from=cfg.max_iter + 1)
+    off = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 0)
+    np.testing.assert_array_equal(never.iters, off.iters)
+    np.testing.assert_array_equal(never.passed, off.passed)
+    np.testing.assert_array_equal(never.hard, off.hard)
