@@ -52,6 +52,17 @@ typedef struct qcldpc_code qcldpc_code_t;
 int qcldpc_code_create(const int32_t* base_shifts, int mb, int nb, int Z, qcldpc_code_t** out_code);
 void qcldpc_code_destroy(qcldpc_code_t* code);
 
+/*
+ * The same handle from the NON-ZERO blocks only (for large base graphs, e.g. the paper's own ensemble with ~20,000
+ * base columns and q = 50, whose dense [mb][nb] array would be 1.5 GB):
+ *   rows, cols, shifts  HOST pointers, int32 [n_entries]: block (rows[k], cols[k]) is the identity shifted right by
+ *                       shifts[k] in [0,Z); any order; every other block is zero.  A repeated (row, col) pair is an
+ *                       error (a block is one circulant).
+ * qcldpc_code_create(base, ...) equals qcldpc_code_create_sparse of the cells of base that are >= 0.
+ */
+int qcldpc_code_create_sparse(const int32_t* rows, const int32_t* cols, const int32_t* shifts, int64_t n_entries,
+                              int mb, int nb, int Z, qcldpc_code_t** out_code);
+
 /* Code facts: n, m, number of active base edges (state = 2 * 4 * Z * that many bytes per frame). */
 int qcldpc_code_info(const qcldpc_code_t* code, int64_t* n, int64_t* m, int64_t* active_base_edges);
 

@@ -47,6 +47,17 @@ def _load():
                                       ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                       ctypes.c_void_p]
+        lib.oracle_decode_sparse.restype = ctypes.c_int
+        lib.oracle_decode_sparse.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                                             ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
+                                             ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                             ctypes.c_void_p]
+        lib.oracle_syndrome_sparse.restype = ctypes.c_int
+        lib.oracle_syndrome_sparse.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                                               ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                               ctypes.c_int, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -105,3 +116,47 @@ def decode(base_shifts: np.ndarray, Z: int, llr: np.ndarray, syndrome: np.ndarra
     if rc != 0:
         raise RuntimeError(f"oracle_decode failed with status {rc}")
     return OracleResult(hard, iters, passed, post, msg)
+
+
+def decode_sparse(rows: np.ndarray, cols: np.ndarray, shifts: np.ndarray, mb: int, nb: int, Z: int,
+                  llr: np.ndarray, syndrome: np.ndarray, max_iter: int, early_stop: int, msg_max: float = MSG_MAX,
+                  precision: int = 64, threads: Optional[int] = None, check_from: int = 1) -> OracleResult:
+    """The oracle on a code given by its non-zero blocks (rows[k], cols[k], shifts[k]); frames as in decode()."""
+    r = np.ascontiguousarray(rows, dtype=np.int32)
+    c = np.ascontiguousarray(cols, dtype=np.int32)
+    p = np.ascontiguousarray(shifts, dtype=np.int32)
+    llr = np.ascontiguousarray(llr, dtype=np.float32)
+    syndrome = np.ascontiguousarray(syndrome, dtype=np.uint8)
+    if llr.ndim == 1:
+        llr = llr[None]
+        syndrome = syndrome[None]
+    F, n = llr.shape
+    m = mb * Z
+    assert n == nb * Z and syndrome.shape == (F, m), (llr.shape, syndrome.shape, nb, mb, Z)
+    hard = np.zeros((F, n), dtype=np.uint8)
+    iters = np.zeros(F, dtype=np.int32)
+    passed = np.zeros(F, dtype=np.uint8)
+    post = np.zeros((F, n), dtype=np.float64)
+    rc = _load().oracle_decode_sparse(r.ctypes.data, c.ctypes.data, p.ctypes.data, len(r), int(mb), int(nb), int(Z),
+                                      llr.ctypes.data, syndrome.ctypes.data, F, int(max_iter), int(early_stop),
+                                      int(check_from), float(msg_max), int(precision), int(threads or 0),
+                                      hard.ctypes.data, iters.ctypes.data, passed.ctypes.data, post.ctypes.data, None)
+    if rc != 0:
+        raise RuntimeError(f"oracle_decode_sparse failed with status {rc}")
+    return OracleResult(hard, iters, passed, post, None)
+
+
+def syndrome_sparse(rows, cols, shifts, mb: int, nb: int, Z: int, x: np.ndarray) -> np.ndarray:
+    """s = H x mod 2 by the oracle's own loop over the non-zero blocks (x uint8 [F][n] -> uint8 [F][m])."""
+    r = np.ascontiguousarray(rows, dtype=np.int32)
+    c = np.ascontiguousarray(cols, dtype=np.int32)
+    p = np.ascontiguousarray(shifts, dtype=np.int32)
+    x = np.ascontiguousarray(x, dtype=np.uint8)
+    if x.ndim == 1:
+        x = x[None]
+    s = np.zeros((x.shape[0], mb * Z), dtype=np.uint8)
+    rc = _load().oracle_syndrome_sparse(r.ctypes.data, c.ctypes.data, p.ctypes.data, len(r), int(mb), int(nb), int(Z),
+                                        x.ctypes.data, x.shape[0], s.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_syndrome_sparse failed with status {rc}")
+    return s

@@ -94,6 +94,62 @@ static int build_h(const int32_t *base, int mb, int nb, int Z, sparse_h *h) {
     return 0;
 }
 
+/* The same H from the non-zero blocks only: block (brow[k], bcol[k]) = identity shifted right by bshift[k].
+ * Entries may come in any order; inside a check the edges are stored by increasing base column, as in build_h.
+ * A repeated (row, col) pair is rejected (a block is one circulant). */
+typedef struct { int32_t r, c, p; } base_entry;
+static int cmp_entry(const void *a, const void *b) {
+    const base_entry *x = a, *y = b;
+    if (x->r != y->r) return x->r < y->r ? -1 : 1;
+    if (x->c != y->c) return x->c < y->c ? -1 : 1;
+    return 0;
+}
+static int build_h_sparse(const int32_t *brow, const int32_t *bcol, const int32_t *bshift, int64_t nnz_base,
+                          int mb, int nb, int Z, sparse_h *h) {
+    memset(h, 0, sizeof(*h));
+    h->n = (int64_t)nb * Z;
+    h->m = (int64_t)mb * Z;
+    h->E = nnz_base * Z;
+    base_entry *ent = malloc(sizeof(base_entry) * (size_t)(nnz_base + 1));
+    int64_t *first = calloc((size_t)mb + 1, sizeof(int64_t));      /* entries of base row R: first[R] .. first[R+1]-1 */
+    if (!ent || !first) { free(ent); free(first); return -2; }
+    for (int64_t k = 0; k < nnz_base; ++k) {
+        if (brow[k] < 0 || brow[k] >= mb || bcol[k] < 0 || bcol[k] >= nb || bshift[k] < 0 || bshift[k] >= Z) {
+            free(ent); free(first); return -1;
+        }
+        ent[k].r = brow[k]; ent[k].c = bcol[k]; ent[k].p = bshift[k];
+    }
+    qsort(ent, (size_t)nnz_base, sizeof(base_entry), cmp_entry);
+    for (int64_t k = 1; k < nnz_base; ++k)
+        if (ent[k].r == ent[k - 1].r && ent[k].c == ent[k - 1].c) { free(ent); free(first); return -1; }
+    for (int64_t k = 0; k < nnz_base; ++k) first[ent[k].r + 1]++;
+    for (int R = 0; R < mb; ++R) first[R + 1] += first[R];
+    h->row_ptr = calloc((size_t)h->m + 1, sizeof(int64_t));
+    h->edge_var = calloc((size_t)h->E + 1, sizeof(int64_t));
+    h->col_ptr = calloc((size_t)h->n + 1, sizeof(int64_t));
+    h->col_edge = calloc((size_t)h->E + 1, sizeof(int64_t));
+    int64_t *fill = calloc((size_t)h->n + 1, sizeof(int64_t));
+    if (!h->row_ptr || !h->edge_var || !h->col_ptr || !h->col_edge || !fill) {
+        free_h(h); free(ent); free(first); free(fill); return -2;
+    }
+    int64_t e = 0;
+    for (int R = 0; R < mb; ++R)
+        for (int r = 0; r < Z; ++r) {
+            h->row_ptr[(int64_t)R * Z + r] = e;
+            for (int64_t k = first[R]; k < first[R + 1]; ++k)
+                h->edge_var[e++] = (int64_t)ent[k].c * Z + (r + ent[k].p) % Z;
+        }
+    h->row_ptr[h->m] = e;
+    for (int64_t k = 0; k < h->E; ++k) h->col_ptr[h->edge_var[k] + 1]++;
+    for (int64_t v = 0; v < h->n; ++v) h->col_ptr[v + 1] += h->col_ptr[v];
+    for (int64_t k = 0; k < h->E; ++k) {
+        int64_t v = h->edge_var[k];
+        h->col_edge[h->col_ptr[v] + fill[v]++] = k;
+    }
+    free(fill); free(ent); free(first);
+    return 0;
+}
+
 /* COO dump of H for the lifting-rule pin (P9). rows/cols have room for nnz_base*Z entries. Returns E or <0. */
 int64_t oracle_build_h_coo(const int32_t *base, int mb, int nb, int Z, int64_t *rows, int64_t *cols) {
     sparse_h h;
@@ -151,6 +207,10 @@ double oracle_phi(double x) { return log1p(2.0 / expm1(x)); }
  * paper enables it after the expected iteration count); 1 = every iteration.
  * Frames are independent and run one per OpenMP thread (n_threads <= 0: the OpenMP default).  Returns 0, or <0 on bad arguments / allocation failure.
  */
+static int decode_frames(sparse_h *hp, const float *llr, const uint8_t *syndrome, int n_frames, int max_iter,
+                         int early_stop, int check_from, double msg_max, int precision, int n_threads,
+                         uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv);
+
 int oracle_decode_from(const int32_t *base, int mb, int nb, int Z,
                        const float *llr, const uint8_t *syndrome, int n_frames, int max_iter, int early_stop,
                        int check_from, double msg_max, int precision, int n_threads,
@@ -161,6 +221,47 @@ int oracle_decode_from(const int32_t *base, int mb, int nb, int Z,
     sparse_h h;
     int rc = build_h(base, mb, nb, Z, &h);
     if (rc != 0) return rc;
+    return decode_frames(&h, llr, syndrome, n_frames, max_iter, early_stop, check_from, msg_max, precision, n_threads,
+                         hard, iters, pass, posterior, msg_cv);
+}
+
+/* The same decode with H given by its non-zero blocks (build_h_sparse). */
+int oracle_decode_sparse(const int32_t *brow, const int32_t *bcol, const int32_t *bshift, int64_t nnz_base,
+                         int mb, int nb, int Z,
+                         const float *llr, const uint8_t *syndrome, int n_frames, int max_iter, int early_stop,
+                         int check_from, double msg_max, int precision, int n_threads,
+                         uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv) {
+    if (!llr || !syndrome || !hard || !iters || !pass || nnz_base < 0) return -1;
+    if (nnz_base > 0 && (!brow || !bcol || !bshift)) return -1;
+    if (mb <= 0 || nb <= 0 || Z <= 0 || n_frames < 0 || max_iter < 0) return -1;
+    if (precision != 64 && precision != 32) return -1;
+    sparse_h h;
+    int rc = build_h_sparse(brow, bcol, bshift, nnz_base, mb, nb, Z, &h);
+    if (rc != 0) return rc;
+    return decode_frames(&h, llr, syndrome, n_frames, max_iter, early_stop, check_from, msg_max, precision, n_threads,
+                         hard, iters, pass, posterior, msg_cv);
+}
+
+/* s = H x (mod 2) for n_frames words with H given by its non-zero blocks: an independent product for the harness of
+ * large base graphs (x uint8 [n_frames][n] -> s uint8 [n_frames][m]). */
+int oracle_syndrome_sparse(const int32_t *brow, const int32_t *bcol, const int32_t *bshift, int64_t nnz_base,
+                           int mb, int nb, int Z, const uint8_t *x, int n_frames, uint8_t *s) {
+    if (!x || !s || mb <= 0 || nb <= 0 || Z <= 0 || n_frames < 0 || nnz_base < 0) return -1;
+    const int64_t n = (int64_t)nb * Z, m = (int64_t)mb * Z;
+    memset(s, 0, (size_t)(m * n_frames));
+    for (int64_t k = 0; k < nnz_base; ++k) {
+        if (brow[k] < 0 || brow[k] >= mb || bcol[k] < 0 || bcol[k] >= nb || bshift[k] < 0 || bshift[k] >= Z) return -1;
+        for (int f = 0; f < n_frames; ++f)
+            for (int r = 0; r < Z; ++r)
+                s[f * m + (int64_t)brow[k] * Z + r] ^= x[f * n + (int64_t)bcol[k] * Z + (r + bshift[k]) % Z] & 1;
+    }
+    return 0;
+}
+
+static int decode_frames(sparse_h *hp, const float *llr, const uint8_t *syndrome, int n_frames, int max_iter,
+                         int early_stop, int check_from, double msg_max, int precision, int n_threads,
+                         uint8_t *hard, int32_t *iters, uint8_t *pass, double *posterior, double *msg_cv) {
+    sparse_h h = *hp;
     int fail = 0;
     const int nt = n_threads > 0 ? n_threads : omp_get_max_threads();
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nt)

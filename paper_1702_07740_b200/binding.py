@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "csrc", "libqcldpc.so")
 
 EXPORTED_SYMBOLS = (
-    "qcldpc_code_create", "qcldpc_code_destroy", "qcldpc_code_info", "qcldpc_workspace_bytes", "qcldpc_decode",
+    "qcldpc_code_create", "qcldpc_code_create_sparse", "qcldpc_code_destroy", "qcldpc_code_info", "qcldpc_workspace_bytes", "qcldpc_decode",
     "qcldpc_decode_ex",
     "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
@@ -30,6 +30,8 @@ _lib = ctypes.CDLL(SO_PATH)
 _vp, _i, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
 _lib.qcldpc_code_create.restype = _i
 _lib.qcldpc_code_create.argtypes = [_vp, _i, _i, _i, ctypes.POINTER(_vp)]
+_lib.qcldpc_code_create_sparse.restype = _i
+_lib.qcldpc_code_create_sparse.argtypes = [_vp, _vp, _vp, ctypes.c_int64, _i, _i, _i, ctypes.POINTER(_vp)]
 _lib.qcldpc_code_destroy.restype = None
 _lib.qcldpc_code_destroy.argtypes = [_vp]
 _lib.qcldpc_code_info.restype = _i
@@ -112,10 +114,29 @@ class QCLDPCCode:
         self._handle = _vp()
         _check(_lib.qcldpc_code_create(base.ctypes.data, self.mb, self.nb, self.Z, ctypes.byref(self._handle)),
                "qcldpc_code_create")
+        self._read_info()
+
+    def _read_info(self):
         n, m, e = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
         _check(_lib.qcldpc_code_info(self._handle, ctypes.byref(n), ctypes.byref(m), ctypes.byref(e)),
                "qcldpc_code_info")
         self.n, self.m, self.active_base_edges = n.value, m.value, e.value
+
+    @classmethod
+    def from_sparse(cls, rows: np.ndarray, cols: np.ndarray, shifts: np.ndarray, mb: int, nb: int, Z: int):
+        """qcldpc_code_create_sparse: the non-zero blocks (rows[k], cols[k]) with shift shifts[k]."""
+        self = cls.__new__(cls)
+        r = np.ascontiguousarray(rows, dtype=np.int32)
+        c = np.ascontiguousarray(cols, dtype=np.int32)
+        p = np.ascontiguousarray(shifts, dtype=np.int32)
+        if not (r.ndim == c.ndim == p.ndim == 1 and len(r) == len(c) == len(p)):
+            raise ValueError("rows, cols, shifts must be 1-D arrays of one length")
+        self.mb, self.nb, self.Z = int(mb), int(nb), int(Z)
+        self._handle = _vp()
+        _check(_lib.qcldpc_code_create_sparse(r.ctypes.data, c.ctypes.data, p.ctypes.data, len(r), self.mb, self.nb,
+                                              self.Z, ctypes.byref(self._handle)), "qcldpc_code_create_sparse")
+        self._read_info()
+        return self
 
     def __del__(self):
         h = getattr(self, "_handle", None)

@@ -320,34 +320,71 @@ Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
 // ---------------------------------------------------------------------------------------------------------------
 extern "C" {
 
+// The non-zero blocks of the base matrix: per base row the (column, shift) pairs, per base column the (row, shift)
+// pairs, both in increasing index order.
+struct BaseEntry { int idx, shift; };
+struct BaseLists { std::vector<std::vector<BaseEntry>> rows, cols; };
+
+static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_code_t** out_code);
+
 int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t** out_code) {
     if (!base || !out_code || mb <= 0 || nb <= 0 || Z <= 0) return QCLDPC_ERR_BAD_ARGUMENT;
     *out_code = nullptr;
+    BaseLists B;
+    B.rows.resize(mb); B.cols.resize(nb);
+    for (int R = 0; R < mb; ++R)
+        for (int C = 0; C < nb; ++C) {
+            const int p = base[(size_t)R * nb + C];
+            if (p < -1 || p >= Z) return QCLDPC_ERR_BAD_ARGUMENT;
+            if (p >= 0) { B.rows[R].push_back(BaseEntry{C, p}); B.cols[C].push_back(BaseEntry{R, p}); }
+        }
+    return code_from_lists(B, mb, nb, Z, out_code);
+}
+
+int qcldpc_code_create_sparse(const int32_t* rows, const int32_t* cols, const int32_t* shifts, int64_t n_entries,
+                              int mb, int nb, int Z, qcldpc_code_t** out_code) {
+    if (!out_code || mb <= 0 || nb <= 0 || Z <= 0 || n_entries < 0) return QCLDPC_ERR_BAD_ARGUMENT;
+    if (n_entries > 0 && (!rows || !cols || !shifts)) return QCLDPC_ERR_BAD_ARGUMENT;
+    *out_code = nullptr;
+    BaseLists B;
+    B.rows.resize(mb); B.cols.resize(nb);
+    for (int64_t k = 0; k < n_entries; ++k) {
+        if (rows[k] < 0 || rows[k] >= mb || cols[k] < 0 || cols[k] >= nb || shifts[k] < 0 || shifts[k] >= Z)
+            return QCLDPC_ERR_BAD_ARGUMENT;
+        B.rows[rows[k]].push_back(BaseEntry{cols[k], shifts[k]});
+        B.cols[cols[k]].push_back(BaseEntry{rows[k], shifts[k]});
+    }
+    auto by_idx = [](const BaseEntry& a, const BaseEntry& b) { return a.idx < b.idx; };
+    for (auto& r : B.rows) {
+        std::sort(r.begin(), r.end(), by_idx);
+        for (size_t k = 1; k < r.size(); ++k)
+            if (r[k].idx == r[k - 1].idx) return QCLDPC_ERR_BAD_ARGUMENT;        // a block is ONE circulant
+    }
+    for (auto& c : B.cols) std::sort(c.begin(), c.end(), by_idx);
+    return code_from_lists(B, mb, nb, Z, out_code);
+}
+
+static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_code_t** out_code) {
     if ((int64_t)mb * Z > (int64_t)1 << 30 || (int64_t)nb * Z > (int64_t)1 << 30) return QCLDPC_ERR_UNSUPPORTED;
-    for (int64_t k = 0; k < (int64_t)mb * nb; ++k)
-        if (base[k] < -1 || base[k] >= Z) return QCLDPC_ERR_BAD_ARGUMENT;
     qcldpc_code* code = new (std::nothrow) qcldpc_code();
     if (!code) return QCLDPC_ERR_ALLOC;
     code->mb = mb; code->nb = nb; code->Z = Z;
     code->Zs = (int)align_up((size_t)Z + kHalo, 32);
     code->n = (int64_t)nb * Z; code->m = (int64_t)mb * Z;
     const int Zs = code->Zs;
-    auto cell = [&](int R, int C) { return base[(size_t)R * nb + C]; };
 
-    // column degrees; absorb at most one degree-1 column per row (the lowest-numbered one)
-    std::vector<int> deg(nb, 0), absorbed_by(nb, -1), n_active(mb, 0);
-    for (int R = 0; R < mb; ++R)
-        for (int C = 0; C < nb; ++C) deg[C] += cell(R, C) >= 0;
+    // absorb at most one degree-1 column per row (the lowest-numbered one)
+    std::vector<int> absorbed_by(nb, -1), n_active(mb, 0);
     code->row.assign(mb, RowDesc{0, 0, -1, 0, 0, 0, 0, 0});
     for (int R = 0; R < mb; ++R)
-        for (int C = 0; C < nb; ++C)
-            if (cell(R, C) >= 0 && deg[C] == 1 && code->row[R].abs_col < 0) {
-                code->row[R].abs_col = C;
-                code->row[R].abs_shift = cell(R, C);
-                absorbed_by[C] = R;
+        for (const BaseEntry& e : B.rows[R])
+            if (B.cols[e.idx].size() == 1 && code->row[R].abs_col < 0) {
+                code->row[R].abs_col = e.idx;
+                code->row[R].abs_shift = e.shift;
+                absorbed_by[e.idx] = R;
             }
     for (int R = 0; R < mb; ++R)
-        for (int C = 0; C < nb; ++C) n_active[R] += (cell(R, C) >= 0 && absorbed_by[C] < 0);
+        for (const BaseEntry& e : B.rows[R]) n_active[R] += absorbed_by[e.idx] < 0;
     code->filter_rows = false;
     for (int R = 0; R < mb; ++R) {
         code->row[R].gen = !(code->row[R].abs_col >= 0 && n_active[R] == 2);
@@ -357,16 +394,25 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
     // active columns and their edges: column by column, gen edges first, then pair edges, each in row order
     struct HostEdge { int shift, row; };
     std::vector<HostEdge> edges;
-    std::vector<int> edge_of_cell((size_t)mb * nb, -1), act_index(nb, -1);
+    std::vector<int> act_index(nb, -1);
+    std::vector<std::vector<int>> edge_of_row_entry(mb);        // parallel to B.rows[R]: active edge id or -1
+    for (int R = 0; R < mb; ++R) edge_of_row_entry[R].assign(B.rows[R].size(), -1);
+    auto row_pos = [&](int R, int C) {                           // position of column C in B.rows[R]
+        const auto& r = B.rows[R];
+        size_t lo = 0, hi = r.size();
+        while (lo < hi) { const size_t mid = (lo + hi) / 2; if (r[mid].idx < C) lo = mid + 1; else hi = mid; }
+        return lo;
+    };
     code->max_dv = 0;
     for (int C = 0; C < nb; ++C) {
         if (absorbed_by[C] >= 0) continue;
         ColDesc cd{C, (int)edges.size(), 0, 0, 0, 0, 0, 0};
         for (int pass = 0; pass < 2; ++pass)
-            for (int R = 0; R < mb; ++R) {
-                if (cell(R, C) < 0 || (code->row[R].gen != 0) != (pass == 0)) continue;
-                edge_of_cell[(size_t)R * nb + C] = (int)edges.size();
-                edges.push_back(HostEdge{cell(R, C), R});
+            for (const BaseEntry& e : B.cols[C]) {
+                const int R = e.idx;
+                if ((code->row[R].gen != 0) != (pass == 0)) continue;
+                edge_of_row_entry[R][row_pos(R, C)] = (int)edges.size();
+                edges.push_back(HostEdge{e.shift, R});
                 ++cd.dv;
                 cd.ng += pass == 0;
             }
@@ -384,9 +430,10 @@ int qcldpc_code_create(const int32_t* base, int mb, int nb, int Z, qcldpc_code_t
     // row view
     for (int R = 0; R < mb; ++R) {
         code->row[R].ebeg = (int)code->redge.size();
-        for (int C = 0; C < nb; ++C) {
-            const int e = edge_of_cell[(size_t)R * nb + C];
-            if (e >= 0) code->redge.push_back(RowEdge{e, cell(R, C), C, act_index[C]});
+        for (size_t k = 0; k < B.rows[R].size(); ++k) {
+            const int e = edge_of_row_entry[R][k];
+            const int C = B.rows[R][k].idx;
+            if (e >= 0) code->redge.push_back(RowEdge{e, B.rows[R][k].shift, C, act_index[C]});
         }
         code->row[R].ne = (int)code->redge.size() - code->row[R].ebeg;
     }

@@ -194,3 +194,134 @@ def make_config(cfg_index: int, snr_point: int = 0, n_frames: int | None = None,
     nf = cfg.n_frames if n_frames is None else n_frames
     frames = make_frames(base, spec.Z, sigma, nf, frame_seed_base(cfg_index, snr_point), first_frame)
     return cfg, base, spec.Z, frames
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-1: the paper's own rate-0.02 multi-edge ensemble, lifted by q.
+# Three edge types.  Variable nodes (fractions of nb base columns, Omega):  9/400 with 2 type-1 + 57 type-2
+# sockets, 7/400 with 3 type-1 + 57 type-2, 24/25 with one type-3 socket (the degree-1 diagonal).  Check nodes
+# (Psi): 3/5 with 2 type-2 + 1 type-3, 9/25 with 3 type-2 + 1 type-3, and the "top" checks with type-1
+# sockets only.  Reading G1: as printed, Psi's type-1 coefficients (3/320 on x1^3, 17/1600 on x1^7) do not
+# balance the type-1 sockets of Omega (97.5 vs 102.5 per 1000 columns); swapped (17/1600 on x1^3, 3/320 on x1^7) they do,
+# and the total edge count matches P:499.  For block lengths where those fractions are not integers the numbers of
+# degree-3 and degree-7 top checks are the integers (a, b) with 3a + 7b = type-1 sockets and a + b closest to nb/50,
+# which is what the paper's q = 50 code does (n = 1e6, rate 0.01995 instead of 0.02).
+@dataclass(frozen=True)
+class EnsembleSpec:
+    nb: int                # base columns (n / q)
+    q: int                 # expansion factor (Z)
+    n_core2: int           # columns with 2 type-1 + 57 type-2 sockets
+    n_core3: int           # columns with 3 type-1 + 57 type-2 sockets
+    n_d1: int              # degree-1 columns
+    rows_t3: int           # top checks of degree 3 (type 1 only)
+    rows_t7: int           # top checks of degree 7
+    rows_l2: int           # lower checks with 2 type-2 sockets (+ 1 type-3)
+    rows_l3: int           # lower checks with 3 type-2 sockets (+ 1 type-3)
+    seed: int
+
+    @property
+    def mb(self) -> int:
+        return self.rows_t3 + self.rows_t7 + self.rows_l2 + self.rows_l3
+
+    @property
+    def n(self) -> int:
+        return self.nb * self.q
+
+    @property
+    def m(self) -> int:
+        return self.mb * self.q
+
+    @property
+    def base_edges(self) -> int:
+        return (2 * self.n_core2 + 3 * self.n_core3) + 57 * (self.n_core2 + self.n_core3) + self.n_d1
+
+
+PAPER_ENSEMBLE_SEED = 17020776000
+
+
+def paper_ensemble_spec(nb: int, q: int, seed: int = PAPER_ENSEMBLE_SEED) -> EnsembleSpec:
+    """Node counts of the ensemble at nb base columns (nb must be a multiple of 400 so that Omega's fractions and the
+    lower-check fractions 3/5, 9/25 are integers)."""
+    if nb % 400:
+        raise ValueError("nb must be a multiple of 400")
+    c2, c3, d1 = 9 * nb // 400, 7 * nb // 400, 24 * nb // 25
+    l2, l3 = 3 * nb // 5, 9 * nb // 25
+    assert l2 + l3 == d1 and 2 * l2 + 3 * l3 == 57 * (c2 + c3)
+    s1 = 2 * c2 + 3 * c3                                    # type-1 sockets on the variable side
+    best = None
+    for b in range(s1 // 7 + 1):
+        if (s1 - 7 * b) % 3 == 0:
+            a = (s1 - 7 * b) // 3
+            score = (abs((a + b) - nb / 50.0), abs(b - 3.0 * nb / 320.0))
+            if best is None or score < best[0]:
+                best = (score, a, b)
+    if best is None:
+        raise ValueError("type-1 sockets cannot be split into checks of degree 3 and 7")
+    return EnsembleSpec(nb, q, c2, c3, d1, best[1], best[2], l2, l3, seed)
+
+
+def _match_sockets(rng: np.random.Generator, vn_sockets: np.ndarray, cn_sockets: np.ndarray):
+    """Random edge-type matching: pair every variable socket with a check socket of the same type,
+    uniformly at random, then repair parallel edges (two edges between one column and one row cannot be one
+    circulant) by swapping the offending variable socket with a random other one until none is left."""
+    assert len(vn_sockets) == len(cn_sockets)
+    cols = rng.permutation(vn_sockets)
+    rows = cn_sockets.copy()
+    for _ in range(10000):
+        key = rows.astype(np.int64) * (int(cols.max()) + 1) + cols
+        order = np.argsort(key, kind="stable")
+        dup = order[1:][key[order][1:] == key[order][:-1]]
+        if len(dup) == 0:
+            return rows, cols
+        other = rng.integers(0, len(cols), size=len(dup))
+        for a, b in zip(dup, other):
+            cols[a], cols[b] = cols[b], cols[a]
+    raise RuntimeError("could not remove parallel edges")
+
+
+def make_paper_ensemble(spec: EnsembleSpec):
+    """Base graph of the paper's ensemble as the non-zero blocks (rows, cols, shifts), int32 arrays of length
+    spec.base_edges, plus (mb, nb).  Columns: the n_core2 + n_core3 core columns first, then the degree-1 diagonal;
+    rows: top checks (degree 3, then degree 7) first, then the lower checks (2, then 3 type-2 sockets); degree-1 column
+    nc + r is the unshifted identity on lower row n_top + r (Fig. 11).  Shifts of all other blocks are
+    uniform in [0, q).  The structure depends on spec.seed only, the shifts on (spec.seed, q)."""
+    rng = np.random.default_rng(spec.seed)
+    nc = spec.n_core2 + spec.n_core3
+    n_top = spec.rows_t3 + spec.rows_t7
+    n_low = spec.rows_l2 + spec.rows_l3
+    deg1 = np.concatenate([np.full(spec.n_core2, 2), np.full(spec.n_core3, 3)])
+    vn1 = np.repeat(np.arange(nc), deg1)
+    cn1 = np.repeat(np.arange(n_top), np.concatenate([np.full(spec.rows_t3, 3), np.full(spec.rows_t7, 7)]))
+    r1, c1 = _match_sockets(rng, vn1, cn1)
+    vn2 = np.repeat(np.arange(nc), 57)
+    cn2 = n_top + np.repeat(np.arange(n_low), np.concatenate([np.full(spec.rows_l2, 2), np.full(spec.rows_l3, 3)]))
+    r2, c2 = _match_sockets(rng, vn2, cn2)
+    rows = np.concatenate([r1, r2, n_top + np.arange(n_low)]).astype(np.int32)
+    cols = np.concatenate([c1, c2, nc + np.arange(n_low)]).astype(np.int32)
+    srng = np.random.default_rng([spec.seed, spec.q])
+    shifts = np.concatenate([srng.integers(0, spec.q, size=len(r1) + len(r2)), np.zeros(n_low, dtype=np.int64)])
+    return rows, cols, shifts.astype(np.int32), spec.mb, spec.nb
+
+
+def syndrome_of_sparse(rows, cols, shifts, mb: int, nb: int, Z: int, x: np.ndarray) -> np.ndarray:
+    """s = H x mod 2 for x uint8 [..., nb*Z], H given by its non-zero blocks (lifting rule P:324)."""
+    xs = x.reshape(x.shape[:-1] + (nb, Z))
+    s = np.zeros(x.shape[:-1] + (mb, Z), dtype=np.uint8)
+    idx = (np.arange(Z)[None, :] + np.asarray(shifts)[:, None]) % Z          # [entries][Z]: (r + p) mod Z
+    for k in range(len(rows)):
+        s[..., rows[k], :] ^= xs[..., cols[k], :][..., idx[k]]
+    return s.reshape(x.shape[:-1] + (mb * Z,))
+
+
+def make_frames_sparse(rows, cols, shifts, mb: int, nb: int, Z: int, sigma: float, n_frames: int,
+                       seed_base: int) -> Frames:
+    """As make_frames, for a code given by its non-zero blocks."""
+    n = nb * Z
+    x = np.empty((n_frames, n), dtype=np.uint8)
+    llr = np.empty((n_frames, n), dtype=np.float32)
+    for k in range(n_frames):
+        rng = np.random.default_rng(seed_base + k)
+        x[k] = rng.integers(0, 2, size=n, dtype=np.uint8)
+        y = (1.0 - 2.0 * x[k].astype(np.float64)) + sigma * rng.standard_normal(n)
+        llr[k] = (2.0 * y / (sigma * sigma)).astype(np.float32)
+    return Frames(x=x, syndrome=syndrome_of_sparse(rows, cols, shifts, mb, nb, Z, x), llr=llr, sigma=sigma)
