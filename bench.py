@@ -66,9 +66,12 @@ def max_over_ranks(values_ms, dist, device):
     return [float(x) for x in t]
 
 
-def algorithmic_bytes(cfg_code: W.CodeSpec):
+def algorithmic_bytes(cfg_code):
     """Per frame-iteration: B_min = 8*E_core + 4*n + m/8, B_2ph = 16*E_core + 4*n + m/8."""
-    e_core = cfg_code.n_core * (cfg_code.top_deg + cfg_code.low_deg) * cfg_code.Z
+    if hasattr(cfg_code, "e_core"):
+        e_core = cfg_code.e_core
+    else:
+        e_core = cfg_code.n_core * (cfg_code.top_deg + cfg_code.low_deg) * cfg_code.Z
     b_min = 8 * e_core + 4 * cfg_code.n + cfg_code.m / 8
     b_2ph = 16 * e_core + 4 * cfg_code.n + cfg_code.m / 8
     return b_min, b_2ph
@@ -143,10 +146,15 @@ def oracle_sample(cfg: W.Config, base, Z, sigma, seed_base, sample_iters: int):
     import oracle
     cores = os.cpu_count() or 1
     frames_n = min(cores, cfg.n_frames)
-    fr = W.make_frames(base, Z, sigma, frames_n, seed_base)
+    sparse = isinstance(base, tuple)                     # (rows, cols, shifts, mb, nb): the NEXT-1 ensemble
+    fr = (W.make_frames_sparse(*base, Z, sigma, frames_n, seed_base) if sparse
+          else W.make_frames(base, Z, sigma, frames_n, seed_base))
     oracle.build()
     t0 = time.perf_counter()
-    res = oracle.decode(base, Z, fr.llr, fr.syndrome, sample_iters, cfg.early_stop, threads=frames_n)
+    if sparse:
+        res = oracle.decode_sparse(*base, Z, fr.llr, fr.syndrome, sample_iters, cfg.early_stop, threads=frames_n)
+    else:
+        res = oracle.decode(base, Z, fr.llr, fr.syndrome, sample_iters, cfg.early_stop, threads=frames_n)
     dt = time.perf_counter() - t0
     frame_iters = float(res.iters.sum())
     sec_per_frame_iter_all_cores = dt / max(frame_iters, 1.0)      # wall seconds per frame-iteration, all cores busy
@@ -182,8 +190,10 @@ def run_reference(args, cfg, base, Z, sigma, seed_base, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def workload_name(cfg: W.Config) -> str:
+def workload_name(cfg) -> str:
     sp = cfg.code
+    if hasattr(cfg, "ensemble_name"):
+        return cfg.ensemble_name
     return (f"BASELINE.json config {cfg.index}: rate-{sp.rate} QC multi-edge code {sp.nb}x{sp.mb} base, Z={sp.Z}, "
             f"n={sp.n}, {cfg.n_frames} frames, BIAWGN +{cfg.gaps_db[0]} dB over capacity, max {cfg.max_iter} "
             f"iterations, early stop {'on' if cfg.early_stop else 'off'}")
@@ -205,6 +215,9 @@ def main():
     ap.add_argument("--snr-point", type=int, default=0, help="index into the config's SNR points (config 5 has 6)")
     ap.add_argument("--check-from", type=int, default=1,
                     help="early-termination scheduling (P:514): run the syndrome test from this iteration on")
+    ap.add_argument("--ensemble", type=int, default=0, choices=[0, 21, 50],
+                    help="NEXT-1: decode the paper's own rate-0.02 multi-edge ensemble lifted by q = 21 (n = 1.008e6) "
+                         "or q = 50 (n = 1e6) at its beta = 0.99 operating point instead of a BASELINE.json config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
@@ -216,16 +229,32 @@ def main():
     if args.frames is not None or args.max_iter is not None:
         cfg = W.Config(cfg.index, cfg.code, args.frames or cfg.n_frames, args.max_iter or cfg.max_iter, cfg.early_stop,
                        cfg.gaps_db, cfg.description)
-    base = W.make_base_matrix(cfg.code)
+    ens = None
+    if args.ensemble:
+        # NEXT-1: the paper's ensemble at its own operating point: beta = 0.99, i.e. SNR s = 2^(2R/beta) - 1 (Eq. 11,
+        # P:231) = 0.02840 for R = 0.02, sigma = s^-1/2; max 500 iterations with early termination
+        from types import SimpleNamespace
+        q = args.ensemble
+        spec = W.paper_ensemble_spec(20000 if q == 50 else 48000, q)
+        ens = W.make_paper_ensemble(spec)
+        n_fr, mx = args.frames or 8, args.max_iter or 500
+        cfg = SimpleNamespace(
+            index=100 + q, n_frames=n_fr, max_iter=mx, early_stop=1, gaps_db=(0.0,),
+            code=SimpleNamespace(n=spec.n, m=spec.m, Z=q, e_core=(spec.base_edges - spec.n_d1) * q),
+            ensemble_name=(f"NEXT-1: the paper's rate-0.02 multi-edge ensemble (P:288-300), {spec.nb} base columns "
+                           f"(core degree 59/60) x {spec.mb} rows lifted by q={q}, n={spec.n}, {n_fr} frames, BIAWGN at "
+                           f"beta=0.99 (SNR 0.0284), max {mx} iterations, early stop on"))
+    base = W.make_base_matrix(cfg.code) if ens is None else None
     Z = cfg.code.Z
     if args.snr_point:
         cfg = W.Config(cfg.index, cfg.code, cfg.n_frames, cfg.max_iter, cfg.early_stop,
                        cfg.gaps_db[args.snr_point:args.snr_point + 1], cfg.description)
-    sigma = W.sigma_for_gap(cfg.code.rate, cfg.gaps_db[0])
+    sigma = (W.sigma_for_gap(cfg.code.rate, cfg.gaps_db[0]) if ens is None
+             else (2.0 ** (2.0 * 0.02 / 0.99) - 1.0) ** -0.5)
     seed_base = rank_seed_base(cfg.index, rank, args.snr_point)
 
     if args.impl == "reference":
-        run_reference(args, cfg, base, Z, sigma, seed_base, rank, world)
+        run_reference(args, cfg, base if ens is None else ens, Z, sigma, seed_base, rank, world)
         return
 
     import torch
@@ -246,8 +275,12 @@ def main():
         torch.cuda.synchronize(dev)
 
     # ---------------------------------------------------------------------------------------------- inputs
-    frames = W.make_frames(base, Z, sigma, cfg.n_frames, seed_base)
-    code = B.QCLDPCCode(base, Z)
+    if ens is None:
+        frames = W.make_frames(base, Z, sigma, cfg.n_frames, seed_base)
+        code = B.QCLDPCCode(base, Z)
+    else:
+        frames = W.make_frames_sparse(*ens, Z, sigma, cfg.n_frames, seed_base)
+        code = B.QCLDPCCode.from_sparse(*ens, Z)
     F, n, m = cfg.n_frames, code.n, code.m
     h_llr = torch.from_numpy(frames.llr).pin_memory()
     h_syn = torch.from_numpy(frames.syndrome).pin_memory()
@@ -348,7 +381,7 @@ def main():
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        mbit, cores, desc, dt = oracle_sample(cfg, base, Z, sigma, seed_base, args.ref_iters)
+        mbit, cores, desc, dt = oracle_sample(cfg, base if ens is None else ens, Z, sigma, seed_base, args.ref_iters)
         cpu_baseline = {"value": mbit, "unit": "Mbit/s", "cores": cores, "kind": "oracle", "sample": desc,
                         "sample_seconds": dt}
 

@@ -59,6 +59,7 @@ struct PassArgs {
     int* topbad;               // [F]  slot of the input iteration: set to 1 if a parity of a row without absorbed variable fails
     int in_buf, out_buf;       // regular pass: qb[in_buf] -> qb[out_buf]
     int Z, Zs, tiles;
+    int table_bytes, max_dv;   // generic kernel: bytes of its shared-memory tables; messages [max_dv][TB] follow
     int64_t n, EZs, mZs, AZs;  // per-frame strides
 };
 
@@ -80,7 +81,7 @@ struct HostTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc*
 struct PassLaunch {
     PassTables tab; PassArgs args; dim3 grid; cudaStream_t stream; int V; bool final_mode;
     const void* exact;         // HOST: the ExactTable of the instantiation (exact families only)
-    int n_cols, n_frames;
+    int n_cols, n_frames, max_np, max_dv;
 };
 using PassLauncher = void (*)(const PassLaunch&);
 using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only

@@ -1,20 +1,19 @@
 // k_pass -- steps a1 + a2 (+ the cheap part of a3) of the hot path: one flooding iteration of Algorithm 1 (steps 2-4,
-// P:348-363), fused and VN-centric, for ANY code the handle accepts (active column degree <= kMaxDv, any row degree).
-// Codes whose columns all have one of the BASELINE.json shapes run k_pass_exact (pass_exact.cuh: same arithmetic,
-// compile-time degrees, tables in the kernel parameters).  One CTA = one tile of kThreads consecutive variables of one
-// active column.
+// P:348-363), fused and VN-centric, for ANY code the handle accepts (active column degree <= kMaxDv, any row degree,
+// any Z): the correctness path for general codes and the path of the paper's own ensemble (NEXT-1: ~800 active
+// columns of degree 59/60 per 20,000, circulants of q = 21 or 50).  Codes whose columns all have one of
+// the BASELINE.json shapes run k_pass_exact (pass_exact.cuh) instead.
 //
-// The thread of variable v = (column C, index i) needs, for each of its edges (c,v), the messages of the OTHER edges
-// of check c from the previous iteration, plus the static term t_c.  Both are cyclic runs in i; thanks to the halo
-// behind every run (common.cuh) the window a tile reads is contiguous, so its start is block-uniform: the preamble
-// computes it once per edge into shared memory and the per-thread cost of an access is one 64-bit multiply-add.
-//   phase 1  loads: t of every row, the partner of every pair row
-//   phase 2  gen rows (the rows that are not "two active edges + one absorbed variable"): fold the partners into
-//            one equivalent q; the row's counter edge also forms the parity of the PREVIOUS iteration's hard
-//            decisions from the bit-0 tags (rows without absorbed variable only: the cheap early-exit filter)
-//   phase 3  check-node rule per edge
-//   phase 4  variable-node rule: L_v, xhat_v, every L_vc by prefix/suffix sums (direct
-//            exclusion, no total-minus-self); writes w(L_vc), aligned and coalesced
+// One CTA = TB consecutive variables of one active column of one frame (TB = 32, 64 or 128: the smallest that covers Z,
+// so that circulants of 21 or 50 do not idle most of a 128-thread block).  Runs are stored compactly (no halo); a tile
+// reads the cyclic window [x0, x0 + TB) of a run with one compare-subtract per element, x0 block-uniform from the
+// preamble (tables in shared memory).
+//   edges are processed in chunks of kChunk with all loads of a chunk in flight: t of the row, then either the single
+//   partner (pair row: two active edges + one absorbed variable) or the fold of all other edges of a gen row; the
+//   row's counter edge also forms the parity of the PREVIOUS iteration's hard decisions from the bit-0 tags;
+//   check-node rule per edge -> m[k] (registers, compile-time indexed);
+//   variable-node rule: L_v = Q_v + sum m, xhat_v, L_vc = L_v - m_cv (the LLR-domain difference is
+//   benign: |m| <= 30; the cancellation hazard of SURVEY N3 is on the check-node side, where exclusion stays direct).
 // FINAL = true: same arithmetic on each frame's frozen state, writes the outputs (hard bits, posterior) instead.
 #pragma once
 
@@ -22,11 +21,31 @@
 
 namespace qc {
 
-template <bool FINAL>
-__global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const PassArgs a) {
-    __shared__ int2 s_eo[kMaxDv];
-    __shared__ GenDesc s_gd[kMaxDv];
-    __shared__ int s_po[kMaxPartners];
+constexpr int kChunk = 8;
+constexpr int kGenSlots = 2;                                 // partners of a gen edge loaded with its chunk
+
+struct StreamDesc { int base, x0; };                         // w[base + (x0 + tid) mod Z]; base = -1: none
+
+// dynamic shared memory: stream tables, then the messages m'_cv of the tile, [max_dv][TB] floats
+inline size_t pass_any_table_bytes(int max_np) {
+    return (size_t)kMaxDv * (2 * sizeof(StreamDesc) + sizeof(GenDesc)) + (size_t)(max_np > 0 ? max_np : 1) * sizeof(StreamDesc);
+}
+inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups) {
+    return pass_any_table_bytes(max_np) + (size_t)((max_dv > 0 ? max_dv : 1) + groups) * tb * sizeof(float);
+}
+
+// G = edge groups: the CTA is TB x G threads, thread (tid, grp) handles the chunks grp, grp + G, ... of the column's
+// edges, so a column of degree 60 is four chains of 15 edges instead of one of 60 (the pass of a single frame is bound
+// by that chain's latency); the partial sums of the groups meet in shared memory.
+template <int TB, int G, bool FINAL>
+__global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const PassArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_any[];
+    StreamDesc* const s_t = reinterpret_cast<StreamDesc*>(smem_any);          // [kMaxDv] t of edge k
+    StreamDesc* const s_p = s_t + kMaxDv;                                     // [kMaxDv] partner of pair edge k
+    GenDesc* const s_gd = reinterpret_cast<GenDesc*>(s_p + kMaxDv);           // [kMaxDv] gen edges
+    StreamDesc* const s_po = reinterpret_cast<StreamDesc*>(s_gd + kMaxDv);    // [np] partners of the gen edges
+    float* const s_m = reinterpret_cast<float*>(smem_any + a.table_bytes) + threadIdx.x;   // m'_cv of edge k: s_m[k * TB]
+    float* const s_part = reinterpret_cast<float*>(smem_any + a.table_bytes) + a.max_dv * TB;   // [G][TB] partial sums
 
     pdl_launch();
     pdl_wait();
@@ -45,108 +64,160 @@ __global__ void __launch_bounds__(kThreads) k_pass(const PassTables tab, const P
     const ColDesc cd = tab.col[ca];
     const int Z = a.Z, Zs = a.Zs;
     const int dv = cd.dv, ng = cd.ng;
-    const int tid = threadIdx.x;
-    const int i0 = tile * kThreads;
+    const int tid = threadIdx.x, grp = threadIdx.y;
+    const int flat = grp * TB + tid;
+    const int i0 = tile * TB;
     const int i = i0 + tid;
+    const bool valid = i < Z;
+    const int lane = valid ? tid : 0;                        // idle threads read element 0 of every window
 
-    // preamble: window starts of this tile, once per edge
-    if (tid < dv) {
-        const EdgeDesc d = tab.edge[cd.ebeg + tid];
-        int r0 = i0 - d.shift; r0 += (r0 < 0) ? Z : 0;       // check index of the tile's first variable
-        int qo = -1;
-        if (d.p_off >= 0) { int x = i0 + d.delta; x -= (x >= Z) ? Z : 0; qo = d.p_off + x; }
-        s_eo[tid] = make_int2(qo < 0 ? -1 : 4 * qo, 4 * (d.t_off + r0));    // byte offsets
+    // preamble: window starts of this tile, once per stream
+    for (int k = flat; k < dv; k += TB * G) {
+        const EdgeDesc d = tab.edge[cd.ebeg + k];
+        int r0 = (i0 - d.shift) % Z; r0 += (r0 < 0) ? Z : 0;  // check index of the tile's first variable
+        s_t[k] = StreamDesc{d.t_off, r0};
+        s_p[k] = StreamDesc{d.p_off, d.p_off >= 0 ? (i0 + d.delta) % Z : 0};
     }
-    if (tid < ng) s_gd[tid] = tab.gen[cd.gbeg + tid];
-#pragma unroll 1
-    for (int j = tid; j < cd.np; j += kThreads) {
+    for (int g = flat; g < ng; g += TB * G) s_gd[g] = tab.gen[cd.gbeg + g];
+    for (int j = flat; j < cd.np; j += TB * G) {
         const PartnerDesc p = tab.partner[cd.pbeg + j];
-        int x = i0 + p.delta; x -= (x >= Z) ? Z : 0;
-        s_po[j] = 4 * (p.off + x);
+        s_po[j] = StreamDesc{p.off, (i0 + p.delta) % Z};
     }
     __syncthreads();
 
-    const float* __restrict__ qP = a.qb[in_buf] + (int64_t)f * a.EZs + tid;
-    const float* __restrict__ tP = a.t + (int64_t)f * a.mZs + tid;
-    const bool valid = i < Z;
+    const float* __restrict__ qP = a.qb[in_buf] + (int64_t)f * a.EZs;
+    const float* __restrict__ tP = a.t + (int64_t)f * a.mZs;
+    auto at = [&](const float* __restrict__ p, const StreamDesc sd) {
+        int idx = sd.x0 + lane; idx -= (idx >= Z) ? Z : 0;
+        return __ldg(p + sd.base + idx);
+    };
     const float Q = valid ? llr_to_log2(__ldg(a.llr + (int64_t)f * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
-    const unsigned xb = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] : 0u;
+    const unsigned xb = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
 
-    // phase 1: loads
-    float tv[kMaxDv], wv[kMaxDv];
-#pragma unroll 1
-    for (int k = 0; k < dv; ++k) {
-        const int2 o = s_eo[k];
-        tv[k] = __ldg(byte_ptr(tP, o.y));
-        if (o.x != -1) wv[k] = __ldg(byte_ptr(qP, o.x));
-    }
-
-    // phase 2: gen rows: fold the partners into one equivalent q (the rule is associative); bit 0 of a gen edge's
-    // state is its variable's hard decision, so the XOR of the raw words carries sign product AND parity
+    // the chunk loop is NOT unrolled: a fully unrolled body for 64 edges is 170 KB of code and the pass becomes bound
+    // by instruction fetch; the messages of the tile wait in shared memory for the variable-node rule instead
+    float sum = 0.0f;
     unsigned bad = 0;
 #pragma unroll 1
-    for (int g = 0; g < ng; ++g) {
-        const GenDesc gd = s_gd[g];
-        float num = 0.0f, den = 1.0f;
-        unsigned xa = 0u;
-#pragma unroll 4
-        for (int j = 0; j < gd.np; ++j) {
-            const unsigned wb = __float_as_uint(__ldg(byte_ptr(qP, s_po[gd.pbeg + j])));
-            xa ^= wb;
-            boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+    for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
+        {
+            float tv[kChunk], wv[kChunk], pw[kChunk][kGenSlots];
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) {               // loads of the chunk, back to back
+                const int k = k0 + j;
+                tv[j] = 0.0f; wv[j] = 0.0f;
+#pragma unroll
+                for (int jj = 0; jj < kGenSlots; ++jj) pw[j][jj] = 0.0f;
+                if (k < dv) {
+                    tv[j] = at(tP, s_t[k]);
+                    if (k >= ng) {
+                        wv[j] = at(qP, s_p[k]);
+                    } else {                                 // gen edge: its first kGenSlots partners travel with the
+                        const GenDesc gd = s_gd[k];          // chunk's other loads (empty slot: +0.0, the identity)
+#pragma unroll
+                        for (int jj = 0; jj < kGenSlots; ++jj)
+                            if (jj < gd.np) pw[j][jj] = at(qP, s_po[gd.pbeg + jj]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) {
+                const int k = k0 + j;
+                if (k < ng) {
+                    // gen row: fold the other edges into one equivalent q (the rule is associative); bit 0 of a gen
+                    // edge's state is its variable's hard decision: the XOR of the raw words carries sign AND parity
+                    const GenDesc gd = s_gd[k];
+                    float num = 0.0f, den = 1.0f;
+                    unsigned xa = 0u;
+#pragma unroll
+                    for (int jj = 0; jj < kGenSlots; ++jj) {
+                        const unsigned wb = __float_as_uint(pw[j][jj]);
+                        xa ^= wb;
+                        boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+                    }
+#pragma unroll 1
+                    for (int jj = kGenSlots; jj < gd.np; ++jj) {   // rows of degree > kGenSlots + 1
+                        const unsigned wb = __float_as_uint(at(qP, s_po[gd.pbeg + jj]));
+                        xa ^= wb;
+                        boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+                    }
+                    wv[j] = with_sign(num * rcp_approx(den), xa & 0x80000000u);
+                    if (!FINAL && gd.counter)    // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
+                        bad |= (xa ^ xb ^ (__float_as_uint(tv[j]) >> 31)) & (valid ? 1u : 0u);
+                }
+                // check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
+                const float qa = fabsf(wv[j]), tt = fabsf(tv[j]);
+                const float mag = mag_of(qa + tt, fmaf(qa, tt, 1.0f));
+                if (k < dv) {
+                    const float mk = with_sign(mag, sign_of(wv[j]) ^ sign_of(tv[j]));
+                    s_m[k * TB] = mk;
+                    sum += mk;
+                }
+            }
         }
-        wv[g] = with_sign(num * rcp_approx(den), xa & 0x80000000u);
-        if (!FINAL && gd.counter)    // parity of the row at the input iteration: s_c ^ XOR xhat (t = (-1)^{s_c} 0)
-            bad |= (xa ^ xb ^ (__float_as_uint(tv[g]) >> 31)) & (valid ? 1u : 0u);
     }
 
-    // phase 3: check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
-#pragma unroll 1
-    for (int k = 0; k < dv; ++k) {
-        const float qa = fabsf(wv[k]), tt = fabsf(tv[k]);
-        const float mag = mag_of(qa + tt, fmaf(qa, tt, 1.0f));
-        tv[k] = with_sign(mag, sign_of(wv[k]) ^ sign_of(tv[k]));   // tv now holds m'_cv
+    // variable-node rule
+    if (G > 1) {                                             // the groups' partial sums meet here, in a fixed order
+        s_part[grp * TB + tid] = sum;
+        __syncthreads();
+        sum = 0.0f;
+#pragma unroll
+        for (int g = 0; g < G; ++g) sum += s_part[g * TB + tid];
     }
-
-    // phase 4: variable-node rule
-    float suf[kMaxDv + 1];
-    suf[dv] = 0.0f;
-#pragma unroll 1
-    for (int k = dv - 1; k >= 0; --k) suf[k] = suf[k + 1] + tv[k];
-    const float L = Q + suf[0];                              // L'_v
+    const float L = Q + sum;                                 // L'_v
     const unsigned xh = __float_as_uint(L) >> 31;            // 0 iff L_v >= 0
     if (FINAL) {
-        if (valid) {
+        if (valid && grp == 0) {
             const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + i;
             a.d_hard[vv] = (uint8_t)xh;
             if (a.d_post) a.d_post[vv] = L * kLn2;
         }
         return;
     }
-    a.hard_out[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh;
+    if (valid && grp == 0) a.hard_out[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh;
     if (ng > 0 && __any_sync(0xffffffffu, bad != 0) && (tid & 31) == 0) a.topbad[f] = 1;
 
-    // tiles that own the first kHalo entries of the run write them twice (run + halo)
-    const int nrep = (i0 < kHalo) ? 2 : 1;
+    float* __restrict__ sp = a.qb[a.out_buf] + (int64_t)f * a.EZs + (int64_t)cd.ebeg * Zs + (valid ? i : 0);
 #pragma unroll 1
-    for (int rep = 0; rep < nrep; ++rep) {
-        float* __restrict__ sp = a.qb[a.out_buf] + (int64_t)f * a.EZs + (int64_t)cd.ebeg * Zs + (rep ? Z : 0) + i;
-        float run = Q;
-#pragma unroll 1
-        for (int k = 0; k < dv; ++k) {
-            const float Lvc = run + suf[k + 1];              // Q + sum_{k' != k} m_k'
-            run += tv[k];
-            unsigned wb = __float_as_uint(w_of(Lvc));
-            if (k < ng) wb = (wb & 0xfffffffeu) | xh;        // gen edge: tag with the hard decision
-            if (valid) *sp = __uint_as_float(wb);
-            sp = byte_ptr(sp, 4u * Zs);
+    for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            const int k = k0 + j;
+            if (k < dv) {
+                const float Lvc = (dv == 1) ? Q : L - s_m[k * TB];   // Q + sum_{k' != k} m_k' (one edge: Q)
+                unsigned wb = __float_as_uint(w_of(Lvc));
+                if (k < ng) wb = (wb & 0xfffffffeu) | xh;    // gen edge: tag with the hard decision
+                if (valid) sp[(int64_t)k * Zs] = __uint_as_float(wb);
+            }
         }
     }
 }
 
+template <int TB, int G>
+inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
+    args.tiles = (args.Z + TB - 1) / TB;
+    args.max_dv = L.max_dv > 0 ? L.max_dv : 1;
+    const size_t smem = pass_any_smem(L.max_np, L.max_dv, TB, G);
+    static thread_local bool attr_set = false;
+    if (!attr_set) {            // tables (<= 18.4 KB) + messages (<= 32 KB) can exceed the 48 KB default
+        cudaFuncSetAttribute(k_pass<TB, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(k_pass<TB, G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        attr_set = true;
+    }
+    const dim3 grid(args.tiles * L.n_cols, L.n_frames), block(TB, G);
+    if (L.final_mode) k_pass<TB, G, true><<<grid, block, smem, L.stream>>>(L.tab, args);
+    else launch_pdl(k_pass<TB, G, false>, grid, block, smem, L.stream, L.tab, args);
+}
+
 inline void launch_pass_any(const PassLaunch& L) {
-    if (L.final_mode) k_pass<true><<<L.grid, kThreads, 0, L.stream>>>(L.tab, L.args);
-    else launch_pdl(k_pass<false>, L.grid, dim3(kThreads), 0, L.stream, L.tab, L.args);
+    PassArgs args = L.args;
+    args.table_bytes = (int)pass_any_table_bytes(L.max_np);
+    const int Z = args.Z;
+    const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
+    if (Z <= 32) { if (split) launch_pass_tb<32, 4>(L, args); else launch_pass_tb<32, 1>(L, args); }
+    else if (Z <= 64) { if (split) launch_pass_tb<64, 4>(L, args); else launch_pass_tb<64, 1>(L, args); }
+    else { if (split) launch_pass_tb<128, 4>(L, args); else launch_pass_tb<128, 1>(L, args); }
 }
 
 }  // namespace qc

@@ -61,6 +61,7 @@ thread_local Profile g_prof;
 
 struct qcldpc_code {
     int mb, nb, Z, Zs, tiles;             // tiles = ceil(Z / kThreads)
+    int halo = 0, max_np = 0;             // halo: runs are followed by kHalo wrapped entries (exact families)
     int64_t n, m;
     int n_act_cols, n_act_edges, max_dv;
     bool filter_rows;                     // some row has no absorbed variable (the early-exit filter exists)
@@ -81,7 +82,7 @@ namespace {
 
 struct InitArgs {
     const float* llr; const uint8_t* syn; float* q0; float* t; uint8_t* hard0; uint8_t* d_hard; float* d_post;
-    int Z, Zs, tiles; int64_t n, m, EZs, mZs, AZs;
+    int Z, Zs, tiles, halo; int64_t n, m, EZs, mZs, AZs;
 };
 
 // a0: w^(0) on every active edge, decisions at t = 0 for active variables.  One thread per (active column, index).
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(kThreads) k_init_cols(const PassTables tab, co
     const unsigned xh = __float_as_uint(Q2) >> 31;
     const unsigned wb = __float_as_uint(w_of(Q2));
     float* q0 = a.q0 + (int64_t)f * a.EZs + (int64_t)cd.ebeg * a.Zs;
-    const bool halo = i < kHalo;
+    const bool halo = a.halo && i < kHalo;
     for (int k = 0; k < cd.dv; ++k) {
         const float w = __uint_as_float(k < cd.ng ? ((wb & 0xfffffffeu) | xh) : wb);
         q0[(int64_t)k * a.Zs + i] = w;
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(kThreads) k_init_rows(const CheckTables tab, c
     const float ts = __uint_as_float(__float_as_uint(t) ^ (s << 31));
     float* tf = a.t + (int64_t)f * a.mZs + (int64_t)R * a.Zs;
     tf[r] = ts;
-    if (r < kHalo) tf[a.Z + r] = ts;
+    if (a.halo && r < kHalo) tf[a.Z + r] = ts;
 }
 
 struct CheckArgs {
@@ -369,9 +370,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     qcldpc_code* code = new (std::nothrow) qcldpc_code();
     if (!code) return QCLDPC_ERR_ALLOC;
     code->mb = mb; code->nb = nb; code->Z = Z;
-    code->Zs = (int)align_up((size_t)Z + kHalo, 32);
     code->n = (int64_t)nb * Z; code->m = (int64_t)mb * Z;
-    const int Zs = code->Zs;
 
     // absorb at most one degree-1 column per row (the lowest-numbered one)
     std::vector<int> absorbed_by(nb, -1), n_active(mb, 0);
@@ -422,6 +421,15 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     }
     code->n_act_cols = (int)code->col.size();
     code->n_act_edges = (int)edges.size();
+    // kernel family: exact instantiations for the column shapes of the BASELINE.json codes (runs stored with a halo of
+    // kHalo wrapped entries, common.cuh), else the generic kernel (compact runs, per-element wrap)
+    bool uniform = code->n_act_cols > 0;
+    for (const ColDesc& cd : code->col) uniform = uniform && cd.dv == code->col[0].dv && cd.ng == code->col[0].ng;
+    const bool exact = uniform && code->n_act_cols <= kMaxExactCols && code->col[0].ng == 3 &&
+                       (code->col[0].dv == 11 || code->col[0].dv == 21);
+    code->halo = exact ? 1 : 0;
+    code->Zs = (int)align_up((size_t)Z + (exact ? kHalo : 0), 32);
+    const int Zs = code->Zs;
     if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Zs >= ((int64_t)1 << 31) ||
         (int64_t)mb * Zs >= ((int64_t)1 << 31)) {
         delete code;
@@ -474,11 +482,9 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     if (!partners_ok) { delete code; return QCLDPC_ERR_UNSUPPORTED; }
 
     // kernel choice: exact instantiations for the column shapes of the BASELINE.json codes, else the generic one
-    bool uniform = code->n_act_cols > 0;
-    for (const ColDesc& cd : code->col) uniform = uniform && cd.dv == code->col[0].dv && cd.ng == code->col[0].ng;
     code->launcher = launch_pass_generic;
-    if (uniform && code->n_act_cols <= kMaxExactCols && code->col[0].ng == 3 &&
-        (code->col[0].dv == 11 || code->col[0].dv == 21)) {
+    code->max_np = max_np;
+    if (exact) {
         code->launcher = code->col[0].dv == 11 ? launch_pass_dv11_ng3 : launch_pass_dv21_ng3;
         const ExactBuilder fill = code->col[0].dv == 11 ? launch_pass_dv11_ng3_table : launch_pass_dv21_ng3_table;
         const HostTables ht{code->edge.data(), code->gen.data(), code->partner.data(), code->col.data(),
@@ -559,7 +565,7 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
     k_reset<<<fblocks, 128, 0, st>>>(w.done, w.unsat, w.topbad, w.fullbad, w.ticket, d_iters, d_pass, n_frames, max_iter);
     ++g_launches;
     const InitArgs ia{d_llr, d_syndrome, w.qbuf[0], w.t, w.hardbuf[0], d_hard, d_posterior,
-                      Z, Zs, tiles1, code->n, code->m, EZs, mZs, AZs};
+                      Z, Zs, tiles1, code->halo, code->n, code->m, EZs, mZs, AZs};
     if (code->n_act_cols > 0) {
         k_init_cols<<<dim3(tiles1 * code->n_act_cols, n_frames), kThreads, 0, st>>>(ptab, ia);
         ++g_launches;
@@ -578,9 +584,9 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
     }
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
-                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, code->n, EZs, mZs, AZs},
+                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, code->n, EZs, mZs, AZs},
                   dim3(code->tiles * code->n_act_cols, n_frames), st, V, false,
-                  code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames};
+                  code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames, code->max_np, code->max_dv};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
                  d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
                  n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
