@@ -85,8 +85,13 @@ __global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const Pas
     }
     __syncthreads();
 
-    const float* __restrict__ qP = a.qb[in_buf] + (int64_t)f * a.EZs;
-    const float* __restrict__ tP = a.t + (int64_t)f * a.mZs;
+    // opaque to the optimiser: otherwise the two frame pointers are re-formed (64-bit multiply, constant loads) at
+    // every one of the ~150 loads of a thread
+    unsigned long long qP_u = reinterpret_cast<unsigned long long>(a.qb[in_buf] + (int64_t)f * a.EZs);
+    unsigned long long tP_u = reinterpret_cast<unsigned long long>(a.t + (int64_t)f * a.mZs);
+    asm volatile("" : "+l"(qP_u), "+l"(tP_u));
+    const float* __restrict__ qP = reinterpret_cast<const float*>(qP_u);
+    const float* __restrict__ tP = reinterpret_cast<const float*>(tP_u);
     auto at = [&](const float* __restrict__ p, const StreamDesc sd) {
         int idx = sd.x0 + lane; idx -= (idx >= Z) ? Z : 0;
         return __ldg(p + sd.base + idx);
