@@ -324,3 +324,47 @@ def test_gpu_argument_errors(B):
     assert ei.value.status == -1
     with pytest.raises(ValueError):
         code.decode(d_llr[:, :-1], d_syn, 5, 0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("which", ["config1_exact", "ensemble_generic"])
+def test_gpu_no_writes_outside_the_buffers(B, which):
+    """compute-sanitizer is not available on the GPU pool: guard bands instead.  Every buffer handed to the C ABI sits
+    inside a larger allocation whose surroundings are filled with a pattern; nothing outside may change, and the
+    result must equal the plain call's."""
+    if which == "config1_exact":
+        cfg, base, Z, fr = W.make_config(1)
+        code = B.QCLDPCCode(base, Z)
+        llr, syn = fr.llr, fr.syndrome
+    else:
+        spec = W.paper_ensemble_spec(400, 50)
+        ens = W.make_paper_ensemble(spec)
+        fr = W.make_frames_sparse(*ens, 50, W.sigma_for_gap(0.02, 2.0), 5, 31337)
+        code = B.QCLDPCCode.from_sparse(*ens, 50)
+        llr, syn = fr.llr, fr.syndrome
+    F, n, m = llr.shape[0], code.n, code.m
+    G = 4096                                               # guard bytes (a multiple of 256: keeps the alignment)
+
+    def guarded(nbytes, dtype):
+        raw = torch.full((G + nbytes + G,), 0xAB, dtype=torch.uint8, device="cuda")
+        return raw, raw[G:G + nbytes].view(dtype)
+
+    need = code.workspace_bytes(F)
+    need_al = (need + 255) // 256 * 256
+    ws_raw, ws = guarded(need_al, torch.uint8)
+    hard_raw, hard = guarded(F * n, torch.uint8)
+    it_raw, iters = guarded(F * 4, torch.int32)
+    ps_raw, passed = guarded((F + 255) // 256 * 256, torch.uint8)
+    po_raw, post = guarded(F * n * 4, torch.float32)
+    out = B.DecodeResult(hard.view(F, n), iters, passed[:F], post.view(F, n))
+    d_llr, d_syn = torch.from_numpy(llr).cuda(), torch.from_numpy(syn).cuda()
+    for early in (0, 1):
+        code.decode(d_llr, d_syn, 30, early, want_posterior=True, workspace=ws, out=out)
+        torch.cuda.synchronize()
+        ref = code.decode(d_llr, d_syn, 30, early, want_posterior=True)
+        torch.cuda.synchronize()
+        assert torch.equal(out.hard, ref.hard) and torch.equal(out.iters, ref.iters)
+        assert torch.equal(out.posterior, ref.posterior) and torch.equal(out.passed, ref.passed)
+        for raw, body in ((ws_raw, need_al), (hard_raw, F * n), (it_raw, F * 4), (ps_raw, (F + 255) // 256 * 256),
+                          (po_raw, F * n * 4)):
+            assert bool((raw[:G] == 0xAB).all()) and bool((raw[G + body:] == 0xAB).all())
