@@ -17,10 +17,11 @@ OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
-# (symbol, DV, NG): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
+# (symbol, DV, NG, PCAP): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
 # 11 or 21 edges, 3 of them into the top rows); pass_generic.cu takes any column of degree <= 64
-PCAP = int(os.environ.get("QCLDPC_PCAP", "4"))   # partner slots per gen edge held in registers (tuning knob)
-PASS_INSTANCES = [("launch_pass_dv11_ng3", 11, 3), ("launch_pass_dv21_ng3", 21, 3)]
+# partner slots per gen edge held in registers, per family (measured: config 2's top rows reach degree 9, configs
+# 3/4/5's degree 6; one more slot than that costs registers in the 21-edge kernel)
+PASS_INSTANCES = [("launch_pass_dv11_ng3", 11, 3, 6), ("launch_pass_dv21_ng3", 21, 3, 5)]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -28,9 +29,9 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 def _units():
     units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), []),
              (os.path.join(CSRC, "pass_generic.cu"), os.path.join(OBJDIR, "pass_generic.o"), [])]
-    for name, dv, ng in PASS_INSTANCES:
+    for name, dv, ng, pcap in PASS_INSTANCES:
         units.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJDIR, f"{name}.o"),
-                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={PCAP}"]))
+                      [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={pcap}"]))
     return units
 
 
