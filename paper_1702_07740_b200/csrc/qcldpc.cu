@@ -590,7 +590,11 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
                  d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
                  n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
-    const int cand_blocks = std::max(1, std::min(code->n_sm * 4, code->mb * tiles1));
+    // early-exit grid: persistent; small batches are launch-bound and almost never have a candidate, so a smaller grid
+    // (less to schedule and retire between two passes) wins there
+    const char* cb = getenv("QCLDPC_CAND_PER_SM");
+    const int cand_per_sm = cb ? std::max(1, atoi(cb)) : (n_frames <= 8 ? 1 : 4);
+    const int cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * tiles1));
 
     for (int t = 1; t <= max_iter; ++t) {
         if (code->n_act_cols > 0) {
