@@ -24,7 +24,106 @@ namespace qc {
 constexpr int kChunk = 8;
 constexpr int kGenSlots = 2;                                 // partners of a gen edge loaded with its chunk
 
-struct StreamDesc { int base, x0; };                         // w[base + (x0 + tid) mod Z]; base = -1: none
+struct StreamDesc { unsigned base, x0; };                     // element (x0 + lane) mod Z of the run at float index base
+
+template <int TB>
+struct PassCtx {
+    const float* qP; const float* tP;                        // this frame's edge state (input buffer) and static terms
+    const StreamDesc* s_t; const StreamDesc* s_p; const GenDesc* s_gd; const StreamDesc* s_po;
+    float* s_m;                                              // messages of this thread: s_m[k * TB]
+    unsigned lane, Z, xb;
+    int dv, ng;
+    bool valid;
+    float sum; unsigned bad;
+};
+
+#ifdef __CUDACC__
+// unsigned index arithmetic and one 32x32+64 multiply-add per address (runs start below 2^30 floats: code_create)
+__device__ __forceinline__ float load_stream(const float* p, const StreamDesc sd, unsigned lane, unsigned Z) {
+    unsigned idx = sd.x0 + lane;
+    idx -= (idx >= Z) ? Z : 0u;
+    return __ldg(byte_ptr(p, 4u * (sd.base + idx)));
+}
+
+// check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
+__device__ __forceinline__ float cn_rule(float wv, float tv) {
+    const float qa = fabsf(wv), tt = fabsf(tv);
+    return with_sign(mag_of(qa + tt, fmaf(qa, tt, 1.0f)), sign_of(wv) ^ sign_of(tv));
+}
+
+// One chunk of kChunk edges starting at edge k0: loads back to back, then the check-node rule, messages to shared memory.
+// MODE 1: all edges are pair edges (k0 >= ng, k0 + kChunk <= dv); MODE 2: all are gen edges (k0 + kChunk <= ng); MODE 0:
+// anything (per-edge predicates).
+template <int TB, bool FINAL, int MODE>
+__device__ __forceinline__ void chunk_cn(PassCtx<TB>& cx, const int k0) {
+    float tv[kChunk], wv[kChunk];
+    if (MODE == 1) {
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            tv[j] = load_stream(cx.tP, cx.s_t[k0 + j], cx.lane, cx.Z);
+            wv[j] = load_stream(cx.qP, cx.s_p[k0 + j], cx.lane, cx.Z);
+        }
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            const float mk = cn_rule(wv[j], tv[j]);
+            cx.s_m[(k0 + j) * TB] = mk;
+            cx.sum += mk;
+        }
+        return;
+    }
+    float pw[kChunk][kGenSlots];
+    int np[kChunk], pbeg[kChunk], ctr[kChunk];
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j) {                       // loads of the chunk, back to back
+        const int k = k0 + j;
+        tv[j] = 0.0f; wv[j] = 0.0f; np[j] = 0; pbeg[j] = 0; ctr[j] = 0;
+#pragma unroll
+        for (int jj = 0; jj < kGenSlots; ++jj) pw[j][jj] = 0.0f;
+        if (MODE == 2 || k < cx.dv) {
+            tv[j] = load_stream(cx.tP, cx.s_t[k], cx.lane, cx.Z);
+            if (MODE == 2 || k < cx.ng) {                    // gen edge: its first kGenSlots partners travel with the
+                const GenDesc gd = cx.s_gd[k];               // chunk's other loads (empty slot: +0.0, the identity)
+                np[j] = gd.np; pbeg[j] = gd.pbeg; ctr[j] = gd.counter;
+#pragma unroll
+                for (int jj = 0; jj < kGenSlots; ++jj)
+                    if (jj < gd.np) pw[j][jj] = load_stream(cx.qP, cx.s_po[gd.pbeg + jj], cx.lane, cx.Z);
+            } else {
+                wv[j] = load_stream(cx.qP, cx.s_p[k], cx.lane, cx.Z);
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j) {
+        const int k = k0 + j;
+        if (MODE == 2 || k < cx.ng) {
+            // gen row: fold the other edges into one equivalent q (the rule is associative); bit 0 of a gen edge's
+            // state is its variable's hard decision: the XOR of the raw words carries sign AND parity
+            float num = 0.0f, den = 1.0f;
+            unsigned xa = 0u;
+#pragma unroll
+            for (int jj = 0; jj < kGenSlots; ++jj) {
+                const unsigned wb = __float_as_uint(pw[j][jj]);
+                xa ^= wb;
+                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+            }
+#pragma unroll 1
+            for (int jj = kGenSlots; jj < np[j]; ++jj) {     // rows of degree > kGenSlots + 1
+                const unsigned wb = __float_as_uint(load_stream(cx.qP, cx.s_po[pbeg[j] + jj], cx.lane, cx.Z));
+                xa ^= wb;
+                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+            }
+            wv[j] = with_sign(num * rcp_approx(den), xa & 0x80000000u);
+            if (!FINAL && ctr[j])            // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
+                cx.bad |= (xa ^ cx.xb ^ (__float_as_uint(tv[j]) >> 31)) & (cx.valid ? 1u : 0u);
+        }
+        if (MODE == 2 || k < cx.dv) {
+            const float mk = cn_rule(wv[j], tv[j]);
+            cx.s_m[k * TB] = mk;
+            cx.sum += mk;
+        }
+    }
+}
+#endif
 
 // dynamic shared memory: stream tables, then the messages m'_cv of the tile, [max_dv][TB] floats
 inline size_t pass_any_table_bytes(int max_np) {
@@ -75,13 +174,13 @@ __global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const Pas
     for (int k = flat; k < dv; k += TB * G) {
         const EdgeDesc d = tab.edge[cd.ebeg + k];
         int r0 = (i0 - d.shift) % Z; r0 += (r0 < 0) ? Z : 0;  // check index of the tile's first variable
-        s_t[k] = StreamDesc{d.t_off, r0};
-        s_p[k] = StreamDesc{d.p_off, d.p_off >= 0 ? (i0 + d.delta) % Z : 0};
+        s_t[k] = StreamDesc{(unsigned)d.t_off, (unsigned)r0};
+        s_p[k] = StreamDesc{(unsigned)(d.p_off >= 0 ? d.p_off : 0), (unsigned)(d.p_off >= 0 ? (i0 + d.delta) % Z : 0)};
     }
     for (int g = flat; g < ng; g += TB * G) s_gd[g] = tab.gen[cd.gbeg + g];
     for (int j = flat; j < cd.np; j += TB * G) {
         const PartnerDesc p = tab.partner[cd.pbeg + j];
-        s_po[j] = StreamDesc{p.off, (i0 + p.delta) % Z};
+        s_po[j] = StreamDesc{(unsigned)p.off, (unsigned)((i0 + p.delta) % Z)};
     }
     __syncthreads();
 
@@ -90,77 +189,24 @@ __global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const Pas
     unsigned long long qP_u = reinterpret_cast<unsigned long long>(a.qb[in_buf] + (int64_t)f * a.EZs);
     unsigned long long tP_u = reinterpret_cast<unsigned long long>(a.t + (int64_t)f * a.mZs);
     asm volatile("" : "+l"(qP_u), "+l"(tP_u));
-    const float* __restrict__ qP = reinterpret_cast<const float*>(qP_u);
-    const float* __restrict__ tP = reinterpret_cast<const float*>(tP_u);
-    auto at = [&](const float* __restrict__ p, const StreamDesc sd) {
-        int idx = sd.x0 + lane; idx -= (idx >= Z) ? Z : 0;
-        return __ldg(p + sd.base + idx);
-    };
+    PassCtx<TB> cx;
+    cx.qP = reinterpret_cast<const float*>(qP_u); cx.tP = reinterpret_cast<const float*>(tP_u);
+    cx.s_t = s_t; cx.s_p = s_p; cx.s_gd = s_gd; cx.s_po = s_po; cx.s_m = s_m;
+    cx.lane = (unsigned)lane; cx.Z = (unsigned)Z; cx.dv = dv; cx.ng = ng;
+    cx.xb = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
+    cx.valid = valid; cx.sum = 0.0f; cx.bad = 0u;
     const float Q = valid ? llr_to_log2(__ldg(a.llr + (int64_t)f * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
-    const unsigned xb = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
 
-    // the chunk loop is NOT unrolled: a fully unrolled body for 64 edges is 170 KB of code and the pass becomes bound
-    // by instruction fetch; the messages of the tile wait in shared memory for the variable-node rule instead
-    float sum = 0.0f;
-    unsigned bad = 0;
+    // The chunk loop is NOT unrolled (a fully unrolled body for 64 edges is 170 KB of code: the pass becomes bound by
+    // instruction fetch); the messages of the tile wait in shared memory for the variable-node rule instead.  A chunk
+    // whose 8 edges are all pair edges, or all gen edges, runs a body without per-edge predicates.
 #pragma unroll 1
     for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
-        {
-            float tv[kChunk], wv[kChunk], pw[kChunk][kGenSlots];
-#pragma unroll
-            for (int j = 0; j < kChunk; ++j) {               // loads of the chunk, back to back
-                const int k = k0 + j;
-                tv[j] = 0.0f; wv[j] = 0.0f;
-#pragma unroll
-                for (int jj = 0; jj < kGenSlots; ++jj) pw[j][jj] = 0.0f;
-                if (k < dv) {
-                    tv[j] = at(tP, s_t[k]);
-                    if (k >= ng) {
-                        wv[j] = at(qP, s_p[k]);
-                    } else {                                 // gen edge: its first kGenSlots partners travel with the
-                        const GenDesc gd = s_gd[k];          // chunk's other loads (empty slot: +0.0, the identity)
-#pragma unroll
-                        for (int jj = 0; jj < kGenSlots; ++jj)
-                            if (jj < gd.np) pw[j][jj] = at(qP, s_po[gd.pbeg + jj]);
-                    }
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < kChunk; ++j) {
-                const int k = k0 + j;
-                if (k < ng) {
-                    // gen row: fold the other edges into one equivalent q (the rule is associative); bit 0 of a gen
-                    // edge's state is its variable's hard decision: the XOR of the raw words carries sign AND parity
-                    const GenDesc gd = s_gd[k];
-                    float num = 0.0f, den = 1.0f;
-                    unsigned xa = 0u;
-#pragma unroll
-                    for (int jj = 0; jj < kGenSlots; ++jj) {
-                        const unsigned wb = __float_as_uint(pw[j][jj]);
-                        xa ^= wb;
-                        boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
-                    }
-#pragma unroll 1
-                    for (int jj = kGenSlots; jj < gd.np; ++jj) {   // rows of degree > kGenSlots + 1
-                        const unsigned wb = __float_as_uint(at(qP, s_po[gd.pbeg + jj]));
-                        xa ^= wb;
-                        boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
-                    }
-                    wv[j] = with_sign(num * rcp_approx(den), xa & 0x80000000u);
-                    if (!FINAL && gd.counter)    // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
-                        bad |= (xa ^ xb ^ (__float_as_uint(tv[j]) >> 31)) & (valid ? 1u : 0u);
-                }
-                // check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
-                const float qa = fabsf(wv[j]), tt = fabsf(tv[j]);
-                const float mag = mag_of(qa + tt, fmaf(qa, tt, 1.0f));
-                if (k < dv) {
-                    const float mk = with_sign(mag, sign_of(wv[j]) ^ sign_of(tv[j]));
-                    s_m[k * TB] = mk;
-                    sum += mk;
-                }
-            }
-        }
+        if (k0 >= ng && k0 + kChunk <= dv) chunk_cn<TB, FINAL, 1>(cx, k0);
+        else if (k0 + kChunk <= ng) chunk_cn<TB, FINAL, 2>(cx, k0);
+        else chunk_cn<TB, FINAL, 0>(cx, k0);
     }
+    float sum = cx.sum;
 
     // variable-node rule
     if (G > 1) {                                             // the groups' partial sums meet here, in a fixed order
@@ -181,19 +227,29 @@ __global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const Pas
         return;
     }
     if (valid && grp == 0) a.hard_out[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh;
-    if (ng > 0 && __any_sync(0xffffffffu, bad != 0) && (tid & 31) == 0) a.topbad[f] = 1;
+    if (ng > 0 && __any_sync(0xffffffffu, cx.bad != 0) && (tid & 31) == 0) a.topbad[f] = 1;
 
-    float* __restrict__ sp = a.qb[a.out_buf] + (int64_t)f * a.EZs + (int64_t)cd.ebeg * Zs + (valid ? i : 0);
+    float* const sp = a.qb[a.out_buf] + (int64_t)f * a.EZs + (int64_t)cd.ebeg * Zs + (valid ? i : 0);
+    const unsigned Zs4 = 4u * (unsigned)Zs;
+    const bool single = dv == 1;                             // a single edge sends Q itself
 #pragma unroll 1
     for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
+        if (k0 >= ng && k0 + kChunk <= dv) {                 // eight pair edges: no tags, no bounds
 #pragma unroll
-        for (int j = 0; j < kChunk; ++j) {
-            const int k = k0 + j;
-            if (k < dv) {
-                const float Lvc = (dv == 1) ? Q : L - s_m[k * TB];   // Q + sum_{k' != k} m_k' (one edge: Q)
-                unsigned wb = __float_as_uint(w_of(Lvc));
-                if (k < ng) wb = (wb & 0xfffffffeu) | xh;    // gen edge: tag with the hard decision
-                if (valid) sp[(int64_t)k * Zs] = __uint_as_float(wb);
+            for (int j = 0; j < kChunk; ++j) {
+                const float Lvc = single ? Q : L - s_m[(k0 + j) * TB];   // Q + sum_{k' != k} m_k'
+                if (valid) *byte_ptr(sp, (unsigned)(k0 + j) * Zs4) = w_of(Lvc);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) {
+                const int k = k0 + j;
+                if (k < dv) {
+                    const float Lvc = single ? Q : L - s_m[k * TB];
+                    unsigned wb = __float_as_uint(w_of(Lvc));
+                    if (k < ng) wb = (wb & 0xfffffffeu) | xh;    // gen edge: tag with the hard decision
+                    if (valid) *byte_ptr(sp, (unsigned)k * Zs4) = __uint_as_float(wb);
+                }
             }
         }
     }

@@ -430,8 +430,10 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     code->halo = exact ? 1 : 0;
     code->Zs = (int)align_up((size_t)Z + (exact ? kHalo : 0), 32);
     const int Zs = code->Zs;
-    if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Zs >= ((int64_t)1 << 31) ||
-        (int64_t)mb * Zs >= ((int64_t)1 << 31)) {
+    // run offsets are formed as 32-bit BYTE offsets in the kernels: a frame's edge state and its static terms must each
+    // stay below 2^30 floats
+    if (code->max_dv > kMaxDv || (int64_t)code->n_act_edges * Zs >= ((int64_t)1 << 30) ||
+        (int64_t)mb * Zs >= ((int64_t)1 << 30)) {
         delete code;
         return QCLDPC_ERR_UNSUPPORTED;
     }
