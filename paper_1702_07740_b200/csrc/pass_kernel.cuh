@@ -137,7 +137,7 @@ inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups) {
 // edges, so a column of degree 60 is four chains of 15 edges instead of one of 60 (the pass of a single frame is bound
 // by that chain's latency); the partial sums of the groups meet in shared memory.
 template <int TB, int G, bool FINAL>
-__global__ void __launch_bounds__(TB * G) k_pass(const PassTables tab, const PassArgs a) {
+__global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTables tab, const PassArgs a) {
     extern __shared__ __align__(16) unsigned char smem_any[];
     StreamDesc* const s_t = reinterpret_cast<StreamDesc*>(smem_any);          // [kMaxDv] t of edge k
     StreamDesc* const s_p = s_t + kMaxDv;                                     // [kMaxDv] partner of pair edge k
