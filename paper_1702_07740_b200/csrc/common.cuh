@@ -59,7 +59,8 @@ struct PassArgs {
     int* topbad;               // [F]  slot of the input iteration: set to 1 if a parity of a row without absorbed variable fails
     int in_buf, out_buf;       // regular pass: qb[in_buf] -> qb[out_buf]
     int Z, Zs, tiles;
-    int table_bytes, max_dv;   // generic kernel: bytes of its shared-memory tables; messages [max_dv][TB] follow
+    int table_bytes, max_dv;   // generic kernel: bytes of its shared-memory tables; messages [max_dv][FV][TB] follow
+    int n_frames;              // generic kernel: frames of the batch (two per thread when batched)
     int64_t n, EZs, mZs, AZs;  // per-frame strides
 };
 

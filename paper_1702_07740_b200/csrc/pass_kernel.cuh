@@ -14,6 +14,8 @@
 //   check-node rule per edge -> m[k] (registers, compile-time indexed);
 //   variable-node rule: L_v = Q_v + sum m, xhat_v, L_vc = L_v - m_cv (the LLR-domain difference is
 //   benign: |m| <= 30; the cancellation hazard of SURVEY N3 is on the check-node side, where exclusion stays direct).
+// FV = 2 (batched decodes): a thread carries the same variable of TWO frames; the table lookups, window indices and
+// predicates -- most of this kernel's instructions -- are shared by the pair.
 // FINAL = true: same arithmetic on each frame's frozen state, writes the outputs (hard bits, posterior) instead.
 #pragma once
 
@@ -26,23 +28,23 @@ constexpr int kGenSlots = 2;                                 // partners of a ge
 
 struct StreamDesc { unsigned base, x0; };                     // element (x0 + lane) mod Z of the run at float index base
 
-template <int TB>
+template <int TB, int FV>
 struct PassCtx {
-    const float* qP; const float* tP;                        // this frame's edge state (input buffer) and static terms
+    const float* qP[FV]; const float* tP[FV];                // per frame: edge state (input buffer) and static terms
     const StreamDesc* s_t; const StreamDesc* s_p; const GenDesc* s_gd; const StreamDesc* s_po;
-    float* s_m;                                              // messages of this thread: s_m[k * TB]
-    unsigned lane, Z, xb;
+    float* s_m;                                              // messages of this thread: s_m[(k * FV + v) * TB]
+    unsigned lane, Z, xb[FV];
     int dv, ng;
     bool valid;
-    float sum; unsigned bad;
+    float sum[FV]; unsigned bad[FV];
 };
 
 #ifdef __CUDACC__
-// unsigned index arithmetic and one 32x32+64 multiply-add per address (runs start below 2^30 floats: code_create)
-__device__ __forceinline__ float load_stream(const float* p, const StreamDesc sd, unsigned lane, unsigned Z) {
+// byte offset of this thread's element of a stream: unsigned arithmetic, runs start below 2^30 floats (code_create)
+__device__ __forceinline__ unsigned stream_off(const StreamDesc sd, unsigned lane, unsigned Z) {
     unsigned idx = sd.x0 + lane;
     idx -= (idx >= Z) ? Z : 0u;
-    return __ldg(byte_ptr(p, 4u * (sd.base + idx)));
+    return 4u * (sd.base + idx);
 }
 
 // check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
@@ -51,113 +53,163 @@ __device__ __forceinline__ float cn_rule(float wv, float tv) {
     return with_sign(mag_of(qa + tt, fmaf(qa, tt, 1.0f)), sign_of(wv) ^ sign_of(tv));
 }
 
-// One chunk of kChunk edges starting at edge k0: loads back to back, then the check-node rule, messages to shared memory.
-// MODE 1: all edges are pair edges (k0 >= ng, k0 + kChunk <= dv); MODE 2: all are gen edges (k0 + kChunk <= ng); MODE 0:
+// One chunk of CH edges starting at edge k0: loads back to back, then the check-node rule, messages to shared memory.
+// MODE 1: all edges are pair edges (k0 >= ng, k0 + CH <= dv); MODE 2: all are gen edges (k0 + CH <= ng); MODE 0:
 // anything (per-edge predicates).
-template <int TB, bool FINAL, int MODE>
-__device__ __forceinline__ void chunk_cn(PassCtx<TB>& cx, const int k0) {
-    float tv[kChunk], wv[kChunk];
+template <int TB, int FV, int CH, bool FINAL, int MODE>
+__device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
+    float tv[CH][FV], wv[CH][FV];
     if (MODE == 1) {
 #pragma unroll
-        for (int j = 0; j < kChunk; ++j) {
-            tv[j] = load_stream(cx.tP, cx.s_t[k0 + j], cx.lane, cx.Z);
-            wv[j] = load_stream(cx.qP, cx.s_p[k0 + j], cx.lane, cx.Z);
+        for (int j = 0; j < CH; ++j) {
+            const unsigned ot = stream_off(cx.s_t[k0 + j], cx.lane, cx.Z);
+            const unsigned op = stream_off(cx.s_p[k0 + j], cx.lane, cx.Z);
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                tv[j][v] = __ldg(byte_ptr(cx.tP[v], ot));
+                wv[j][v] = __ldg(byte_ptr(cx.qP[v], op));
+            }
         }
 #pragma unroll
-        for (int j = 0; j < kChunk; ++j) {
-            const float mk = cn_rule(wv[j], tv[j]);
-            cx.s_m[(k0 + j) * TB] = mk;
-            cx.sum += mk;
+        for (int j = 0; j < CH; ++j) {
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                const float mk = cn_rule(wv[j][v], tv[j][v]);
+                cx.s_m[((k0 + j) * FV + v) * TB] = mk;
+                cx.sum[v] += mk;
+            }
         }
         return;
     }
-    float pw[kChunk][kGenSlots];
-    int np[kChunk], pbeg[kChunk], ctr[kChunk];
+    float pw[CH][kGenSlots][FV];
+    int np[CH], pbeg[CH], ctr[CH];
 #pragma unroll
-    for (int j = 0; j < kChunk; ++j) {                       // loads of the chunk, back to back
+    for (int j = 0; j < CH; ++j) {                           // loads of the chunk, back to back
         const int k = k0 + j;
-        tv[j] = 0.0f; wv[j] = 0.0f; np[j] = 0; pbeg[j] = 0; ctr[j] = 0;
+        np[j] = 0; pbeg[j] = 0; ctr[j] = 0;
 #pragma unroll
-        for (int jj = 0; jj < kGenSlots; ++jj) pw[j][jj] = 0.0f;
+        for (int v = 0; v < FV; ++v) {
+            tv[j][v] = 0.0f; wv[j][v] = 0.0f;
+#pragma unroll
+            for (int jj = 0; jj < kGenSlots; ++jj) pw[j][jj][v] = 0.0f;
+        }
         if (MODE == 2 || k < cx.dv) {
-            tv[j] = load_stream(cx.tP, cx.s_t[k], cx.lane, cx.Z);
+            const unsigned ot = stream_off(cx.s_t[k], cx.lane, cx.Z);
+#pragma unroll
+            for (int v = 0; v < FV; ++v) tv[j][v] = __ldg(byte_ptr(cx.tP[v], ot));
             if (MODE == 2 || k < cx.ng) {                    // gen edge: its first kGenSlots partners travel with the
                 const GenDesc gd = cx.s_gd[k];               // chunk's other loads (empty slot: +0.0, the identity)
                 np[j] = gd.np; pbeg[j] = gd.pbeg; ctr[j] = gd.counter;
 #pragma unroll
                 for (int jj = 0; jj < kGenSlots; ++jj)
-                    if (jj < gd.np) pw[j][jj] = load_stream(cx.qP, cx.s_po[gd.pbeg + jj], cx.lane, cx.Z);
+                    if (jj < gd.np) {
+                        const unsigned op = stream_off(cx.s_po[gd.pbeg + jj], cx.lane, cx.Z);
+#pragma unroll
+                        for (int v = 0; v < FV; ++v) pw[j][jj][v] = __ldg(byte_ptr(cx.qP[v], op));
+                    }
             } else {
-                wv[j] = load_stream(cx.qP, cx.s_p[k], cx.lane, cx.Z);
+                const unsigned op = stream_off(cx.s_p[k], cx.lane, cx.Z);
+#pragma unroll
+                for (int v = 0; v < FV; ++v) wv[j][v] = __ldg(byte_ptr(cx.qP[v], op));
             }
         }
     }
 #pragma unroll
-    for (int j = 0; j < kChunk; ++j) {
+    for (int j = 0; j < CH; ++j) {
         const int k = k0 + j;
         if (MODE == 2 || k < cx.ng) {
             // gen row: fold the other edges into one equivalent q (the rule is associative); bit 0 of a gen edge's
             // state is its variable's hard decision: the XOR of the raw words carries sign AND parity
-            float num = 0.0f, den = 1.0f;
-            unsigned xa = 0u;
+            float num[FV], den[FV];
+            unsigned xa[FV];
 #pragma unroll
-            for (int jj = 0; jj < kGenSlots; ++jj) {
-                const unsigned wb = __float_as_uint(pw[j][jj]);
-                xa ^= wb;
-                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+            for (int v = 0; v < FV; ++v) {
+                num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u;
+#pragma unroll
+                for (int jj = 0; jj < kGenSlots; ++jj) {
+                    const unsigned wb = __float_as_uint(pw[j][jj][v]);
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
             }
 #pragma unroll 1
             for (int jj = kGenSlots; jj < np[j]; ++jj) {     // rows of degree > kGenSlots + 1
-                const unsigned wb = __float_as_uint(load_stream(cx.qP, cx.s_po[pbeg[j] + jj], cx.lane, cx.Z));
-                xa ^= wb;
-                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+                const unsigned op = stream_off(cx.s_po[pbeg[j] + jj], cx.lane, cx.Z);
+#pragma unroll
+                for (int v = 0; v < FV; ++v) {
+                    const unsigned wb = __float_as_uint(__ldg(byte_ptr(cx.qP[v], op)));
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
             }
-            wv[j] = with_sign(num * rcp_approx(den), xa & 0x80000000u);
-            if (!FINAL && ctr[j])            // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
-                cx.bad |= (xa ^ cx.xb ^ (__float_as_uint(tv[j]) >> 31)) & (cx.valid ? 1u : 0u);
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                wv[j][v] = with_sign(num[v] * rcp_approx(den[v]), xa[v] & 0x80000000u);
+                if (!FINAL && ctr[j])        // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
+                    cx.bad[v] |= (xa[v] ^ cx.xb[v] ^ (__float_as_uint(tv[j][v]) >> 31)) & (cx.valid ? 1u : 0u);
+            }
         }
         if (MODE == 2 || k < cx.dv) {
-            const float mk = cn_rule(wv[j], tv[j]);
-            cx.s_m[k * TB] = mk;
-            cx.sum += mk;
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                const float mk = cn_rule(wv[j][v], tv[j][v]);
+                cx.s_m[(k * FV + v) * TB] = mk;
+                cx.sum[v] += mk;
+            }
         }
     }
 }
 #endif
 
-// dynamic shared memory: stream tables, then the messages m'_cv of the tile, [max_dv][TB] floats
+// dynamic shared memory: stream tables, then the messages m'_cv of the tile [max_dv][FV][TB], then partial sums [G][FV][TB]
 inline size_t pass_any_table_bytes(int max_np) {
     return (size_t)kMaxDv * (2 * sizeof(StreamDesc) + sizeof(GenDesc)) + (size_t)(max_np > 0 ? max_np : 1) * sizeof(StreamDesc);
 }
-inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups) {
-    return pass_any_table_bytes(max_np) + (size_t)((max_dv > 0 ? max_dv : 1) + groups) * tb * sizeof(float);
+inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups, int fv) {
+    return pass_any_table_bytes(max_np) + (size_t)((max_dv > 0 ? max_dv : 1) + groups) * fv * tb * sizeof(float);
 }
 
 // G = edge groups: the CTA is TB x G threads, thread (tid, grp) handles the chunks grp, grp + G, ... of the column's
 // edges, so a column of degree 60 is four chains of 15 edges instead of one of 60 (the pass of a single frame is bound
 // by that chain's latency); the partial sums of the groups meet in shared memory.
-template <int TB, int G, bool FINAL>
+template <int TB, int G, int FV, bool FINAL>
 __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTables tab, const PassArgs a) {
+    constexpr int CH = kChunk / FV;                           // edges per chunk: the loads in flight stay the same
     extern __shared__ __align__(16) unsigned char smem_any[];
     StreamDesc* const s_t = reinterpret_cast<StreamDesc*>(smem_any);          // [kMaxDv] t of edge k
     StreamDesc* const s_p = s_t + kMaxDv;                                     // [kMaxDv] partner of pair edge k
     GenDesc* const s_gd = reinterpret_cast<GenDesc*>(s_p + kMaxDv);           // [kMaxDv] gen edges
     StreamDesc* const s_po = reinterpret_cast<StreamDesc*>(s_gd + kMaxDv);    // [np] partners of the gen edges
-    float* const s_m = reinterpret_cast<float*>(smem_any + a.table_bytes) + threadIdx.x;   // m'_cv of edge k: s_m[k * TB]
-    float* const s_part = reinterpret_cast<float*>(smem_any + a.table_bytes) + a.max_dv * TB;   // [G][TB] partial sums
+    float* const s_m = reinterpret_cast<float*>(smem_any + a.table_bytes) + threadIdx.x;
+    float* const s_part = reinterpret_cast<float*>(smem_any + a.table_bytes) + a.max_dv * FV * TB;
 
     pdl_launch();
     pdl_wait();
-    const int f = blockIdx.y;
-    int in_buf;
-    if (FINAL) {
-        const int T = a.iters[f];
-        if (T <= 0) return;                                  // t = 0: k_init_cols wrote the outputs
-        in_buf = (T - 1) % 3;
-    } else {
-        if (a.done[f]) return;                               // frame already stopped: its state stays frozen
-        in_buf = a.in_buf;
+    // frames of this CTA; a frame that is out of range or stopped is not live: it is computed on the first live
+    // frame's data (valid memory) and nothing of it is stored
+    int fr[FV], in_buf[FV];
+    bool live[FV];
+    int f_any = -1;
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        fr[v] = blockIdx.y * FV + v;
+        live[v] = fr[v] < a.n_frames;
+        in_buf[v] = a.in_buf;
+        if (live[v]) {
+            if (FINAL) {
+                const int T = a.iters[fr[v]];
+                live[v] = T > 0;                             // t = 0: k_init_cols wrote the outputs
+                in_buf[v] = (T + 2) % 3;                     // (T - 1) mod 3
+            } else {
+                live[v] = !a.done[fr[v]];                    // frame already stopped: its state stays frozen
+            }
+        }
+        if (live[v] && f_any < 0) f_any = v;
     }
+    if (f_any < 0) return;
+#pragma unroll
+    for (int v = 0; v < FV; ++v)
+        if (!live[v]) { fr[v] = fr[f_any]; in_buf[v] = in_buf[f_any]; }
     const int ca = blockIdx.x / a.tiles;                     // block-uniform active column
     const int tile = blockIdx.x - ca * a.tiles;
     const ColDesc cd = tab.col[ca];
@@ -184,101 +236,133 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     }
     __syncthreads();
 
-    // opaque to the optimiser: otherwise the two frame pointers are re-formed (64-bit multiply, constant loads) at
-    // every one of the ~150 loads of a thread
-    unsigned long long qP_u = reinterpret_cast<unsigned long long>(a.qb[in_buf] + (int64_t)f * a.EZs);
-    unsigned long long tP_u = reinterpret_cast<unsigned long long>(a.t + (int64_t)f * a.mZs);
-    asm volatile("" : "+l"(qP_u), "+l"(tP_u));
-    PassCtx<TB> cx;
-    cx.qP = reinterpret_cast<const float*>(qP_u); cx.tP = reinterpret_cast<const float*>(tP_u);
+    PassCtx<TB, FV> cx;
+    float Q[FV];
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        // opaque to the optimiser: otherwise the frame pointers are re-formed (64-bit multiply, constant loads) at
+        // every one of the ~150 loads of a thread
+        unsigned long long qP_u = reinterpret_cast<unsigned long long>(a.qb[in_buf[v]] + (int64_t)fr[v] * a.EZs);
+        unsigned long long tP_u = reinterpret_cast<unsigned long long>(a.t + (int64_t)fr[v] * a.mZs);
+        asm volatile("" : "+l"(qP_u), "+l"(tP_u));
+        cx.qP[v] = reinterpret_cast<const float*>(qP_u);
+        cx.tP[v] = reinterpret_cast<const float*>(tP_u);
+        cx.xb[v] = (!FINAL && ng > 0) ? a.hard_in[(int64_t)fr[v] * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
+        cx.sum[v] = 0.0f; cx.bad[v] = 0u;
+        Q[v] = valid ? llr_to_log2(__ldg(a.llr + (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
+    }
     cx.s_t = s_t; cx.s_p = s_p; cx.s_gd = s_gd; cx.s_po = s_po; cx.s_m = s_m;
-    cx.lane = (unsigned)lane; cx.Z = (unsigned)Z; cx.dv = dv; cx.ng = ng;
-    cx.xb = (!FINAL && ng > 0) ? a.hard_in[(int64_t)f * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
-    cx.valid = valid; cx.sum = 0.0f; cx.bad = 0u;
-    const float Q = valid ? llr_to_log2(__ldg(a.llr + (int64_t)f * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
+    cx.lane = (unsigned)lane; cx.Z = (unsigned)Z; cx.dv = dv; cx.ng = ng; cx.valid = valid;
 
     // The chunk loop is NOT unrolled (a fully unrolled body for 64 edges is 170 KB of code: the pass becomes bound by
     // instruction fetch); the messages of the tile wait in shared memory for the variable-node rule instead.  A chunk
-    // whose 8 edges are all pair edges, or all gen edges, runs a body without per-edge predicates.
+    // whose edges are all pair edges, or all gen edges, runs a body without per-edge predicates.
+    // Edge k belongs to group (k / kChunk) mod G whatever FV is, and every group adds its messages in increasing k: a
+    // frame's result does not depend on the batch it is decoded in (bit for bit).
 #pragma unroll 1
-    for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
-        if (k0 >= ng && k0 + kChunk <= dv) chunk_cn<TB, FINAL, 1>(cx, k0);
-        else if (k0 + kChunk <= ng) chunk_cn<TB, FINAL, 2>(cx, k0);
-        else chunk_cn<TB, FINAL, 0>(cx, k0);
+    for (int kb = grp * kChunk; kb < dv; kb += G * kChunk) {
+#pragma unroll 1
+        for (int k0 = kb; k0 < min(kb + kChunk, dv); k0 += CH) {
+            if (k0 >= ng && k0 + CH <= dv) chunk_cn<TB, FV, CH, FINAL, 1>(cx, k0);
+            else if (k0 + CH <= ng) chunk_cn<TB, FV, CH, FINAL, 2>(cx, k0);
+            else chunk_cn<TB, FV, CH, FINAL, 0>(cx, k0);
+        }
     }
-    float sum = cx.sum;
 
     // variable-node rule
     if (G > 1) {                                             // the groups' partial sums meet here, in a fixed order
-        s_part[grp * TB + tid] = sum;
-        __syncthreads();
-        sum = 0.0f;
 #pragma unroll
-        for (int g = 0; g < G; ++g) sum += s_part[g * TB + tid];
-    }
-    const float L = Q + sum;                                 // L'_v
-    const unsigned xh = __float_as_uint(L) >> 31;            // 0 iff L_v >= 0
-    if (FINAL) {
-        if (valid && grp == 0) {
-            const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + i;
-            a.d_hard[vv] = (uint8_t)xh;
-            if (a.d_post) a.d_post[vv] = L * kLn2;
+        for (int v = 0; v < FV; ++v) s_part[(grp * FV + v) * TB + tid] = cx.sum[v];
+        __syncthreads();
+#pragma unroll
+        for (int v = 0; v < FV; ++v) {
+            cx.sum[v] = 0.0f;
+#pragma unroll
+            for (int g = 0; g < G; ++g) cx.sum[v] += s_part[(g * FV + v) * TB + tid];
         }
-        return;
     }
-    if (valid && grp == 0) a.hard_out[(int64_t)f * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh;
-    if (ng > 0 && __any_sync(0xffffffffu, cx.bad != 0) && (tid & 31) == 0) a.topbad[f] = 1;
+    float L[FV];
+    unsigned xh[FV];
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        L[v] = Q[v] + cx.sum[v];                             // L'_v
+        xh[v] = __float_as_uint(L[v]) >> 31;                 // 0 iff L_v >= 0
+        if (FINAL) {
+            if (live[v] && valid && grp == 0) {
+                const int64_t vv = (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i;
+                a.d_hard[vv] = (uint8_t)xh[v];
+                if (a.d_post) a.d_post[vv] = L[v] * kLn2;
+            }
+        } else if (live[v]) {
+            if (valid && grp == 0) a.hard_out[(int64_t)fr[v] * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh[v];
+            if (ng > 0 && __any_sync(__activemask(), cx.bad[v] != 0) && (tid & 31) == 0) a.topbad[fr[v]] = 1;
+        }
+    }
+    if (FINAL) return;
 
-    float* const sp = a.qb[a.out_buf] + (int64_t)f * a.EZs + (int64_t)cd.ebeg * Zs + (valid ? i : 0);
     const unsigned Zs4 = 4u * (unsigned)Zs;
     const bool single = dv == 1;                             // a single edge sends Q itself
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        if (!live[v] || !valid) continue;
+        float* const sp = a.qb[a.out_buf] + (int64_t)fr[v] * a.EZs + (int64_t)cd.ebeg * Zs + i;
 #pragma unroll 1
-    for (int k0 = grp * kChunk; k0 < dv; k0 += G * kChunk) {
-        if (k0 >= ng && k0 + kChunk <= dv) {                 // eight pair edges: no tags, no bounds
+        for (int kb = grp * kChunk; kb < dv; kb += G * kChunk)
+#pragma unroll 1
+        for (int k0 = kb; k0 < min(kb + kChunk, dv); k0 += CH) {
+            if (k0 >= ng && k0 + CH <= dv) {                 // pair edges only: no tags, no bounds
 #pragma unroll
-            for (int j = 0; j < kChunk; ++j) {
-                const float Lvc = single ? Q : L - s_m[(k0 + j) * TB];   // Q + sum_{k' != k} m_k'
-                if (valid) *byte_ptr(sp, (unsigned)(k0 + j) * Zs4) = w_of(Lvc);
-            }
-        } else {
+                for (int j = 0; j < CH; ++j) {
+                    const float Lvc = single ? Q[v] : L[v] - s_m[((k0 + j) * FV + v) * TB];   // Q + sum_{k' != k} m_k'
+                    *byte_ptr(sp, (unsigned)(k0 + j) * Zs4) = w_of(Lvc);
+                }
+            } else {
 #pragma unroll
-            for (int j = 0; j < kChunk; ++j) {
-                const int k = k0 + j;
-                if (k < dv) {
-                    const float Lvc = single ? Q : L - s_m[k * TB];
-                    unsigned wb = __float_as_uint(w_of(Lvc));
-                    if (k < ng) wb = (wb & 0xfffffffeu) | xh;    // gen edge: tag with the hard decision
-                    if (valid) *byte_ptr(sp, (unsigned)k * Zs4) = __uint_as_float(wb);
+                for (int j = 0; j < CH; ++j) {
+                    const int k = k0 + j;
+                    if (k < dv) {
+                        const float Lvc = single ? Q[v] : L[v] - s_m[(k * FV + v) * TB];
+                        unsigned wb = __float_as_uint(w_of(Lvc));
+                        if (k < ng) wb = (wb & 0xfffffffeu) | xh[v];    // gen edge: tag with the hard decision
+                        *byte_ptr(sp, (unsigned)k * Zs4) = __uint_as_float(wb);
+                    }
                 }
             }
         }
     }
 }
 
-template <int TB, int G>
+template <int TB, int G, int FV>
 inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     args.tiles = (args.Z + TB - 1) / TB;
     args.max_dv = L.max_dv > 0 ? L.max_dv : 1;
-    const size_t smem = pass_any_smem(L.max_np, L.max_dv, TB, G);
+    args.n_frames = L.n_frames;
+    const size_t smem = pass_any_smem(L.max_np, L.max_dv, TB, G, FV);
     static thread_local bool attr_set = false;
-    if (!attr_set) {            // tables (<= 18.4 KB) + messages (<= 32 KB) can exceed the 48 KB default
-        cudaFuncSetAttribute(k_pass<TB, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        cudaFuncSetAttribute(k_pass<TB, G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (!attr_set) {            // tables (<= 18.4 KB) + messages can exceed the 48 KB default
+        cudaFuncSetAttribute(k_pass<TB, G, FV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(k_pass<TB, G, FV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         attr_set = true;
     }
-    const dim3 grid(args.tiles * L.n_cols, L.n_frames), block(TB, G);
-    if (L.final_mode) k_pass<TB, G, true><<<grid, block, smem, L.stream>>>(L.tab, args);
-    else launch_pdl(k_pass<TB, G, false>, grid, block, smem, L.stream, L.tab, args);
+    const dim3 grid(args.tiles * L.n_cols, (L.n_frames + FV - 1) / FV), block(TB, G);
+    if (L.final_mode) k_pass<TB, G, FV, true><<<grid, block, smem, L.stream>>>(L.tab, args);
+    else launch_pdl(k_pass<TB, G, FV, false>, grid, block, smem, L.stream, L.tab, args);
+}
+
+template <int TB>
+inline void launch_pass_z(const PassLaunch& L, const PassArgs& args) {
+    const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
+    const bool pair = L.n_frames >= 4;                      // batched: two frames per thread
+    if (split) { if (pair) launch_pass_tb<TB, 4, 2>(L, args); else launch_pass_tb<TB, 4, 1>(L, args); }
+    else { if (pair) launch_pass_tb<TB, 1, 2>(L, args); else launch_pass_tb<TB, 1, 1>(L, args); }
 }
 
 inline void launch_pass_any(const PassLaunch& L) {
     PassArgs args = L.args;
     args.table_bytes = (int)pass_any_table_bytes(L.max_np);
-    const int Z = args.Z;
-    const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
-    if (Z <= 32) { if (split) launch_pass_tb<32, 4>(L, args); else launch_pass_tb<32, 1>(L, args); }
-    else if (Z <= 64) { if (split) launch_pass_tb<64, 4>(L, args); else launch_pass_tb<64, 1>(L, args); }
-    else { if (split) launch_pass_tb<128, 4>(L, args); else launch_pass_tb<128, 1>(L, args); }
+    if (args.Z <= 32) launch_pass_z<32>(L, args);
+    else if (args.Z <= 64) launch_pass_z<64>(L, args);
+    else launch_pass_z<128>(L, args);
 }
 
 }  // namespace qc

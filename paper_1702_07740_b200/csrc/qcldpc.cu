@@ -586,7 +586,7 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
     }
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
-                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, code->n, EZs, mZs, AZs},
+                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, code->n, EZs, mZs, AZs},
                   dim3(code->tiles * code->n_act_cols, n_frames), st, V, false,
                   code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames, code->max_np, code->max_dv};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,

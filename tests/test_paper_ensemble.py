@@ -143,3 +143,24 @@ def test_gpu_paper_ensemble_early_stop(oracle_lib):
     assert ok.any()
     np.testing.assert_array_equal(hard[ok], ref.hard[ok])
     np.testing.assert_array_equal(W.syndrome_of_sparse(rows, cols, shifts, mb, nb, 50, hard[ok]), fr.syndrome[ok])
+
+
+@pytest.mark.gpu
+def test_gpu_generic_kernel_frame_independence():
+    """Batched decodes carry two frames per thread in the generic kernel, single frames one: a frame's outputs must not
+    depend on the batch (bit for bit), also when its pair partner stops early or is missing (odd batch)."""
+    from paper_1702_07740_b200 import binding as B
+    spec = W.paper_ensemble_spec(400, 21)
+    rows, cols, shifts, mb, nb = W.make_paper_ensemble(spec)
+    code = B.QCLDPCCode.from_sparse(rows, cols, shifts, mb, nb, 21)
+    hi = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 3.0), 4, 555)
+    lo = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 0.3), 3, 556)
+    llr = np.concatenate([hi.llr[:2], lo.llr[:1], hi.llr[2:], lo.llr[1:]])          # 7 frames, converging and not
+    syn = np.concatenate([hi.syndrome[:2], lo.syndrome[:1], hi.syndrome[2:], lo.syndrome[1:]])
+    for early in (0, 1):
+        batch = _gpu_decode(code, llr, syn, 40, early)
+        assert early == 0 or (0 < batch[2].sum() < 7)                                # some stop early, some do not
+        for f in range(7):
+            alone = _gpu_decode(code, llr[f:f + 1], syn[f:f + 1], 40, early)
+            for a, b in zip(batch, alone):
+                np.testing.assert_array_equal(a[f], b[0])
