@@ -42,8 +42,8 @@ from paper_1702_07740_b200 import workloads as W  # noqa: E402
 FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 NOMINAL_HBM_GBS = 8000.0       # north_star's "about 8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per k_pass launch on config 4 (64 live frames) from the committed
-# `ncu --set full` capture (profiles/r01b_k_pass_full.md: 824.6 + 524.5 Mbyte); reported only for that workload.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1349.1e6
+# `ncu --set full` capture (profiles/r01f_k_pass_full.md: 826.6 + 524.0 Mbyte); reported only for that workload.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1350.6e6
 
 
 def decoded_mbit_per_s(block_length_bits: float, n_frames: float, seconds: float) -> float:
@@ -302,7 +302,7 @@ def main():
     launches_per_step = B.qcldpc_last_launch_count()
     # sample at least ~20 launches per step, spread evenly, also when the frames stop after a few iterations
     iters_warm = max(int(out.iters.max().item()), 1)
-    stride = max(1, min(args.profile_stride, iters_warm // 20))
+    stride = max(4, min(args.profile_stride, iters_warm // 20))
     w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     w0.record(stream); step(); w1.record(stream); barrier()
     if w0.elapsed_time(w1) / iters_warm < 0.05:             # launch-bound (one L2-resident frame): an event pair costs
