@@ -338,11 +338,13 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     args.max_dv = L.max_dv > 0 ? L.max_dv : 1;
     args.n_frames = L.n_frames;
     const size_t smem = pass_any_smem(L.max_np, L.max_dv, TB, G, FV);
-    static thread_local bool attr_set = false;
-    if (!attr_set) {            // tables (<= 18.4 KB) + messages can exceed the 48 KB default
+    static thread_local int attr_dev = -1;                  // the attribute is per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (attr_dev != dev) {      // tables (<= 18.4 KB) + messages can exceed the 48 KB default
         cudaFuncSetAttribute(k_pass<TB, G, FV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         cudaFuncSetAttribute(k_pass<TB, G, FV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        attr_set = true;
+        attr_dev = dev;
     }
     const dim3 grid(args.tiles * L.n_cols, (L.n_frames + FV - 1) / FV), block(TB, G);
     if (L.final_mode) k_pass<TB, G, FV, true><<<grid, block, smem, L.stream>>>(L.tab, args);
