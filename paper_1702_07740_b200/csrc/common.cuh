@@ -80,7 +80,7 @@ struct ExactTable { ExactCol<DV, NG, PCAP> c[kMaxExactCols]; };
 struct HostTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc* partner; const ColDesc* col; int n_cols; };
 
 struct PassLaunch {
-    PassTables tab; PassArgs args; dim3 grid; cudaStream_t stream; int V; bool final_mode;
+    PassTables tab; PassArgs args; cudaStream_t stream; int V; bool final_mode;
     const void* exact;         // HOST: the ExactTable of the instantiation (exact families only)
     int n_cols, n_frames, max_np, max_dv;
 };

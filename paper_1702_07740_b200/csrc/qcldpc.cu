@@ -14,13 +14,15 @@
 // Kernels:
 //   k_init_cols a0  w^(0) = w(Q_v) on every active edge (+ halo), decisions at t = 0 of the active variables
 //   k_init_rows a0  t_c from the absorbed variable's LLR and the syndrome bit (+ halo)
-//   k_pass      a1+a2  (pass_kernel.cuh) fused check-node + variable-node update of one iteration, VN-centric; also
-//               forms, from bit-0 tags, the parity of the rows WITHOUT absorbed variable at the previous iteration:
-//               a necessary condition for H xhat = s that costs no extra memory traffic
+//   k_pass_exact / k_pass  a1+a2  (pass_exact.cuh: the BASELINE.json column shapes, tables in kernel parameters;
+//               pass_kernel.cuh: any code, the paper's own ensemble included) fused check-node + variable-node update
+//               of one iteration, VN-centric; also forms, from bit-0 tags, the parity of the rows WITHOUT absorbed
+//               variable at the previous iteration: a necessary condition for H xhat = s that costs no extra traffic.
+//               Launched with programmatic dependent launch (common.cuh), like k_cand.
 //   k_cand      a3  early exit: for the frames that pass that filter, the full check (decisions of the absorbed
 //               variables L_j = Q_j + m_cj and every parity) on the still intact state of that iteration; persistent
 //               grid, returns at once when there is no candidate.  Freezes d_iters / d_pass / done per frame.
-//   k_pass<FINAL>, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
+//   the FINAL instantiations of the pass, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
 // Edge state is triple-buffered: pass t reads w^(t-1) and writes w^(t) over w^(t-2), so that when the check of
 // iteration t-1 runs (after pass t), w^(t-2) -- the input of iteration t-1 -- is still there.
 #include "common.cuh"
@@ -587,7 +589,7 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, code->n, EZs, mZs, AZs},
-                  dim3(code->tiles * code->n_act_cols, n_frames), st, V, false,
+                  st, V, false,
                   code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames, code->max_np, code->max_dv};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
                  d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
