@@ -106,7 +106,9 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
 /*
  * Same decode with HOST buffers (h_* are HOST pointers, same shapes; pinned memory makes the copies asynchronous):
  * copies inputs host->device, decodes, copies outputs device->host on `stream`, then WAITS for the stream so that the
- * h_* outputs are valid on return.  h_posterior may be NULL.  The device staging area is part of d_workspace, which
+ * h_* outputs are valid on return.  Because this call waits anyway, it reads the number of live frames back every 32
+ * iterations and stops launching once every frame has stopped (same results; qcldpc_decode, which never waits, issues
+ * all max_iter iterations and the leftover ones are empty grids).  h_posterior may be NULL.  The device staging area is part of d_workspace, which
  * must hold qcldpc_host_workspace_bytes(code, n_frames, h_posterior != NULL) bytes.
  */
 size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int want_posterior);

@@ -247,6 +247,18 @@ __global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const 
     if (threadIdx.x == 0) *a.ticket = 0;
 }
 
+// number of frames still iterating (decode_host polls it between chunks of iterations)
+__global__ void k_live_count(const int* done, int n_frames, int* n_live) {
+    int c = 0;
+    for (int f = threadIdx.x; f < n_frames; f += blockDim.x) c += done[f] ? 0 : 1;
+    __shared__ int s_c;
+    if (threadIdx.x == 0) s_c = 0;
+    __syncthreads();
+    if (c) atomicAdd(&s_c, c);
+    __syncthreads();
+    if (threadIdx.x == 0) *n_live = s_c;
+}
+
 __global__ void k_reset(int* done, int* unsat, int* topbad2, int* fullbad, unsigned* ticket, int32_t* iters,
                         uint8_t* pass, int n_frames, int max_iter) {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
@@ -546,9 +558,26 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
                             d_posterior, d_workspace, workspace_bytes, stream);
 }
 
+// host_poll: the caller waits for the stream anyway (qcldpc_decode_host), so every kPollEvery iterations the number of
+// live frames is read back and the launch sequence ends once every frame has stopped.  The device-pointer API never
+// waits: there the leftover launches of a fully stopped batch are empty grids.
+static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                       int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                       uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream,
+                       bool host_poll);
+
 int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                      int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
                      uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream) {
+    return decode_impl(code, d_llr, d_syndrome, n_frames, max_iter, early_stop, check_from_iter, d_hard, d_iters,
+                       d_pass, d_posterior, d_workspace, workspace_bytes, stream, false);
+}
+
+static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                       int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                       uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream,
+                       bool host_poll) {
+    constexpr int kPollEvery = 32;
     g_launches = 0;
     if (check_from_iter < 1) return QCLDPC_ERR_BAD_ARGUMENT;
     if (!code || !d_llr || !d_syndrome || !d_hard || !d_iters || !d_pass) return QCLDPC_ERR_BAD_ARGUMENT;
@@ -621,6 +650,15 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
             prof_end(pk, st);
             ++g_launches;
         }
+        if (host_poll && early_stop && t % kPollEvery == 0 && t < max_iter) {
+            int* const d_live = reinterpret_cast<int*>(w.ticket) + 16;
+            int live = 1;
+            k_live_count<<<1, 128, 0, st>>>(w.done, n_frames, d_live);
+            ++g_launches;
+            CUDA_TRY(cudaMemcpyAsync(&live, d_live, sizeof(int), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            if (live == 0) break;                        // every frame is frozen: the remaining launches would be empty
+        }
     }
     // outputs from each frame's frozen state: iteration d_iters[f] (= max_iter for the frames that did not stop)
     if (code->n_act_cols > 0 && max_iter > 0) {
@@ -671,8 +709,8 @@ int qcldpc_decode_host(const qcldpc_code_t* code, const float* h_llr, const uint
     if (h_posterior) { d_post = reinterpret_cast<float*>(p + off); off += align_up(llr_b, 256); }
     CUDA_TRY(cudaMemcpyAsync(d_llr, h_llr, llr_b, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_syn, h_syndrome, syn_b, cudaMemcpyHostToDevice, st));
-    const int rc = qcldpc_decode(code, d_llr, d_syn, n_frames, max_iter, early_stop, d_hard, d_iters, d_pass, d_post,
-                                 d_workspace, core, stream);
+    const int rc = decode_impl(code, d_llr, d_syn, n_frames, max_iter, early_stop, 1, d_hard, d_iters, d_pass, d_post,
+                               d_workspace, core, stream, true);
     if (rc != QCLDPC_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(h_hard, d_hard, hard_b, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(h_iters, d_iters, (size_t)n_frames * sizeof(int32_t), cudaMemcpyDeviceToHost, st));

@@ -308,6 +308,19 @@ def test_decode_host_matches_device_path(B):
     out2 = code.decode_host(fr.llr, fr.syndrome, 30, 1, want_posterior=False)
     np.testing.assert_array_equal(out2.hard, h)
     assert B.qcldpc_last_launch_count() > 0
+    # a batch whose frames all stop early: the host path ends the launch sequence once nothing is live (it waits for
+    # the stream anyway), the device path enqueues all max_iter iterations; same outputs, far fewer launches
+    conv = np.nonzero(p)[0][:6]
+    h2, i2, p2, post2 = gpu_decode(B, base, Z, fr.llr[conv], fr.syndrome[conv], 400, 1)
+    n_dev = B.qcldpc_last_launch_count()
+    out3 = code.decode_host(fr.llr[conv], fr.syndrome[conv], 400, 1, want_posterior=True)
+    n_host = B.qcldpc_last_launch_count()
+    assert p2.all() and i2.max() < 64
+    np.testing.assert_array_equal(out3.hard, h2)
+    np.testing.assert_array_equal(out3.iters, i2)
+    np.testing.assert_array_equal(out3.passed, p2)
+    np.testing.assert_array_equal(out3.posterior, post2)
+    assert n_host < n_dev // 3
 
 
 def test_gpu_argument_errors(B):
