@@ -48,7 +48,7 @@ struct CheckTables { const RowDesc* row; const RowEdge* redge; };
 // ---- kernel arguments -------------------------------------------------------------------------------------------
 struct PassArgs {
     const float* llr;          // [F][n]
-    float* qb[3];              // the three edge-state buffers [F][E][Zs]
+    float* qb[4];              // the four edge-state buffers [F][E][Zs] (iteration t lives in buffer t mod 4: check.cuh)
     const float* t;            // [F][mb][Zs]
     const uint8_t* hard_in;    // xhat of the input iteration, active columns only [F][A][Zs]
     uint8_t* hard_out;

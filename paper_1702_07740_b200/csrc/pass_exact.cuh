@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(kThreads) k_pass_exact(const __grid_constant__
     if (FINAL) {
         const int Tit = a.iters[f];
         if (Tit <= 0) return;                                // t = 0: k_init_cols wrote the outputs
-        in_buf = (Tit - 1) % 3;
+        in_buf = (Tit + 3) % 4;                              // w^(T-1)
     } else {
         if (a.done[f]) return;                               // frame already stopped: its state stays frozen
         in_buf = a.in_buf;

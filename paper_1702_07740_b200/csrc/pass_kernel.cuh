@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
             if (FINAL) {
                 const int T = a.iters[fr[v]];
                 live[v] = T > 0;                             // t = 0: k_init_cols wrote the outputs
-                in_buf[v] = (T + 2) % 3;                     // (T - 1) mod 3
+                in_buf[v] = (T + 3) % 4;                     // w^(T-1): buffer (T - 1) mod 4
             } else {
                 live[v] = !a.done[fr[v]];                    // frame already stopped: its state stays frozen
             }

@@ -25,6 +25,7 @@
 //   the FINAL instantiations of the pass, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
 // Edge state is triple-buffered: pass t reads w^(t-1) and writes w^(t) over w^(t-2), so that when the check of
 // iteration t-1 runs (after pass t), w^(t-2) -- the input of iteration t-1 -- is still there.
+#include "check.cuh"
 #include "common.cuh"
 
 #include <algorithm>
@@ -131,57 +132,6 @@ __global__ void __launch_bounds__(kThreads) k_init_rows(const CheckTables tab, c
     if (a.halo && r < kHalo) tf[a.Z + r] = ts;
 }
 
-struct CheckArgs {
-    const float* llr; const uint8_t* syn;
-    const float* qb[3];
-    const uint8_t* hardbuf[2];   // candidate mode: xhat of iteration t in hardbuf[t & 1], active columns [F][A][Zs]
-    uint8_t* d_hard; float* d_post;
-    int* done; int32_t* iters; uint8_t* pass;
-    const int* topbad;           // slot of the iteration being checked
-    int* topbad_clear;           // the other slot
-    int* fullbad; int* unsat; unsigned* ticket;
-    int n_frames, mb, Z, Zs, tiles, t, check_from; int64_t n, m, EZs, AZs;
-};
-
-// a3: parity of check (R, r) of frame f for the decisions of iteration T: decides the absorbed degree-1 variable from
-// the messages of iteration T-1 (L_j = Q_j + m_cj), XORs the hard decisions against s_c.
-// FINAL: decisions of the active variables come from d_hard, the absorbed variable's outputs are written.
-template <bool FINAL>
-__device__ __forceinline__ unsigned check_one(const CheckTables& tab, const CheckArgs& a, int f, int R, int r, int T) {
-    const RowDesc rd = tab.row[R];
-    const int Z = a.Z;
-    const float* __restrict__ qprev = a.qb[(T + 2) % 3] + (int64_t)f * a.EZs;     // w^(T-1)
-    unsigned par = a.syn[(int64_t)f * a.m + (int64_t)R * Z + r] & 1u;
-    unsigned sg = par << 31;
-    float num = 0.0f, den = 1.0f;
-    for (int k = 0; k < rd.ne; ++k) {
-        const RowEdge re = tab.redge[rd.ebeg + k];
-        int iv = r + re.shift; iv -= (iv >= Z) ? Z : 0;
-        if (FINAL) par ^= a.d_hard[(int64_t)f * a.n + (int64_t)re.col * Z + iv] & 1u;
-        else par ^= a.hardbuf[T & 1][(int64_t)f * a.AZs + (int64_t)re.ca * a.Zs + iv] & 1u;
-        if (rd.abs_col >= 0 && T > 0) {
-            unsigned wb = __float_as_uint(__ldg(qprev + (int64_t)re.edge * a.Zs + iv));
-            sg ^= wb & 0x80000000u;
-            wb &= rd.gen ? 0x7ffffffeu : 0x7fffffffu;         // gen edges carry a tag in bit 0
-            boxplus_acc(__uint_as_float(wb), num, den);
-        }
-    }
-    if (rd.abs_col >= 0) {
-        int j = r + rd.abs_shift; j -= (j >= Z) ? Z : 0;
-        const int64_t v = (int64_t)f * a.n + (int64_t)rd.abs_col * Z + j;
-        const float Qj = __ldg(a.llr + v);
-        float Lj = llr_to_log2(Qj);
-        if (T > 0) Lj += with_sign(mag_of(num, den), sg);   // L'_j = Q'_j + m'_cj
-        const unsigned xj = __float_as_uint(Lj) >> 31;
-        if (FINAL) {
-            a.d_hard[v] = (uint8_t)xj;
-            if (a.d_post) a.d_post[v] = T > 0 ? Lj * kLn2 : Qj;
-        }
-        par ^= xj;
-    }
-    return par;
-}
-
 // a4: one thread per check of every frame, on the frame's frozen state (iteration d_iters[f]); counts failed parities
 __global__ void __launch_bounds__(kThreads) k_check_final(const CheckTables tab, const CheckArgs a) {
     const int f = blockIdx.y;
@@ -200,51 +150,12 @@ __global__ void k_flags_final(int* unsat, uint8_t* pass, int n_frames) {
     unsat[f] = 0;
 }
 
-// a3: early exit for iteration t (runs after pass t+1).  Persistent grid.  A frame is a candidate if it is still live
-// and no row without absorbed variable failed its parity (topbad, formed by pass t+1 from the bit-0 tags).  Every
-// block walks the candidates in the same order; the last block to finish freezes the frames whose full check passed.
+// a3, stand-alone launch of the early-exit work (check.cuh): the generic kernel family, and the last checked iteration
+// of every decode
 __global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const CheckArgs a) {
-    __shared__ unsigned s_last;
     pdl_launch();
     pdl_wait();
-    const int units = a.mb * a.tiles;
-    if (blockIdx.x == 0)
-        for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.topbad_clear[f] = 0;
-    if (a.t < a.check_from) return;                                      // launched only to clear the filter slot
-    bool any = false;
-    for (int f0 = 0; f0 < a.n_frames; f0 += kThreads) {
-        const int f = f0 + threadIdx.x;
-        const int c = (f < a.n_frames && !a.done[f] && !a.topbad[f]) ? 1 : 0;
-        if (!__syncthreads_or(c)) continue;
-        any = true;
-        const int fend = min(f0 + kThreads, a.n_frames);
-        for (int g = f0; g < fend; ++g) {
-            if (a.done[g] || a.topbad[g]) continue;                      // block-uniform
-            for (int u = blockIdx.x; u < units; u += gridDim.x) {
-                // some block already found a failed parity of this frame: skip the rest of it
-                if (__syncthreads_or(threadIdx.x == 0 ? *((volatile int*)(a.fullbad + g)) : 0)) break;
-                const int R = u / a.tiles;
-                const int r = (u - R * a.tiles) * kThreads + threadIdx.x;
-                unsigned bad = 0;
-                if (r < a.Z) bad = check_one<false>(tab, a, g, R, r, a.t);
-                if (__syncthreads_or(bad != 0) && threadIdx.x == 0) a.fullbad[g] = 1;
-            }
-        }
-    }
-    if (!any) return;                                                    // the same decision in every block
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    for (int f = threadIdx.x; f < a.n_frames; f += kThreads) {
-        if (!a.done[f] && !a.topbad[f]) {
-            if (*((volatile int*)(a.fullbad + f)) == 0) { a.done[f] = 1; a.iters[f] = a.t; a.pass[f] = 1; }
-            a.fullbad[f] = 0;
-        }
-    }
-    if (threadIdx.x == 0) *a.ticket = 0;
+    cand_work(tab, a, blockIdx.x, gridDim.x);
 }
 
 // number of frames still iterating (decode_host polls it between chunks of iterations)
@@ -259,12 +170,13 @@ __global__ void k_live_count(const int* done, int n_frames, int* n_live) {
     if (threadIdx.x == 0) *n_live = s_c;
 }
 
-__global__ void k_reset(int* done, int* unsat, int* topbad2, int* fullbad, unsigned* ticket, int32_t* iters,
+__global__ void k_reset(int* done2, int* unsat, int* topbad3, int* fullbad, unsigned* ticket, int32_t* iters,
                         uint8_t* pass, int n_frames, int max_iter) {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f == 0) *ticket = 0;
     if (f >= n_frames) return;
-    done[f] = 0; unsat[f] = 0; topbad2[f] = 0; topbad2[n_frames + f] = 0; fullbad[f] = 0;
+    done2[f] = 0; done2[n_frames + f] = 0; unsat[f] = 0; fullbad[f] = 0;
+    topbad3[f] = 0; topbad3[n_frames + f] = 0; topbad3[2 * n_frames + f] = 0;
     iters[f] = max_iter; pass[f] = 0;
 }
 
@@ -304,7 +216,7 @@ int cuda_fail(cudaError_t e, const char* what) {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Workspace {
-    float* qbuf[3]; float* t; uint8_t* hardbuf[2]; int* done; int* unsat; int* topbad; int* fullbad; unsigned* ticket;
+    float* qbuf[4]; float* t; uint8_t* hardbuf[3]; int* done; int* unsat; int* topbad; int* fullbad; unsigned* ticket;
     size_t bytes;
 };
 
@@ -316,12 +228,12 @@ Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
     const size_t tbytes = align_up((size_t)n_frames * code->mb * code->Zs * sizeof(float), 256);
     const size_t hbytes = align_up((size_t)n_frames * code->n_act_cols * code->Zs, 256);
     const size_t fbytes = align_up((size_t)n_frames * sizeof(int), 256);
-    for (int b = 0; b < 3; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
+    for (int b = 0; b < 4; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
     w.t = reinterpret_cast<float*>(p + off); off += tbytes;
-    for (int b = 0; b < 2; ++b) { w.hardbuf[b] = reinterpret_cast<uint8_t*>(p + off); off += hbytes; }
-    w.done = reinterpret_cast<int*>(p + off); off += fbytes;
+    for (int b = 0; b < 3; ++b) { w.hardbuf[b] = reinterpret_cast<uint8_t*>(p + off); off += hbytes; }
+    w.done = reinterpret_cast<int*>(p + off); off += 2 * fbytes;       // two versions of n_frames ints, contiguous
     w.unsat = reinterpret_cast<int*>(p + off); off += fbytes;
-    w.topbad = reinterpret_cast<int*>(p + off); off += 2 * fbytes;     // two slots of n_frames ints, contiguous
+    w.topbad = reinterpret_cast<int*>(p + off); off += 3 * fbytes;     // three slots of n_frames ints, contiguous
     w.fullbad = reinterpret_cast<int*>(p + off); off += fbytes;
     w.ticket = reinterpret_cast<unsigned*>(p + off); off += 256;
     w.bytes = off;
@@ -616,12 +528,13 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         if (v && (atoi(v) == 1 || atoi(v) == 2)) V = atoi(v);
     }
     PassLaunch pl{ptab,
-                  PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, w.t, nullptr, nullptr, d_hard, d_posterior,
+                  PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, code->n, EZs, mZs, AZs},
                   st, V, false,
                   code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames, code->max_np, code->max_dv};
-    CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2]}, {w.hardbuf[0], w.hardbuf[1]}, d_hard,
-                 d_posterior, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
+    CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
+                 {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
+                 d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
                  n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
     // early-exit grid: persistent; small batches are launch-bound and almost never have a candidate, so a smaller grid
     // (less to schedule and retire between two passes) wins there
@@ -629,37 +542,50 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     const int cand_per_sm = cb ? std::max(1, atoi(cb)) : (n_frames <= 8 ? 1 : 4);
     const int cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * tiles1));
 
+    // Launch t = pass t, then the early-exit check of iteration t-2 (check.cuh explains the lag): the check reads the
+    // stopped-frame flags of version t & 1 (the ones pass t reads) and writes version (t + 1) & 1 for pass t+1.
+    auto done_ver = [&](int t) { return w.done + (size_t)(t & 1) * n_frames; };
+    auto topbad_slot = [&](int T) { return w.topbad + (size_t)(((T % 3) + 3) % 3) * n_frames; };
+    auto launch_check = [&](int T, int t) {              // check of iteration T, issued with launch t
+        ca.t = T;
+        ca.topbad = topbad_slot(T);
+        ca.topbad_clear = topbad_slot(t);                // the slot pass t+1 writes (filter of iteration t)
+        ca.done_r = done_ver(t);
+        ca.done_w = done_ver(t + 1);
+        const int pk = prof_begin(1, st);
+        launch_pdl(k_cand, dim3(cand_blocks), dim3(kThreads), 0, st, ctab, ca);
+        prof_end(pk, st);
+        ++g_launches;
+    };
+    // the check is launched for iterations T >= check_from_iter - 2: the filter slot of iteration I is dirty from pass
+    // I-2 and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
+    auto check_wanted = [&](int T) { return early_stop && T >= 1 && T >= check_from_iter - 2; };
+    int t_last = 0;                                      // last launch issued
     for (int t = 1; t <= max_iter; ++t) {
         if (code->n_act_cols > 0) {
-            pl.args.in_buf = (t - 1) % 3; pl.args.out_buf = t % 3;
-            pl.args.hard_in = w.hardbuf[(t - 1) & 1]; pl.args.hard_out = w.hardbuf[t & 1];
-            pl.args.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
+            pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
+            pl.args.hard_in = w.hardbuf[(t - 1) % 3]; pl.args.hard_out = w.hardbuf[t % 3];
+            pl.args.topbad = topbad_slot(t - 1);
+            pl.args.done = done_ver(t);
             const int pk = prof_begin(0, st);
             code->launcher(pl);
             prof_end(pk, st);
             ++g_launches;
         }
-        if (early_stop && t >= 2 && t - 1 >= check_from_iter - 1) {
-            // early exit for iteration t-1: its filter bits were formed by pass t, its input state w^(t-2) is intact
-            // (the launch for iteration check_from_iter - 1 only clears the filter slot of the first checked one)
-            ca.t = t - 1;
-            ca.topbad = w.topbad + (size_t)((t - 1) & 1) * n_frames;
-            ca.topbad_clear = w.topbad + (size_t)(t & 1) * n_frames;
-            const int pk = prof_begin(1, st);
-            launch_pdl(k_cand, dim3(cand_blocks), dim3(kThreads), 0, st, ctab, ca);
-            prof_end(pk, st);
-            ++g_launches;
-        }
+        if (check_wanted(t - 2)) launch_check(t - 2, t);
+        t_last = t;
         if (host_poll && early_stop && t % kPollEvery == 0 && t < max_iter) {
             int* const d_live = reinterpret_cast<int*>(w.ticket) + 16;
             int live = 1;
-            k_live_count<<<1, 128, 0, st>>>(w.done, n_frames, d_live);
+            k_live_count<<<1, 128, 0, st>>>(check_wanted(t - 2) ? done_ver(t + 1) : done_ver(t), n_frames, d_live);
             ++g_launches;
             CUDA_TRY(cudaMemcpyAsync(&live, d_live, sizeof(int), cudaMemcpyDeviceToHost, st));
             CUDA_TRY(cudaStreamSynchronize(st));
             if (live == 0) break;                        // every frame is frozen: the remaining launches would be empty
         }
     }
+    // the check of the last but one executed iteration (the last one is settled by k_check_final below)
+    if (t_last >= 2 && check_wanted(t_last - 1)) launch_check(t_last - 1, t_last + 1);
     // outputs from each frame's frozen state: iteration d_iters[f] (= max_iter for the frames that did not stop)
     if (code->n_act_cols > 0 && max_iter > 0) {
         pl.final_mode = true;
