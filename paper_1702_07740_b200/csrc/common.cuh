@@ -61,6 +61,7 @@ struct PassArgs {
     int Z, Zs, tiles;
     int table_bytes, max_dv;   // generic kernel: bytes of its shared-memory tables; messages [max_dv][FV][TB] follow
     int n_frames;              // generic kernel: frames of the batch (two per thread when batched)
+    int cand_y;                // exact kernels: blockIdx.y of the CTAs that run the early-exit check (check.cuh), or -1
     int64_t n, EZs, mZs, AZs;  // per-frame strides
 };
 
@@ -82,6 +83,8 @@ struct HostTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc*
 struct PassLaunch {
     PassTables tab; PassArgs args; cudaStream_t stream; int V; bool final_mode;
     const void* exact;         // HOST: the ExactTable of the instantiation (exact families only)
+    const void* check_tab;     // HOST: CheckTables / CheckArgs of the early-exit check this launch carries in its grid
+    const void* check_args;    //       (exact families; NULL: none)
     int n_cols, n_frames, max_np, max_dv;
 };
 using PassLauncher = void (*)(const PassLaunch&);

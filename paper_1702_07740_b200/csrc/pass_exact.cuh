@@ -6,16 +6,23 @@
 // state load is issued a few hundred cycles after the CTA starts instead of after three dependent L2 round trips.
 #pragma once
 
+#include "check.cuh"
 #include "common.cuh"
 
 namespace qc {
 
 template <int DV, int NG, int PCAP, int V, bool FINAL>
-__global__ void __launch_bounds__(kThreads) k_pass_exact(const __grid_constant__ ExactTable<DV, NG, PCAP> T,
+__global__ void __launch_bounds__(kThreads, V == 1 ? 7 : 4) k_pass_exact(const __grid_constant__ ExactTable<DV, NG, PCAP> T,
                                                          const __grid_constant__ PassArgs a,
-                                                         const PartnerDesc* __restrict__ partner) {
+                                                         const PartnerDesc* __restrict__ partner,
+                                                         const CheckTables ctab, const __grid_constant__ CheckArgs chk) {
     constexpr int NGS = NG > 0 ? NG : 1;
     pdl_launch();
+    if (!FINAL && (int)blockIdx.y == a.cand_y) {             // the extra grid row: early-exit check of iteration t-2
+        pdl_wait();
+        cand_work(ctab, chk, blockIdx.z * gridDim.x + blockIdx.x, gridDim.x * gridDim.z);
+        return;
+    }
     const int f = blockIdx.z;
     const int ca = blockIdx.y;                               // block-uniform active column
     const ExactCol<DV, NG, PCAP>& cd = T.c[ca];

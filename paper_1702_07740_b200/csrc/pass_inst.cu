@@ -42,13 +42,20 @@ size_t PASS_CAT(PASS_NAME, _table)(const HostTables& h, void* out) {
 
 template <int V, bool FINAL>
 static void launch_exact(const PassLaunch& L) {
-    const dim3 grid((L.args.Z + kThreads * V - 1) / (kThreads * V), L.n_cols, L.n_frames);
+    const bool with_check = !FINAL && L.check_args != nullptr;
+    const dim3 grid((L.args.Z + kThreads * V - 1) / (kThreads * V), L.n_cols + (with_check ? 1 : 0), L.n_frames);
+    PassArgs args = L.args;
+    args.cand_y = with_check ? L.n_cols : -1;
+    static const CheckTables no_tab{nullptr, nullptr};
+    static const CheckArgs no_args{};
+    const CheckTables& ctab = with_check ? *static_cast<const CheckTables*>(L.check_tab) : no_tab;
+    const CheckArgs& ca = with_check ? *static_cast<const CheckArgs*>(L.check_args) : no_args;
     if (FINAL)
         k_pass_exact<PASS_DV, PASS_NG, PASS_PCAP, V, FINAL><<<grid, kThreads, 0, L.stream>>>(
-            *static_cast<const Table*>(L.exact), L.args, L.tab.partner);
+            *static_cast<const Table*>(L.exact), args, L.tab.partner, ctab, ca);
     else
         launch_pdl(k_pass_exact<PASS_DV, PASS_NG, PASS_PCAP, V, FINAL>, grid, dim3(kThreads), 0, L.stream,
-                   *static_cast<const Table*>(L.exact), L.args, L.tab.partner);
+                   *static_cast<const Table*>(L.exact), args, L.tab.partner, ctab, ca);
 }
 
 void PASS_NAME(const PassLaunch& L) {

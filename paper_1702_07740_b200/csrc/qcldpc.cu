@@ -529,9 +529,10 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     }
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
-                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, code->n, EZs, mZs, AZs},
+                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
                   st, V, false,
-                  code->exact.empty() ? nullptr : code->exact.data(), code->n_act_cols, n_frames, code->max_np, code->max_dv};
+                  code->exact.empty() ? nullptr : code->exact.data(), nullptr, nullptr, code->n_act_cols, n_frames,
+                  code->max_np, code->max_dv};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
                  {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
                  d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
@@ -560,19 +561,33 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     // the check is launched for iterations T >= check_from_iter - 2: the filter slot of iteration I is dirty from pass
     // I-2 and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
     auto check_wanted = [&](int T) { return early_stop && T >= 1 && T >= check_from_iter - 2; };
+    const char* mc = getenv("QCLDPC_MERGE_CHECK");        // tuning knob: 0 = always a separate k_cand launch
+    const bool merge_check = !code->exact.empty() && !(mc && atoi(mc) == 0);
+    pl.check_tab = nullptr; pl.check_args = nullptr;
     int t_last = 0;                                      // last launch issued
     for (int t = 1; t <= max_iter; ++t) {
+        // exact families carry the check of iteration t-2 in the grid of pass t (one launch per iteration)
+        const bool merged = merge_check && check_wanted(t - 2) && code->n_act_cols > 0;
         if (code->n_act_cols > 0) {
             pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
             pl.args.hard_in = w.hardbuf[(t - 1) % 3]; pl.args.hard_out = w.hardbuf[t % 3];
             pl.args.topbad = topbad_slot(t - 1);
             pl.args.done = done_ver(t);
+            pl.check_tab = nullptr; pl.check_args = nullptr;
+            if (merged) {
+                ca.t = t - 2;
+                ca.topbad = topbad_slot(t - 2);
+                ca.topbad_clear = topbad_slot(t);
+                ca.done_r = done_ver(t);
+                ca.done_w = done_ver(t + 1);
+                pl.check_tab = &ctab; pl.check_args = &ca;
+            }
             const int pk = prof_begin(0, st);
             code->launcher(pl);
             prof_end(pk, st);
             ++g_launches;
         }
-        if (check_wanted(t - 2)) launch_check(t - 2, t);
+        if (check_wanted(t - 2) && !merged) launch_check(t - 2, t);
         t_last = t;
         if (host_poll && early_stop && t % kPollEvery == 0 && t < max_iter) {
             int* const d_live = reinterpret_cast<int*>(w.ticket) + 16;
