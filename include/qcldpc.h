@@ -63,7 +63,7 @@ void qcldpc_code_destroy(qcldpc_code_t* code);
 int qcldpc_code_create_sparse(const int32_t* rows, const int32_t* cols, const int32_t* shifts, int64_t n_entries,
                               int mb, int nb, int Z, qcldpc_code_t** out_code);
 
-/* Code facts: n, m, number of active base edges (state = 2 * 4 * Z * that many bytes per frame). */
+/* Code facts: n, m, number of active base edges (one fp32 of state per active edge and buffer; four buffers). */
 int qcldpc_code_info(const qcldpc_code_t* code, int64_t* n, int64_t* m, int64_t* active_base_edges);
 
 /* Bytes of DEVICE workspace qcldpc_decode needs for n_frames frames (0 on bad arguments). */

@@ -19,12 +19,13 @@
 //               of one iteration, VN-centric; also forms, from bit-0 tags, the parity of the rows WITHOUT absorbed
 //               variable at the previous iteration: a necessary condition for H xhat = s that costs no extra traffic.
 //               Launched with programmatic dependent launch (common.cuh), like k_cand.
-//   k_cand      a3  early exit: for the frames that pass that filter, the full check (decisions of the absorbed
-//               variables L_j = Q_j + m_cj and every parity) on the still intact state of that iteration; persistent
-//               grid, returns at once when there is no candidate.  Freezes d_iters / d_pass / done per frame.
+//   cand_work   a3  (check.cuh) early exit: for the frames that pass that filter, the full check (decisions of the
+//               absorbed variables L_j = Q_j + m_cj and every parity) on the still intact state of that iteration;
+//               returns at once when there is no candidate; freezes d_iters / d_pass / done per frame.  Runs in an
+//               extra grid row of k_pass_exact, or as the stand-alone k_cand (generic family, last iteration).
 //   the FINAL instantiations of the pass, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
-// Edge state is triple-buffered: pass t reads w^(t-1) and writes w^(t) over w^(t-2), so that when the check of
-// iteration t-1 runs (after pass t), w^(t-2) -- the input of iteration t-1 -- is still there.
+// Edge state lives in four buffers (iteration t in buffer t mod 4); the early-exit check of iteration t-2 runs next to
+// pass t and touches nothing that pass writes: check.cuh has the timeline.
 #include "check.cuh"
 #include "common.cuh"
 
