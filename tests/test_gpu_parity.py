@@ -381,3 +381,23 @@ def test_gpu_no_writes_outside_the_buffers(B, which):
         for raw, body in ((ws_raw, need_al), (hard_raw, F * n), (it_raw, F * 4), (ps_raw, (F + 255) // 256 * 256),
                           (po_raw, F * n * 4)):
             assert bool((raw[:G] == 0xAB).all()) and bool((raw[G + body:] == 0xAB).all())
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("max_iter", [1, 2, 3, 4, 5, 12, 13, 14])
+def test_early_stop_with_small_iteration_budgets(oracle_lib, B, max_iter):
+    """The early-exit check of iteration T rides two launches behind pass T: budgets around that lag, and frames that
+    pass exactly at max_iter - 2, max_iter - 1 and max_iter, must give the oracle's flags, counts and outputs."""
+    cfg, base, Z, fr = W.make_config(1)
+    llr = np.concatenate([fr.llr, 25.0 * np.sign(fr.llr[:2])])             # two noiseless frames: pass at iteration 1
+    # noiseless copies of frames 0, 1 with the signs of the TRUE words
+    llr[-2:] = 25.0 * (1.0 - 2.0 * fr.x[:2].astype(np.float32))
+    syn = np.concatenate([fr.syndrome, fr.syndrome[:2]])
+    ref = oracle_lib.decode(base, Z, llr, syn, max_iter, 1)
+    hard, iters, passed, post = gpu_decode(B, base, Z, llr, syn, max_iter, 1)
+    np.testing.assert_array_equal(passed, ref.passed)
+    np.testing.assert_array_equal(iters, ref.iters)
+    assert iters[-1] == 1 and iters[-2] == 1 and passed[-2:].all()
+    ok = ref.passed.astype(bool)
+    np.testing.assert_array_equal(hard[ok], ref.hard[ok])
+    assert rel_err(post, ref.posterior).max() <= TOL
