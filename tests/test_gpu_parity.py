@@ -401,3 +401,27 @@ def test_early_stop_with_small_iteration_budgets(oracle_lib, B, max_iter):
     ok = ref.passed.astype(bool)
     np.testing.assert_array_equal(hard[ok], ref.hard[ok])
     assert rel_err(post, ref.posterior).max() <= TOL
+
+
+@pytest.mark.gpu
+def test_gpu_two_streams_share_one_handle(B):
+    """include/qcldpc.h: the handle is immutable and may be used concurrently from several streams with distinct
+    workspaces.  Two decodes of different frames enqueued on two streams must equal the same decodes run alone."""
+    cfg, base, Z, fr = W.make_config(3, n_frames=2, Z=1000)
+    code = B.QCLDPCCode(base, Z)
+    d_llr = torch.from_numpy(fr.llr).cuda()
+    d_syn = torch.from_numpy(fr.syndrome).cuda()
+    alone = [code.decode(d_llr[k:k + 1], d_syn[k:k + 1], 60, 1, want_posterior=True) for k in range(2)]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = []
+    for rep in range(3):
+        outs = []
+        for k, st in enumerate(streams):
+            st.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(st):
+                outs.append(code.decode(d_llr[k:k + 1], d_syn[k:k + 1], 60, 1, want_posterior=True, stream=st))
+        torch.cuda.synchronize()
+        for k in range(2):
+            assert torch.equal(outs[k].hard, alone[k].hard) and torch.equal(outs[k].iters, alone[k].iters)
+            assert torch.equal(outs[k].posterior, alone[k].posterior) and torch.equal(outs[k].passed, alone[k].passed)
