@@ -215,9 +215,11 @@ def main():
     ap.add_argument("--snr-point", type=int, default=0, help="index into the config's SNR points (config 5 has 6)")
     ap.add_argument("--check-from", type=int, default=1,
                     help="early-termination scheduling (P:514): run the syndrome test from this iteration on")
-    ap.add_argument("--ensemble", type=int, default=0, choices=[0, 21, 50],
+    ap.add_argument("--ensemble", type=int, default=0, choices=[0, 21, 50, 512],
                     help="NEXT-1: decode the paper's own rate-0.02 multi-edge ensemble lifted by q = 21 (n = 1.008e6) "
-                         "or q = 50 (n = 1e6) at its beta = 0.99 operating point instead of a BASELINE.json config")
+                         "or q = 50 (n = 1e6) at its beta = 0.99 operating point instead of a BASELINE.json config; "
+                         "512 = NEXT-2: a labelled STAND-IN for the paper's rate-1/10, n = 2^20, q = 512 code at SNR "
+                         "0.161, max 100 iterations (Table IV; its degree distribution is not printed)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
@@ -235,22 +237,31 @@ def main():
         # P:231) = 0.02840 for R = 0.02, sigma = s^-1/2; max 500 iterations with early termination
         from types import SimpleNamespace
         q = args.ensemble
-        spec = W.paper_ensemble_spec(20000 if q == 50 else 48000, q)
-        ens = W.make_paper_ensemble(spec)
-        n_fr, mx = args.frames or 8, args.max_iter or 500
-        cfg = SimpleNamespace(
-            index=100 + q, n_frames=n_fr, max_iter=mx, early_stop=1, gaps_db=(0.0,),
-            code=SimpleNamespace(n=spec.n, m=spec.m, Z=q, e_core=(spec.base_edges - spec.n_d1) * q),
-            ensemble_name=(f"NEXT-1: the paper's rate-0.02 multi-edge ensemble (P:288-300), {spec.nb} base columns "
-                           f"(core degree 59/60) x {spec.mb} rows lifted by q={q}, n={spec.n}, {n_fr} frames, BIAWGN at "
-                           f"beta=0.99 (SNR 0.0284), max {mx} iterations, early stop on"))
+        if q == 512:
+            # NEXT-2: a STAND-IN for the paper's rate-1/10, n = 2^20, q = 512 code (Table IV) at SNR 0.161, 100 iterations
+            ens = W.make_rate10_standin(2048, 512)
+            n_fr, mx = args.frames or 1, args.max_iter or 100
+            code_ns = SimpleNamespace(n=2048 * q, m=ens[3] * q, Z=q, e_core=int((ens[1] < (2048 + 2) // 5).sum()) * q)
+            name = (f"NEXT-2 STAND-IN (not the paper's code: its degree distribution is not printed): rate-0.1 base "
+                    f"graph 2048 columns x {ens[3]} rows lifted by q=512, n=2^20, {n_fr} frames, BIAWGN SNR 0.161 "
+                    f"(P:620), max {mx} iterations, early stop on")
+        else:
+            spec = W.paper_ensemble_spec(20000 if q == 50 else 48000, q)
+            ens = W.make_paper_ensemble(spec)
+            n_fr, mx = args.frames or 8, args.max_iter or 500
+            code_ns = SimpleNamespace(n=spec.n, m=spec.m, Z=q, e_core=(spec.base_edges - spec.n_d1) * q)
+            name = (f"NEXT-1: the paper's rate-0.02 multi-edge ensemble (P:288-300), {spec.nb} base columns (core "
+                    f"degree 59/60) x {spec.mb} rows lifted by q={q}, n={spec.n}, {n_fr} frames, BIAWGN at beta=0.99 "
+                    f"(SNR 0.0284), max {mx} iterations, early stop on")
+        cfg = SimpleNamespace(index=100 + q, n_frames=n_fr, max_iter=mx, early_stop=1, gaps_db=(0.0,), code=code_ns,
+                              ensemble_name=name)
     base = W.make_base_matrix(cfg.code) if ens is None else None
     Z = cfg.code.Z
     if args.snr_point:
         cfg = W.Config(cfg.index, cfg.code, cfg.n_frames, cfg.max_iter, cfg.early_stop,
                        cfg.gaps_db[args.snr_point:args.snr_point + 1], cfg.description)
     sigma = (W.sigma_for_gap(cfg.code.rate, cfg.gaps_db[0]) if ens is None
-             else (2.0 ** (2.0 * 0.02 / 0.99) - 1.0) ** -0.5)
+             else 0.161 ** -0.5 if args.ensemble == 512 else (2.0 ** (2.0 * 0.02 / 0.99) - 1.0) ** -0.5)
     seed_base = rank_seed_base(cfg.index, rank, args.snr_point)
 
     if args.impl == "reference":

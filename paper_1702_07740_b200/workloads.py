@@ -325,3 +325,33 @@ def make_frames_sparse(rows, cols, shifts, mb: int, nb: int, Z: int, sigma: floa
         y = (1.0 - 2.0 * x[k].astype(np.float64)) + sigma * rng.standard_normal(n)
         llr[k] = (2.0 * y / (sigma * sigma)).astype(np.float32)
     return Frames(x=x, syndrome=syndrome_of_sparse(rows, cols, shifts, mb, nb, Z, x), llr=llr, sigma=sigma)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-2: the paper's second operating point -- rate 1/10, n = 2^20, q = 512, SNR 0.161, 100 iterations
+# (Table IV).  The paper does NOT print that code's degree distribution (refs [25], [39]); this is a labelled
+# STAND-IN with the shape of BASELINE.json's rate-0.1 configs at the paper's base-graph size: nb/5 core columns with 3
+# edges into nb/10 top checks and 7 or 8 edges into the lower checks (each lower check: 2 core edges + 1 degree-1
+# column on the unshifted diagonal).  It measures the decoder on that SIZE and lifting factor, nothing else.
+def make_rate10_standin(nb: int = 2048, q: int = 512, seed: int = 17020777000):
+    """Non-zero blocks (rows, cols, shifts, mb, nb) of the stand-in; structure from seed, shifts from (seed, q)."""
+    rng = np.random.default_rng(seed)
+    nc = (nb + 2) // 5
+    n_top = nb // 10
+    n_low = nb - nc
+    mb = n_top + n_low
+    while True:                                            # 3 distinct top checks per core column, every top check >= 2
+        top = np.stack([rng.choice(n_top, size=3, replace=False) for _ in range(nc)])
+        if np.bincount(top.ravel(), minlength=n_top).min() >= 2:
+            break
+    r1, c1 = top.ravel(), np.repeat(np.arange(nc), 3)
+    sockets = np.repeat(np.arange(n_low), 2)               # every lower check receives exactly 2 core edges
+    share = np.full(nc, len(sockets) // nc)
+    share[: len(sockets) - share.sum()] += 1               # 8, 8, ..., 7: dealt in column order
+    vn2 = np.repeat(np.arange(nc), share)
+    r2, c2 = _match_sockets(rng, vn2, n_top + sockets)
+    rows = np.concatenate([r1, r2, n_top + np.arange(n_low)]).astype(np.int32)
+    cols = np.concatenate([c1, c2, nc + np.arange(n_low)]).astype(np.int32)
+    srng = np.random.default_rng([seed, q])
+    shifts = np.concatenate([srng.integers(0, q, size=len(r1) + len(r2)), np.zeros(n_low, dtype=np.int64)])
+    return rows, cols, shifts.astype(np.int32), mb, nb

@@ -164,3 +164,35 @@ def test_gpu_generic_kernel_frame_independence():
             alone = _gpu_decode(code, llr[f:f + 1], syn[f:f + 1], 40, early)
             for a, b in zip(batch, alone):
                 np.testing.assert_array_equal(a[f], b[0])
+
+
+def test_rate10_standin_structure():
+    """NEXT-2 stand-in (the paper does not print that code's degree distribution): size and shape only."""
+    rows, cols, shifts, mb, nb = W.make_rate10_standin()
+    assert nb * 512 == 2 ** 20 and abs((1.0 - mb / nb) - 0.1) < 1e-3                  # n = 2^20, rate 1/10 (P:592-600)
+    nc, n_top = (nb + 2) // 5, nb // 10
+    cdeg, rdeg = np.bincount(cols, minlength=nb), np.bincount(rows, minlength=mb)
+    assert set(cdeg[:nc]) <= {10, 11} and (cdeg[nc:] == 1).all()
+    assert rdeg[:n_top].min() >= 2 and (rdeg[n_top:] == 3).all()
+    key = rows.astype(np.int64) * nb + cols
+    assert len(np.unique(key)) == len(key)
+    d1 = cols >= nc
+    assert (rows[d1] - n_top == cols[d1] - nc).all() and (shifts[d1] == 0).all()
+
+
+@pytest.mark.gpu
+def test_gpu_rate10_standin_reduced(oracle_lib):
+    from paper_1702_07740_b200 import binding as B
+    rows, cols, shifts, mb, nb = W.make_rate10_standin(200, 64)
+    fr = W.make_frames_sparse(rows, cols, shifts, mb, nb, 64, 0.161 ** -0.5, 5, 2020)
+    for early, n_iter in ((0, 20), (1, 100)):
+        ref = oracle_lib.decode_sparse(rows, cols, shifts, mb, nb, 64, fr.llr, fr.syndrome, n_iter, early)
+        hard, iters, passed, post = _gpu_decode(B.QCLDPCCode.from_sparse(rows, cols, shifts, mb, nb, 64), fr.llr,
+                                                fr.syndrome, n_iter, early)
+        np.testing.assert_array_equal(passed, ref.passed)
+        np.testing.assert_array_equal(iters, ref.iters)
+        if early == 0:
+            err = np.abs(post - ref.posterior) / np.maximum(1.0, np.abs(ref.posterior))
+            assert err.max() <= TOL, err.max()
+            decided = np.abs(ref.posterior) > 1e-2
+            np.testing.assert_array_equal(hard[decided], ref.hard[decided])
