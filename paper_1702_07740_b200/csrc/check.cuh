@@ -67,48 +67,50 @@ __device__ __forceinline__ unsigned check_one(const CheckTables& tab, const Chec
     return par;
 }
 
-// Early exit for iteration a.t by worker `worker` of `n_workers` CTAs (all of them call this, with kThreads threads).  A
+// Early exit for iteration a.t by worker `worker` of `n_workers` CTAs (all threads of each of them call this).  A
 // frame is a candidate if it is still live and no row without absorbed variable failed its parity (topbad).  Every
 // worker walks the candidates in the same order; the last worker to finish freezes the frames whose full check passed
 // and publishes the flags of the next pass.
-__device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArgs& a, const int worker, const int n_workers) {
+// tid / nthr: the calling thread's index in its CTA and the CTA's size (any shape); a.tiles = ceil(Z / nthr).
+__device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArgs& a, const int worker, const int n_workers,
+                                          const int tid, const int nthr) {
     __shared__ unsigned s_last;
     const int units = a.mb * a.tiles;
     if (worker == 0)
-        for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.topbad_clear[f] = 0;
+        for (int f = tid; f < a.n_frames; f += nthr) a.topbad_clear[f] = 0;
     if (a.t < a.check_from) return;                                      // launched only to clear the filter slot
     bool any = false;
-    for (int f0 = 0; f0 < a.n_frames; f0 += kThreads) {
-        const int f = f0 + threadIdx.x;
+    for (int f0 = 0; f0 < a.n_frames; f0 += nthr) {
+        const int f = f0 + tid;
         const int c = (f < a.n_frames && !a.done_r[f] && !a.topbad[f]) ? 1 : 0;
         if (!__syncthreads_or(c)) continue;
         any = true;
-        const int fend = min(f0 + kThreads, a.n_frames);
+        const int fend = min(f0 + nthr, a.n_frames);
         for (int g = f0; g < fend; ++g) {
             if (a.done_r[g] || a.topbad[g]) continue;                    // block-uniform
             for (int u = worker; u < units; u += n_workers) {
                 // some worker already found a failed parity of this frame: skip the rest of it
-                if (__syncthreads_or(threadIdx.x == 0 ? *((volatile int*)(a.fullbad + g)) : 0)) break;
+                if (__syncthreads_or(tid == 0 ? *((volatile int*)(a.fullbad + g)) : 0)) break;
                 const int R = u / a.tiles;
-                const int r = (u - R * a.tiles) * kThreads + threadIdx.x;
+                const int r = (u - R * a.tiles) * nthr + tid;
                 unsigned bad = 0;
                 if (r < a.Z) bad = check_one<false>(tab, a, g, R, r, a.t);
-                if (__syncthreads_or(bad != 0) && threadIdx.x == 0) a.fullbad[g] = 1;
+                if (__syncthreads_or(bad != 0) && tid == 0) a.fullbad[g] = 1;
             }
         }
     }
     if (!any) {                                                          // the same decision in every worker
         if (worker == 0)
-            for (int f = threadIdx.x; f < a.n_frames; f += kThreads) a.done_w[f] = a.done_r[f];
+            for (int f = tid; f < a.n_frames; f += nthr) a.done_w[f] = a.done_r[f];
         return;
     }
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == (unsigned)n_workers - 1u) ? 1u : 0u;
+    if (tid == 0) s_last = (atomicAdd(a.ticket, 1u) == (unsigned)n_workers - 1u) ? 1u : 0u;
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    for (int f = threadIdx.x; f < a.n_frames; f += kThreads) {
+    for (int f = tid; f < a.n_frames; f += nthr) {
         int d = a.done_r[f];
         if (!d && !a.topbad[f]) {
             if (*((volatile int*)(a.fullbad + f)) == 0) { d = 1; a.iters[f] = a.t; a.pass[f] = 1; }
@@ -116,7 +118,7 @@ __device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArg
         }
         a.done_w[f] = d;
     }
-    if (threadIdx.x == 0) *a.ticket = 0;
+    if (tid == 0) *a.ticket = 0;
 }
 #endif
 

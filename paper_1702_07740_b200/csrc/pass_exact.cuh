@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(kThreads, V == 1 ? 7 : 4) k_pass_exact(const _
     pdl_launch();
     if (!FINAL && (int)blockIdx.y == a.cand_y) {             // the extra grid row: early-exit check of iteration t-2
         pdl_wait();
-        cand_work(ctab, chk, blockIdx.z * gridDim.x + blockIdx.x, gridDim.x * gridDim.z);
+        cand_work(ctab, chk, blockIdx.z * gridDim.x + blockIdx.x, gridDim.x * gridDim.z, threadIdx.x, kThreads);
         return;
     }
     const int f = blockIdx.z;

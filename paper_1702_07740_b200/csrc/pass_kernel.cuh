@@ -19,7 +19,10 @@
 // FINAL = true: same arithmetic on each frame's frozen state, writes the outputs (hard bits, posterior) instead.
 #pragma once
 
+#include "check.cuh"
 #include "common.cuh"
+
+#include <algorithm>
 
 namespace qc {
 
@@ -173,8 +176,16 @@ inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups, int fv) 
 // edges, so a column of degree 60 is four chains of 15 edges instead of one of 60 (the pass of a single frame is bound
 // by that chain's latency); the partial sums of the groups meet in shared memory.
 template <int TB, int G, int FV, bool FINAL>
-__global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTables tab, const PassArgs a) {
+__global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTables tab, const PassArgs a,
+                                                                  const CheckTables ctab, const CheckArgs chk) {
     constexpr int CH = kChunk / FV;                           // edges per chunk: the loads in flight stay the same
+    if (!FINAL && a.cand_y >= 0 && (int)blockIdx.x >= a.cand_y) {   // extra CTAs: early-exit check of iteration t-2
+        pdl_launch();
+        pdl_wait();
+        cand_work(ctab, chk, blockIdx.y * (gridDim.x - a.cand_y) + (blockIdx.x - a.cand_y),
+                  (gridDim.x - a.cand_y) * gridDim.y, threadIdx.y * TB + threadIdx.x, TB * G);
+        return;
+    }
     extern __shared__ __align__(16) unsigned char smem_any[];
     StreamDesc* const s_t = reinterpret_cast<StreamDesc*>(smem_any);          // [kMaxDv] t of edge k
     StreamDesc* const s_p = s_t + kMaxDv;                                     // [kMaxDv] partner of pair edge k
@@ -346,9 +357,19 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
         cudaFuncSetAttribute(k_pass<TB, G, FV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         attr_dev = dev;
     }
-    const dim3 grid(args.tiles * L.n_cols, (L.n_frames + FV - 1) / FV), block(TB, G);
-    if (L.final_mode) k_pass<TB, G, FV, true><<<grid, block, smem, L.stream>>>(L.tab, args);
-    else launch_pdl(k_pass<TB, G, FV, false>, grid, block, smem, L.stream, L.tab, args);
+    // the early-exit check of iteration t-2 rides in extra CTAs of the same grid (check.cuh): about four per SM
+    const bool with_check = !L.final_mode && L.check_args != nullptr;
+    const int rows_y = (L.n_frames + FV - 1) / FV;
+    const int extra = with_check ? std::max(1, std::min(args.tiles * L.n_cols, (4 * 148 + rows_y - 1) / rows_y)) : 0;
+    static const CheckTables no_tab{nullptr, nullptr};
+    static const CheckArgs no_args{};
+    CheckArgs chk = with_check ? *static_cast<const CheckArgs*>(L.check_args) : no_args;
+    chk.tiles = (args.Z + TB * G - 1) / (TB * G);           // its units are CTA-sized here
+    args.cand_y = with_check ? args.tiles * L.n_cols : -1;
+    const dim3 grid(args.tiles * L.n_cols + extra, rows_y), block(TB, G);
+    const CheckTables& ctab = with_check ? *static_cast<const CheckTables*>(L.check_tab) : no_tab;
+    if (L.final_mode) k_pass<TB, G, FV, true><<<grid, block, smem, L.stream>>>(L.tab, args, ctab, chk);
+    else launch_pdl(k_pass<TB, G, FV, false>, grid, block, smem, L.stream, L.tab, args, ctab, chk);
 }
 
 template <int TB>

@@ -156,7 +156,7 @@ __global__ void k_flags_final(int* unsat, uint8_t* pass, int n_frames) {
 __global__ void __launch_bounds__(kThreads) k_cand(const CheckTables tab, const CheckArgs a) {
     pdl_launch();
     pdl_wait();
-    cand_work(tab, a, blockIdx.x, gridDim.x);
+    cand_work(tab, a, blockIdx.x, gridDim.x, threadIdx.x, kThreads);
 }
 
 // number of frames still iterating (decode_host polls it between chunks of iterations)
@@ -563,11 +563,11 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     // I-2 and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
     auto check_wanted = [&](int T) { return early_stop && T >= 1 && T >= check_from_iter - 2; };
     const char* mc = getenv("QCLDPC_MERGE_CHECK");        // tuning knob: 0 = always a separate k_cand launch
-    const bool merge_check = !code->exact.empty() && !(mc && atoi(mc) == 0);
+    const bool merge_check = !(mc && atoi(mc) == 0);
     pl.check_tab = nullptr; pl.check_args = nullptr;
     int t_last = 0;                                      // last launch issued
     for (int t = 1; t <= max_iter; ++t) {
-        // exact families carry the check of iteration t-2 in the grid of pass t (one launch per iteration)
+        // the check of iteration t-2 rides in the grid of pass t (one launch per iteration)
         const bool merged = merge_check && check_wanted(t - 2) && code->n_act_cols > 0;
         if (code->n_act_cols > 0) {
             pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
