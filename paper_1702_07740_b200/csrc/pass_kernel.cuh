@@ -62,7 +62,7 @@ __device__ __forceinline__ float cn_rule(float wv, float tv) {
 template <int TB, int FV, int CH, bool FINAL, int MODE>
 __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
     float tv[CH][FV], wv[CH][FV];
-    if (MODE == 1) {
+    if constexpr (MODE == 1) {
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
             const unsigned ot = stream_off(cx.s_t[k0 + j], cx.lane, cx.Z);
@@ -82,8 +82,7 @@ __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
                 cx.sum[v] += mk;
             }
         }
-        return;
-    }
+    } else {
     float pw[CH][kGenSlots][FV];
     int np[CH], pbeg[CH], ctr[CH];
 #pragma unroll
@@ -161,6 +160,7 @@ __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
             }
         }
     }
+    }   // MODE != 1
 }
 #endif
 
