@@ -425,3 +425,37 @@ def test_gpu_two_streams_share_one_handle(B):
         for k in range(2):
             assert torch.equal(outs[k].hard, alone[k].hard) and torch.equal(outs[k].iters, alone[k].iters)
             assert torch.equal(outs[k].posterior, alone[k].posterior) and torch.equal(outs[k].passed, alone[k].passed)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_random_codes_against_oracle(oracle_lib, B, seed):
+    """Random base matrices (any row and column degree up to the supported 64, degree-0 and degree-1 rows and columns,
+    several degree-1 columns in a row), random lifting sizes around the tile sizes of both kernel families, 1-9
+    frames (one and two frames per thread), fixed iterations and early stop."""
+    rng = np.random.default_rng(9000 + seed)
+    Z = int(rng.choice([1, 2, 3, 7, 21, 31, 32, 33, 50, 63, 64, 65, 127, 128, 129, 200, 257]))
+    mb = int(rng.integers(2, 13))
+    nb = int(rng.integers(mb, mb + 15))
+    base = _random_code(rng, mb, nb, Z, float(rng.choice([0.15, 0.3, 0.5, 0.8])))
+    if seed % 4 == 0:                                      # a degree-1 diagonal on the right, like the paper's codes
+        k = min(mb, nb // 2)
+        base[:, nb - k:] = -1
+        base[np.arange(k), nb - k + np.arange(k)] = 0
+    n_frames = int(rng.integers(1, 10))
+    n, m = nb * Z, mb * Z
+    x = rng.integers(0, 2, size=(n_frames, n), dtype=np.uint8)
+    syn = W.syndrome_of(base, Z, x)
+    sigma = float(rng.choice([0.5, 0.8, 1.2]))
+    llr = (2.0 * ((1.0 - 2.0 * x) + sigma * rng.standard_normal((n_frames, n))) / sigma ** 2).astype(np.float32)
+    n_iter = int(rng.integers(1, 26))
+    assert_parity(oracle_lib, B, base, Z, llr, syn, n_iter, f"random seed {seed}")
+    ref = oracle_lib.decode(base, Z, llr, syn, 40, 1)
+    hard, iters, passed, post = gpu_decode(B, base, Z, llr, syn, 40, 1)
+    ref32 = oracle_lib.decode(base, Z, llr, syn, 40, 1, precision=32)
+    stable = (ref32.iters == ref.iters) & (ref32.passed == ref.passed)   # frames whose stop does not hinge on rounding
+    np.testing.assert_array_equal(passed[stable], ref.passed[stable])
+    np.testing.assert_array_equal(iters[stable], ref.iters[stable])
+    ok = stable & ref.passed.astype(bool)
+    np.testing.assert_array_equal(hard[ok], ref.hard[ok])
+    np.testing.assert_array_equal(W.syndrome_of(base, Z, hard[passed.astype(bool)]), syn[passed.astype(bool)])
