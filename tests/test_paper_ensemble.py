@@ -196,3 +196,22 @@ def test_gpu_rate10_standin_reduced(oracle_lib):
             assert err.max() <= TOL, err.max()
             decided = np.abs(ref.posterior) > 1e-2
             np.testing.assert_array_equal(hard[decided], ref.hard[decided])
+
+
+@pytest.mark.gpu
+def test_gpu_paper_ensemble_full_size(oracle_lib):
+    """The paper's q = 50 code at full size (n = 1e6, 66,750 base blocks, 3.34 M edges), one frame at the paper's
+    operating point (beta = 0.99, SNR 0.0284): posterior and hard bits after 12 iterations against the oracle."""
+    from paper_1702_07740_b200 import binding as B
+    spec = W.paper_ensemble_spec(20000, 50)
+    rows, cols, shifts, mb, nb = W.make_paper_ensemble(spec)
+    sigma = (2.0 ** (2.0 * 0.02 / 0.99) - 1.0) ** -0.5
+    fr = W.make_frames_sparse(rows, cols, shifts, mb, nb, 50, sigma, 1, 31415)
+    ref = oracle_lib.decode_sparse(rows, cols, shifts, mb, nb, 50, fr.llr, fr.syndrome, 12, 0)
+    hard, iters, passed, post = _gpu_decode(B.QCLDPCCode.from_sparse(rows, cols, shifts, mb, nb, 50), fr.llr,
+                                            fr.syndrome, 12, 0)
+    err = np.abs(post - ref.posterior) / np.maximum(1.0, np.abs(ref.posterior))
+    assert err.max() <= TOL, err.max()
+    decided = np.abs(ref.posterior) > 1e-2
+    np.testing.assert_array_equal(hard[decided], ref.hard[decided])
+    np.testing.assert_array_equal(passed, ref.passed)
