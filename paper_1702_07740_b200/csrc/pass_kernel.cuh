@@ -45,9 +45,8 @@ struct PassCtx {
 #ifdef __CUDACC__
 // byte offset of this thread's element of a stream: unsigned arithmetic, runs start below 2^30 floats (code_create)
 __device__ __forceinline__ unsigned stream_off(const StreamDesc sd, unsigned lane, unsigned Z) {
-    unsigned idx = sd.x0 + lane;
-    idx -= (idx >= Z) ? Z : 0u;
-    return 4u * (sd.base + idx);
+    const unsigned idx = sd.x0 + lane;                       // < 2 Z
+    return 4u * (sd.base + min(idx, idx - Z));               // idx - Z wraps to a huge value when idx < Z
 }
 
 // check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
