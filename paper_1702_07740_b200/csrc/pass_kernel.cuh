@@ -235,14 +235,16 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     // preamble: window starts of this tile, once per stream
     for (int k = flat; k < dv; k += TB * G) {
         const EdgeDesc d = tab.edge[cd.ebeg + k];
-        int r0 = (i0 - d.shift) % Z; r0 += (r0 < 0) ? Z : 0;  // check index of the tile's first variable
+        int r0 = i0 - d.shift; r0 += (r0 < 0) ? Z : 0;        // check index of the tile's first variable (i0, shift < Z)
+        int x0 = i0 + d.delta; x0 -= (x0 >= Z) ? Z : 0;       // delta < Z: one wrap at most, no division
         s_t[k] = StreamDesc{(unsigned)d.t_off, (unsigned)r0};
-        s_p[k] = StreamDesc{(unsigned)(d.p_off >= 0 ? d.p_off : 0), (unsigned)(d.p_off >= 0 ? (i0 + d.delta) % Z : 0)};
+        s_p[k] = StreamDesc{(unsigned)(d.p_off >= 0 ? d.p_off : 0), (unsigned)(d.p_off >= 0 ? x0 : 0)};
     }
     for (int g = flat; g < ng; g += TB * G) s_gd[g] = tab.gen[cd.gbeg + g];
     for (int j = flat; j < cd.np; j += TB * G) {
         const PartnerDesc p = tab.partner[cd.pbeg + j];
-        s_po[j] = StreamDesc{(unsigned)p.off, (unsigned)((i0 + p.delta) % Z)};
+        int x0 = i0 + p.delta; x0 -= (x0 >= Z) ? Z : 0;
+        s_po[j] = StreamDesc{(unsigned)p.off, (unsigned)x0};
     }
     __syncthreads();
 
