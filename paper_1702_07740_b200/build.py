@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"),
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"), os.path.join(CSRC, "check.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
 # (symbol, DV, NG, PCAP): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
 # 11 or 21 edges, 3 of them into the top rows); pass_generic.cu takes any column of degree <= 64

@@ -33,13 +33,19 @@ constexpr float kMsgMax2 = QCLDPC_MSG_MAX * kLog2e;   // the clamp S2 in log2 un
 // ---- code tables (built once by qcldpc_code_create, read from global memory in each block's preamble) -----------
 // A base row is a PAIR row if it has an absorbed variable and exactly two active edges (every lower row of the
 // BASELINE.json codes); every other row is a GEN row.  Inside an active column the gen edges come first.
-struct EdgeDesc { int shift; int t_off; int p_off; int delta; };  // t at t[t_off + (i - shift) mod Z]; pair edge:
-                                                                  // partner at w[p_off + (i + delta) mod Z], else p_off = -1
+// A TRIPLE row is a gen row with an absorbed variable and exactly three active edges (the lower rows of the paper's
+// ensemble): its edges have two partners and no parity to report; the generic pass gives them a predicate-free body.
+struct EdgeDesc {                       // t at t[t_off + (i - shift) mod Z]
+    int shift; int t_off;
+    int p_off; int delta;               // pair or triple edge: partner at w[p_off + (i + delta) mod Z], else p_off = -1
+    int p2_off; int delta2;             // triple edge: second partner, else p2_off = -1
+};
 struct GenDesc { int pbeg; int np; int counter; int pad; };       // partners [pbeg, pbeg+np) relative to the column's
                                                                   // first partner; counter: this edge reports the row's parity
 struct PartnerDesc { int off; int delta; };                       // w[off + (i + delta) mod Z]
-struct ColDesc { int col; int ebeg; int dv; int ng; int gbeg; int pbeg; int np; int pad; };
-struct RowDesc { int ebeg; int ne; int abs_col; int abs_shift; int gen; int pad0, pad1, pad2; };
+struct ColDesc { int col; int ebeg; int dv; int ng; int gbeg; int pbeg; int np; int ngh; };
+// edges of a column: [0, ngh) gen edges of other gen rows, [ngh, ng) gen edges of triple rows, [ng, dv) pair edges
+struct RowDesc { int ebeg; int ne; int abs_col; int abs_shift; int gen; int pad0, pad1, pad2; };   // gen: 0 pair, 1 gen, 2 triple
 struct RowEdge { int edge; int shift; int col; int ca; };         // active edge seen from its row (ca = active column)
 
 struct PassTables { const EdgeDesc* edge; const GenDesc* gen; const PartnerDesc* partner; const ColDesc* col; };

@@ -28,13 +28,14 @@ namespace qc {
 
 constexpr int kChunk = 8;
 constexpr int kGenSlots = 2;                                 // partners of a gen edge loaded with its chunk
+constexpr int kGenMore = 4;                                  // further partners of a gen edge per round trip
 
 struct StreamDesc { unsigned base, x0; };                     // element (x0 + lane) mod Z of the run at float index base
 
 template <int TB, int FV>
 struct PassCtx {
     const float* qP[FV]; const float* tP[FV];                // per frame: edge state (input buffer) and static terms
-    const StreamDesc* s_t; const StreamDesc* s_p; const GenDesc* s_gd; const StreamDesc* s_po;
+    const StreamDesc* s_t; const StreamDesc* s_p; const StreamDesc* s_p2; const GenDesc* s_gd; const StreamDesc* s_po;
     float* s_m;                                              // messages of this thread: s_m[(k * FV + v) * TB]
     unsigned lane, Z, xb[FV];
     int dv, ng;
@@ -56,8 +57,8 @@ __device__ __forceinline__ float cn_rule(float wv, float tv) {
 }
 
 // One chunk of CH edges starting at edge k0: loads back to back, then the check-node rule, messages to shared memory.
-// MODE 1: all edges are pair edges (k0 >= ng, k0 + CH <= dv); MODE 2: all are gen edges (k0 + CH <= ng); MODE 0:
-// anything (per-edge predicates).
+// MODE 1: all edges are pair edges (k0 >= ng, k0 + CH <= dv); MODE 3: all are edges of triple rows (k0 >= ngh,
+// k0 + CH <= ng); MODE 2: all are gen edges (k0 + CH <= ng); MODE 0: anything (per-edge predicates).
 template <int TB, int FV, int CH, bool FINAL, int MODE>
 __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
     float tv[CH][FV], wv[CH][FV];
@@ -77,6 +78,35 @@ __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
 #pragma unroll
             for (int v = 0; v < FV; ++v) {
                 const float mk = cn_rule(wv[j][v], tv[j][v]);
+                cx.s_m[((k0 + j) * FV + v) * TB] = mk;
+                cx.sum[v] += mk;
+            }
+        }
+    } else if constexpr (MODE == 3) {
+        // triple row: two partners, an absorbed variable, no parity to report.  (a [+] b) [+] |t| as one fraction:
+        // num = a + b + |t| (1 + a b), den = 1 + a b + |t| (a + b): no reciprocal in between
+        float pa[CH][FV], pb[CH][FV];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            const unsigned ot = stream_off(cx.s_t[k0 + j], cx.lane, cx.Z);
+            const unsigned oa = stream_off(cx.s_p[k0 + j], cx.lane, cx.Z);
+            const unsigned ob = stream_off(cx.s_p2[k0 + j], cx.lane, cx.Z);
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                tv[j][v] = __ldg(byte_ptr(cx.tP[v], ot));
+                pa[j][v] = __ldg(byte_ptr(cx.qP[v], oa));
+                pb[j][v] = __ldg(byte_ptr(cx.qP[v], ob));
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                const unsigned ua = __float_as_uint(pa[j][v]), ub = __float_as_uint(pb[j][v]);
+                const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
+                float num = qa + qb, den = fmaf(qa, qb, 1.0f);
+                boxplus_acc(fabsf(tv[j][v]), num, den);
+                const float mk = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j][v])) & 0x80000000u);
                 cx.s_m[((k0 + j) * FV + v) * TB] = mk;
                 cx.sum[v] += mk;
             }
@@ -133,24 +163,38 @@ __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
                     boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
                 }
             }
+            // rows of degree > kGenSlots + 1: kGenMore partners per round trip (an empty slot is +0.0, the identity)
 #pragma unroll 1
-            for (int jj = kGenSlots; jj < np[j]; ++jj) {     // rows of degree > kGenSlots + 1
-                const unsigned op = stream_off(cx.s_po[pbeg[j] + jj], cx.lane, cx.Z);
+            for (int jb = kGenSlots; jb < np[j]; jb += kGenMore) {
+                float pm[kGenMore][FV];
 #pragma unroll
-                for (int v = 0; v < FV; ++v) {
-                    const unsigned wb = __float_as_uint(__ldg(byte_ptr(cx.qP[v], op)));
-                    xa[v] ^= wb;
-                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                for (int u = 0; u < kGenMore; ++u) {
+                    const bool have = jb + u < np[j];
+                    const unsigned op = stream_off(cx.s_po[pbeg[j] + (have ? jb + u : 0)], cx.lane, cx.Z);
+#pragma unroll
+                    for (int v = 0; v < FV; ++v) pm[u][v] = have ? __ldg(byte_ptr(cx.qP[v], op)) : 0.0f;
                 }
+#pragma unroll
+                for (int u = 0; u < kGenMore; ++u)
+#pragma unroll
+                    for (int v = 0; v < FV; ++v) {
+                        const unsigned wb = __float_as_uint(pm[u][v]);
+                        xa[v] ^= wb;
+                        boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                    }
             }
 #pragma unroll
             for (int v = 0; v < FV; ++v) {
-                wv[j][v] = with_sign(num[v] * rcp_approx(den[v]), xa[v] & 0x80000000u);
                 if (!FINAL && ctr[j])        // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
                     cx.bad[v] |= (xa[v] ^ cx.xb[v] ^ (__float_as_uint(tv[j][v]) >> 31)) & (cx.valid ? 1u : 0u);
+                // the static term joins the same fraction (as in MODE 3: an edge's message does not depend on the
+                // body that computes it)
+                boxplus_acc(fabsf(tv[j][v]), num[v], den[v]);
+                const float mk = with_sign(mag_of(num[v], den[v]), (xa[v] ^ __float_as_uint(tv[j][v])) & 0x80000000u);
+                cx.s_m[(k * FV + v) * TB] = mk;
+                cx.sum[v] += mk;
             }
-        }
-        if (MODE == 2 || k < cx.dv) {
+        } else if (k < cx.dv) {
 #pragma unroll
             for (int v = 0; v < FV; ++v) {
                 const float mk = cn_rule(wv[j][v], tv[j][v]);
@@ -165,7 +209,7 @@ __device__ __forceinline__ void chunk_cn(PassCtx<TB, FV>& cx, const int k0) {
 
 // dynamic shared memory: stream tables, then the messages m'_cv of the tile [max_dv][FV][TB], then partial sums [G][FV][TB]
 inline size_t pass_any_table_bytes(int max_np) {
-    return (size_t)kMaxDv * (2 * sizeof(StreamDesc) + sizeof(GenDesc)) + (size_t)(max_np > 0 ? max_np : 1) * sizeof(StreamDesc);
+    return (size_t)kMaxDv * (3 * sizeof(StreamDesc) + sizeof(GenDesc)) + (size_t)(max_np > 0 ? max_np : 1) * sizeof(StreamDesc);
 }
 inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups, int fv) {
     return pass_any_table_bytes(max_np) + (size_t)((max_dv > 0 ? max_dv : 1) + groups) * fv * tb * sizeof(float);
@@ -188,7 +232,8 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     extern __shared__ __align__(16) unsigned char smem_any[];
     StreamDesc* const s_t = reinterpret_cast<StreamDesc*>(smem_any);          // [kMaxDv] t of edge k
     StreamDesc* const s_p = s_t + kMaxDv;                                     // [kMaxDv] partner of pair edge k
-    GenDesc* const s_gd = reinterpret_cast<GenDesc*>(s_p + kMaxDv);           // [kMaxDv] gen edges
+    StreamDesc* const s_p2 = s_p + kMaxDv;                                    // [kMaxDv] second partner of triple edge k
+    GenDesc* const s_gd = reinterpret_cast<GenDesc*>(s_p2 + kMaxDv);          // [kMaxDv] gen edges
     StreamDesc* const s_po = reinterpret_cast<StreamDesc*>(s_gd + kMaxDv);    // [np] partners of the gen edges
     float* const s_m = reinterpret_cast<float*>(smem_any + a.table_bytes) + threadIdx.x;
     float* const s_part = reinterpret_cast<float*>(smem_any + a.table_bytes) + a.max_dv * FV * TB;
@@ -224,7 +269,7 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     const int tile = blockIdx.x - ca * a.tiles;
     const ColDesc cd = tab.col[ca];
     const int Z = a.Z, Zs = a.Zs;
-    const int dv = cd.dv, ng = cd.ng;
+    const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
     const int tid = threadIdx.x, grp = threadIdx.y;
     const int flat = grp * TB + tid;
     const int i0 = tile * TB;
@@ -238,7 +283,9 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         int r0 = i0 - d.shift; r0 += (r0 < 0) ? Z : 0;        // check index of the tile's first variable (i0, shift < Z)
         int x0 = i0 + d.delta; x0 -= (x0 >= Z) ? Z : 0;       // delta < Z: one wrap at most, no division
         s_t[k] = StreamDesc{(unsigned)d.t_off, (unsigned)r0};
+        int x1 = i0 + d.delta2; x1 -= (x1 >= Z) ? Z : 0;
         s_p[k] = StreamDesc{(unsigned)(d.p_off >= 0 ? d.p_off : 0), (unsigned)(d.p_off >= 0 ? x0 : 0)};
+        s_p2[k] = StreamDesc{(unsigned)(d.p2_off >= 0 ? d.p2_off : 0), (unsigned)(d.p2_off >= 0 ? x1 : 0)};
     }
     for (int g = flat; g < ng; g += TB * G) s_gd[g] = tab.gen[cd.gbeg + g];
     for (int j = flat; j < cd.np; j += TB * G) {
@@ -263,12 +310,12 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         cx.sum[v] = 0.0f; cx.bad[v] = 0u;
         Q[v] = valid ? llr_to_log2(__ldg(a.llr + (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
     }
-    cx.s_t = s_t; cx.s_p = s_p; cx.s_gd = s_gd; cx.s_po = s_po; cx.s_m = s_m;
+    cx.s_t = s_t; cx.s_p = s_p; cx.s_p2 = s_p2; cx.s_gd = s_gd; cx.s_po = s_po; cx.s_m = s_m;
     cx.lane = (unsigned)lane; cx.Z = (unsigned)Z; cx.dv = dv; cx.ng = ng; cx.valid = valid;
 
     // The chunk loop is NOT unrolled (a fully unrolled body for 64 edges is 170 KB of code: the pass becomes bound by
     // instruction fetch); the messages of the tile wait in shared memory for the variable-node rule instead.  A chunk
-    // whose edges are all pair edges, or all gen edges, runs a body without per-edge predicates.
+    // whose edges are all pair edges, all edges of triple rows, or all gen edges, runs a body without per-edge predicates.
     // Edge k belongs to group (k / kChunk) mod G whatever FV is, and every group adds its messages in increasing k: a
     // frame's result does not depend on the batch it is decoded in (bit for bit).
 #pragma unroll 1
@@ -276,6 +323,7 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
 #pragma unroll 1
         for (int k0 = kb; k0 < min(kb + kChunk, dv); k0 += CH) {
             if (k0 >= ng && k0 + CH <= dv) chunk_cn<TB, FV, CH, FINAL, 1>(cx, k0);
+            else if (k0 >= ngh && k0 + CH <= ng) chunk_cn<TB, FV, CH, FINAL, 3>(cx, k0);
             else if (k0 + CH <= ng) chunk_cn<TB, FV, CH, FINAL, 2>(cx, k0);
             else chunk_cn<TB, FV, CH, FINAL, 0>(cx, k0);
         }
@@ -353,7 +401,7 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     static thread_local int attr_dev = -1;                  // the attribute is per device
     int dev = 0;
     cudaGetDevice(&dev);
-    if (attr_dev != dev) {      // tables (<= 18.4 KB) + messages can exceed the 48 KB default
+    if (attr_dev != dev) {      // tables (<= 18.9 KB) + messages can exceed the 48 KB default
         cudaFuncSetAttribute(k_pass<TB, G, FV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         cudaFuncSetAttribute(k_pass<TB, G, FV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         attr_dev = dev;

@@ -313,11 +313,13 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         for (const BaseEntry& e : B.rows[R]) n_active[R] += absorbed_by[e.idx] < 0;
     code->filter_rows = false;
     for (int R = 0; R < mb; ++R) {
-        code->row[R].gen = !(code->row[R].abs_col >= 0 && n_active[R] == 2);
+        const bool absorbed = code->row[R].abs_col >= 0;
+        code->row[R].gen = (absorbed && n_active[R] == 2) ? 0 : (absorbed && n_active[R] == 3) ? 2 : 1;
         code->filter_rows = code->filter_rows || (code->row[R].abs_col < 0 && n_active[R] > 0);
     }
 
-    // active columns and their edges: column by column, gen edges first, then pair edges, each in row order
+    // active columns and their edges: column by column, gen edges first (triple rows last among them), then pair
+    // edges, each in row order
     struct HostEdge { int shift, row; };
     std::vector<HostEdge> edges;
     std::vector<int> act_index(nb, -1);
@@ -333,14 +335,15 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     for (int C = 0; C < nb; ++C) {
         if (absorbed_by[C] >= 0) continue;
         ColDesc cd{C, (int)edges.size(), 0, 0, 0, 0, 0, 0};
-        for (int pass = 0; pass < 2; ++pass)
+        for (int pass = 0; pass < 3; ++pass)
             for (const BaseEntry& e : B.cols[C]) {
                 const int R = e.idx;
-                if ((code->row[R].gen != 0) != (pass == 0)) continue;
+                if (code->row[R].gen != (pass == 0 ? 1 : pass == 1 ? 2 : 0)) continue;
                 edge_of_row_entry[R][row_pos(R, C)] = (int)edges.size();
                 edges.push_back(HostEdge{e.shift, R});
                 ++cd.dv;
-                cd.ng += pass == 0;
+                cd.ng += pass < 2;
+                cd.ngh += pass == 0;
             }
         act_index[C] = (int)code->col.size();
         code->col.push_back(cd);
@@ -384,7 +387,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
             const int e = cd.ebeg + k;
             const HostEdge& he = edges[e];
             const RowDesc& rd = code->row[he.row];
-            EdgeDesc ed{he.shift, he.row * Zs, -1, 0};
+            EdgeDesc ed{he.shift, he.row * Zs, -1, 0, -1, 0};
             if (!rd.gen) {
                 for (int j = 0; j < rd.ne; ++j) {
                     const RowEdge& re = code->redge[rd.ebeg + j];
@@ -398,7 +401,12 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
                 for (int j = 0; j < rd.ne; ++j) {
                     const RowEdge& re = code->redge[rd.ebeg + j];
                     if (re.edge == e) continue;
-                    code->partner.push_back(PartnerDesc{re.edge * Zs, ((re.shift - he.shift) % Z + Z) % Z});
+                    const PartnerDesc pd{re.edge * Zs, ((re.shift - he.shift) % Z + Z) % Z};
+                    code->partner.push_back(pd);
+                    if (rd.gen == 2) {                       // triple row: both partners also travel with the edge
+                        if (ed.p_off < 0) { ed.p_off = pd.off; ed.delta = pd.delta; }
+                        else { ed.p2_off = pd.off; ed.delta2 = pd.delta; }
+                    }
                 }
                 code->gen.push_back(gd);
             }
