@@ -238,36 +238,23 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     float* const s_m = reinterpret_cast<float*>(smem_any + a.table_bytes) + threadIdx.x;
     float* const s_part = reinterpret_cast<float*>(smem_any + a.table_bytes) + a.max_dv * FV * TB;
 
+    // The loads of the prologue are ordered by dependence, not by meaning: the stop flags, the column descriptor and
+    // then everything that hangs on it (edge tables, Q, last iteration's hard decisions) are in flight together, and
+    // the flags are looked at last: three memory round trips before the first chunk instead of five.
     pdl_launch();
+    const int ca = blockIdx.x / a.tiles;                     // block-uniform active column
+    const int tile = blockIdx.x - ca * a.tiles;
+    const ColDesc cd = tab.col[ca];                          // tables: constant, not the previous launch's output
     pdl_wait();
-    // frames of this CTA; a frame that is out of range or stopped is not live: it is computed on the first live
-    // frame's data (valid memory) and nothing of it is stored
-    int fr[FV], in_buf[FV];
+    int fr[FV], in_buf[FV], flag[FV];
     bool live[FV];
-    int f_any = -1;
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
         fr[v] = blockIdx.y * FV + v;
         live[v] = fr[v] < a.n_frames;
-        in_buf[v] = a.in_buf;
-        if (live[v]) {
-            if (FINAL) {
-                const int T = a.iters[fr[v]];
-                live[v] = T > 0;                             // t = 0: k_init_cols wrote the outputs
-                in_buf[v] = (T + 3) % 4;                     // w^(T-1): buffer (T - 1) mod 4
-            } else {
-                live[v] = !a.done[fr[v]];                    // frame already stopped: its state stays frozen
-            }
-        }
-        if (live[v] && f_any < 0) f_any = v;
+        fr[v] = live[v] ? fr[v] : a.n_frames - 1;            // out of range: any valid frame, nothing of it is stored
+        flag[v] = FINAL ? a.iters[fr[v]] : a.done[fr[v]];
     }
-    if (f_any < 0) return;
-#pragma unroll
-    for (int v = 0; v < FV; ++v)
-        if (!live[v]) { fr[v] = fr[f_any]; in_buf[v] = in_buf[f_any]; }
-    const int ca = blockIdx.x / a.tiles;                     // block-uniform active column
-    const int tile = blockIdx.x - ca * a.tiles;
-    const ColDesc cd = tab.col[ca];
     const int Z = a.Z, Zs = a.Zs;
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
     const int tid = threadIdx.x, grp = threadIdx.y;
@@ -277,13 +264,13 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     const bool valid = i < Z;
     const int lane = valid ? tid : 0;                        // idle threads read element 0 of every window
 
-    // preamble: window starts of this tile, once per stream
+    // window starts of this tile, once per stream
     for (int k = flat; k < dv; k += TB * G) {
         const EdgeDesc d = tab.edge[cd.ebeg + k];
         int r0 = i0 - d.shift; r0 += (r0 < 0) ? Z : 0;        // check index of the tile's first variable (i0, shift < Z)
         int x0 = i0 + d.delta; x0 -= (x0 >= Z) ? Z : 0;       // delta < Z: one wrap at most, no division
-        s_t[k] = StreamDesc{(unsigned)d.t_off, (unsigned)r0};
         int x1 = i0 + d.delta2; x1 -= (x1 >= Z) ? Z : 0;
+        s_t[k] = StreamDesc{(unsigned)d.t_off, (unsigned)r0};
         s_p[k] = StreamDesc{(unsigned)(d.p_off >= 0 ? d.p_off : 0), (unsigned)(d.p_off >= 0 ? x0 : 0)};
         s_p2[k] = StreamDesc{(unsigned)(d.p2_off >= 0 ? d.p2_off : 0), (unsigned)(d.p2_off >= 0 ? x1 : 0)};
     }
@@ -293,10 +280,34 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         int x0 = i0 + p.delta; x0 -= (x0 >= Z) ? Z : 0;
         s_po[j] = StreamDesc{(unsigned)p.off, (unsigned)x0};
     }
-    __syncthreads();
-
     PassCtx<TB, FV> cx;
     float Q[FV];
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        cx.xb[v] = (!FINAL && ng > 0) ? a.hard_in[(int64_t)fr[v] * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
+        Q[v] = valid ? llr_to_log2(__ldg(a.llr + (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
+    }
+
+    // a frame that is out of range or stopped is not live: it is computed on the first live frame's state (valid
+    // memory) and nothing of it is stored
+    int f_any = -1;
+#pragma unroll
+    for (int v = 0; v < FV; ++v) {
+        in_buf[v] = a.in_buf;
+        if (FINAL) {
+            live[v] = live[v] && flag[v] > 0;                // t = 0: k_init_cols wrote the outputs
+            in_buf[v] = (flag[v] + 3) % 4;                   // w^(T-1): buffer (T - 1) mod 4
+        } else {
+            live[v] = live[v] && !flag[v];                   // frame already stopped: its state stays frozen
+        }
+        if (live[v] && f_any < 0) f_any = v;
+    }
+    if (f_any < 0) return;
+#pragma unroll
+    for (int v = 0; v < FV; ++v)
+        if (!live[v]) { fr[v] = fr[f_any]; in_buf[v] = in_buf[f_any]; }
+    __syncthreads();
+
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
         // opaque to the optimiser: otherwise the frame pointers are re-formed (64-bit multiply, constant loads) at
@@ -306,9 +317,7 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         asm volatile("" : "+l"(qP_u), "+l"(tP_u));
         cx.qP[v] = reinterpret_cast<const float*>(qP_u);
         cx.tP[v] = reinterpret_cast<const float*>(tP_u);
-        cx.xb[v] = (!FINAL && ng > 0) ? a.hard_in[(int64_t)fr[v] * a.AZs + (int64_t)ca * Zs + (valid ? i : 0)] : 0u;
         cx.sum[v] = 0.0f; cx.bad[v] = 0u;
-        Q[v] = valid ? llr_to_log2(__ldg(a.llr + (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
     }
     cx.s_t = s_t; cx.s_p = s_p; cx.s_p2 = s_p2; cx.s_gd = s_gd; cx.s_po = s_po; cx.s_m = s_m;
     cx.lane = (unsigned)lane; cx.Z = (unsigned)Z; cx.dv = dv; cx.ng = ng; cx.valid = valid;
