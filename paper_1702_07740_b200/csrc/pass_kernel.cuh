@@ -325,10 +325,12 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     // The chunk loop is NOT unrolled (a fully unrolled body for 64 edges is 170 KB of code: the pass becomes bound by
     // instruction fetch); the messages of the tile wait in shared memory for the variable-node rule instead.  A chunk
     // whose edges are all pair edges, all edges of triple rows, or all gen edges, runs a body without per-edge predicates.
-    // Edge k belongs to group (k / kChunk) mod G whatever FV is, and every group adds its messages in increasing k: a
-    // frame's result does not depend on the batch it is decoded in (bit for bit).
+    // Blocks of kChunk edges go to the groups in boustrophedon order (0 .. G-1, G-1 .. 0, ...: the group with the
+    // column's first block, where the long gen rows are, gets the last, short one) whatever FV is, and every group
+    // adds its messages in increasing k: a frame's result does not depend on the batch it is decoded in (bit for bit).
 #pragma unroll 1
-    for (int kb = grp * kChunk; kb < dv; kb += G * kChunk) {
+    for (int rnd = 0; rnd * G * kChunk < dv; ++rnd) {
+        const int kb = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kChunk;
 #pragma unroll 1
         for (int k0 = kb; k0 < min(kb + kChunk, dv); k0 += CH) {
             if (k0 >= ng && k0 + CH <= dv) chunk_cn<TB, FV, CH, FINAL, 1>(cx, k0);
@@ -376,9 +378,9 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         if (!live[v] || !valid) continue;
         float* const sp = a.qb[a.out_buf] + (int64_t)fr[v] * a.EZs + (int64_t)cd.ebeg * Zs + i;
 #pragma unroll 1
-        for (int kb = grp * kChunk; kb < dv; kb += G * kChunk)
+        for (int rnd = 0; rnd * G * kChunk < dv; ++rnd)
 #pragma unroll 1
-        for (int k0 = kb; k0 < min(kb + kChunk, dv); k0 += CH) {
+        for (int k0 = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kChunk, kb = k0; k0 < min(kb + kChunk, dv); k0 += CH) {
             if (k0 >= ng && k0 + CH <= dv) {                 // pair edges only: no tags, no bounds
 #pragma unroll
                 for (int j = 0; j < CH; ++j) {
