@@ -92,6 +92,7 @@ struct PassLaunch {
     const void* check_tab;     // HOST: CheckTables / CheckArgs of the early-exit check this launch carries in its grid
     const void* check_args;    //       (exact families; NULL: none)
     int n_cols, n_frames, max_np, max_dv;
+    int n_sm;                  // multiprocessors of the device
 };
 using PassLauncher = void (*)(const PassLaunch&);
 using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only

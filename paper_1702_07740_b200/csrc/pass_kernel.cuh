@@ -420,7 +420,7 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     // the early-exit check of iteration t-2 rides in extra CTAs of the same grid (check.cuh): about four per SM
     const bool with_check = !L.final_mode && L.check_args != nullptr;
     const int rows_y = (L.n_frames + FV - 1) / FV;
-    const int extra = with_check ? std::max(1, std::min(args.tiles * L.n_cols, (4 * 148 + rows_y - 1) / rows_y)) : 0;
+    const int extra = with_check ? std::max(1, std::min(args.tiles * L.n_cols, (4 * L.n_sm + rows_y - 1) / rows_y)) : 0;
     static const CheckTables no_tab{nullptr, nullptr};
     static const CheckArgs no_args{};
     CheckArgs chk = with_check ? *static_cast<const CheckArgs*>(L.check_args) : no_args;

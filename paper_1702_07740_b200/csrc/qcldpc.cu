@@ -541,7 +541,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
                   st, V, false,
                   code->exact.empty() ? nullptr : code->exact.data(), nullptr, nullptr, code->n_act_cols, n_frames,
-                  code->max_np, code->max_dv};
+                  code->max_np, code->max_dv, code->n_sm};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
                  {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
                  d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
