@@ -9,9 +9,10 @@
 // reads the cyclic window [x0, x0 + TB) of a run with one compare-subtract per element, x0 block-uniform from the
 // preamble (tables in shared memory).
 //   edges are processed in chunks of kChunk with all loads of a chunk in flight: t of the row, then either the single
-//   partner (pair row: two active edges + one absorbed variable) or the fold of all other edges of a gen row; the
-//   row's counter edge also forms the parity of the PREVIOUS iteration's hard decisions from the bit-0 tags;
-//   check-node rule per edge -> m[k] (registers, compile-time indexed);
+//   partner (pair row: two active edges + one absorbed variable), the two partners of a triple row (three active
+//   edges + one absorbed variable), or the fold of all other edges of a gen row; the row's counter edge also forms
+//   the parity of the PREVIOUS iteration's hard decisions from the bit-0 tags;
+//   check-node rule per edge -> m[k] (shared memory, one column of the tile per thread);
 //   variable-node rule: L_v = Q_v + sum m, xhat_v, L_vc = L_v - m_cv (the LLR-domain difference is
 //   benign: |m| <= 30; the cancellation hazard of SURVEY N3 is on the check-node side, where exclusion stays direct).
 // FV = 2 (batched decodes): a thread carries the same variable of TWO frames; the table lookups, window indices and
