@@ -145,6 +145,54 @@ def test_gpu_paper_ensemble_early_stop(oracle_lib):
     np.testing.assert_array_equal(W.syndrome_of_sparse(rows, cols, shifts, mb, nb, 50, hard[ok]), fr.syndrome[ok])
 
 
+def _mixed_rows_code(rng, nc, kinds, q):
+    """Test input only: nc core columns; `kinds` = [(core edges, has degree-1 column, count)] rows in that order, core
+    sockets drawn without repetition inside a row.  Rows with a degree-1 column and 2 / 3 / more core edges are the
+    pair / triple / gen rows of the generic kernel; rows without one report the parity (counter edges)."""
+    rows, cols, r, n_abs = [], [], 0, 0
+    for n_core, has_abs, count in kinds:
+        for _ in range(count):
+            for c in rng.choice(nc, size=n_core, replace=False):
+                rows.append(r); cols.append(int(c))
+            if has_abs:
+                rows.append(r); cols.append(nc + n_abs); n_abs += 1
+            r += 1
+    rows, cols = np.asarray(rows, np.int32), np.asarray(cols, np.int32)
+    return rows, cols, rng.integers(0, q, size=len(rows)).astype(np.int32), r, nc + n_abs
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", ["triples only", "all kinds", "triples across chunks", "long columns", "tiny q"])
+@pytest.mark.parametrize("n_frames", [1, 5])
+def test_gpu_row_kinds_of_the_generic_kernel(oracle_lib, case, n_frames):
+    """Every chunk body of the generic pass (pair, triple, gen, mixed), with the boundaries between the edge classes of
+    a column falling at different places of the 4- and 8-edge chunks, one and two frames per thread."""
+    from paper_1702_07740_b200 import binding as B
+    rng = np.random.default_rng(sum(map(ord, case)))
+    nc, q, sigma, kinds = {
+        "triples only": (6, 33, 2.0, [(3, True, 40)]),
+        "all kinds": (9, 70, 3.2, [(2, False, 3), (3, False, 2), (7, False, 2), (4, True, 5), (3, True, 30), (2, True, 25)]),
+        "triples across chunks": (5, 50, 2.0, [(5, False, 1), (3, True, 21), (2, True, 9)]),
+        "long columns": (4, 130, 4.5, [(3, False, 2), (4, False, 3), (3, True, 60), (2, True, 20), (1, True, 3)]),
+        "tiny q": (7, 5, 3.2, [(2, False, 2), (3, True, 35), (2, True, 14)]),
+    }[case]
+    rows, cols, shifts, mb, nb = _mixed_rows_code(rng, nc, kinds, q)
+    assert np.bincount(cols[cols < nc], minlength=nc).max() <= 64
+    code = B.QCLDPCCode.from_sparse(rows, cols, shifts, mb, nb, q)
+    # fixed iterations near the code's limit (messages of every size), early stop well inside it (no marginal frames)
+    for n_iter, early, sg in ((7, 0, sigma), (40, 1, 0.6 * sigma)):
+        fr = W.make_frames_sparse(rows, cols, shifts, mb, nb, q, sg, n_frames, 31337)
+        ref = oracle_lib.decode_sparse(rows, cols, shifts, mb, nb, q, fr.llr, fr.syndrome, n_iter, early)
+        hard, iters, passed, post = _gpu_decode(code, fr.llr, fr.syndrome, n_iter, early)
+        np.testing.assert_array_equal(passed, ref.passed)
+        np.testing.assert_array_equal(iters, ref.iters)
+        assert early == 0 or (ref.passed.all() and ref.iters.max() < 40)
+        err = np.abs(post - ref.posterior) / np.maximum(1.0, np.abs(ref.posterior))
+        assert err.max() <= TOL, (case, n_iter, err.max())
+        decided = np.abs(ref.posterior) > 1e-2
+        np.testing.assert_array_equal(hard[decided], ref.hard[decided])
+
+
 @pytest.mark.gpu
 def test_gpu_generic_kernel_frame_independence():
     """Batched decodes carry two frames per thread in the generic kernel, single frames one: a frame's outputs must not
