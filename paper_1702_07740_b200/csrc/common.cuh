@@ -69,6 +69,7 @@ struct PassArgs {
     int n_frames;              // generic kernel: frames of the batch (two per thread when batched)
     int cand_y;                // exact kernels: blockIdx.y of the CTAs that run the early-exit check (check.cuh), or -1
     int64_t n, EZs, mZs, AZs;  // per-frame strides
+    int pack;                  // generic pass: frames side by side in one tile (circulants of at most half a tile), >= 1
 };
 
 // Codes whose active columns all have the same shape (DV edges, the first NG of them gen edges; at most kMaxExactCols

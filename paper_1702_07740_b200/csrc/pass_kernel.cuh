@@ -24,6 +24,7 @@
 #include "common.cuh"
 
 #include <algorithm>
+#include <cstdlib>
 
 namespace qc {
 
@@ -219,7 +220,7 @@ inline size_t pass_any_smem(int max_np, int max_dv, int tb, int groups, int fv) 
 // G = edge groups: the CTA is TB x G threads, thread (tid, grp) handles the chunks grp, grp + G, ... of the column's
 // edges, so a column of degree 60 is four chains of 15 edges instead of one of 60 (the pass of a single frame is bound
 // by that chain's latency); the partial sums of the groups meet in shared memory.
-template <int TB, int G, int FV, bool FINAL>
+template <int TB, int G, int FV, bool FINAL, bool PACK>
 __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTables tab, const PassArgs a,
                                                                   const CheckTables ctab, const CheckArgs chk) {
     constexpr int CH = kChunk / FV;                           // edges per chunk: the loads in flight stay the same
@@ -247,23 +248,29 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     const int tile = blockIdx.x - ca * a.tiles;
     const ColDesc cd = tab.col[ca];                          // tables: constant, not the previous launch's output
     pdl_wait();
+    // PACK: frames side by side in the tile when the circulant is at most half of it (one tile per column): thread
+    // tid carries variable tid mod Z of the tile's frame tid / Z, so a circulant of 21 fills 63 of 64 lanes instead
+    // of 21 of 32.  Frame of (CTA row y, v, sub) = (y FV + v) pack + sub; liveness is then per lane.
+    const int Z = a.Z, Zs = a.Zs;
+    const int tid = threadIdx.x, grp = threadIdx.y;
+    const int sub_raw = PACK ? tid / Z : 0;
+    const int i0 = tile * TB;
+    const int li = tid - sub_raw * Z;                        // position in the tile's window
+    const int i = i0 + li;
+    const bool valid = PACK ? sub_raw < a.pack : i < Z;
+    const int lane = valid ? li : 0;                         // idle threads read element 0 of every window
     int fr[FV], in_buf[FV], flag[FV];
     bool live[FV];
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
-        fr[v] = blockIdx.y * FV + v;
+        fr[v] = PACK ? ((int)blockIdx.y * FV + v) * a.pack + (valid ? sub_raw : 0) : (int)blockIdx.y * FV + v;
         live[v] = fr[v] < a.n_frames;
         fr[v] = live[v] ? fr[v] : a.n_frames - 1;            // out of range: any valid frame, nothing of it is stored
+        if (PACK) live[v] = live[v] && valid;
         flag[v] = FINAL ? a.iters[fr[v]] : a.done[fr[v]];
     }
-    const int Z = a.Z, Zs = a.Zs;
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
-    const int tid = threadIdx.x, grp = threadIdx.y;
     const int flat = grp * TB + tid;
-    const int i0 = tile * TB;
-    const int i = i0 + tid;
-    const bool valid = i < Z;
-    const int lane = valid ? tid : 0;                        // idle threads read element 0 of every window
 
     // window starts of this tile, once per stream
     for (int k = flat; k < dv; k += TB * G) {
@@ -289,8 +296,8 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         Q[v] = valid ? llr_to_log2(__ldg(a.llr + (int64_t)fr[v] * a.n + (int64_t)cd.col * Z + i)) : 0.0f;
     }
 
-    // a frame that is out of range or stopped is not live: it is computed on the first live frame's state (valid
-    // memory) and nothing of it is stored
+    // a frame that is out of range or stopped is not live: it is computed on valid memory (the first live frame's
+    // state; PACK: the frame's own, stale buffers) and nothing of it is stored; a CTA without a live frame leaves
     int f_any = -1;
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
@@ -303,11 +310,15 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
         }
         if (live[v] && f_any < 0) f_any = v;
     }
-    if (f_any < 0) return;
+    if constexpr (PACK) {
+        if (!__syncthreads_or(f_any >= 0)) return;           // the vote is also the barrier of the prologue
+    } else {
+        if (f_any < 0) return;
 #pragma unroll
-    for (int v = 0; v < FV; ++v)
-        if (!live[v]) { fr[v] = fr[f_any]; in_buf[v] = in_buf[f_any]; }
-    __syncthreads();
+        for (int v = 0; v < FV; ++v)
+            if (!live[v]) { fr[v] = fr[f_any]; in_buf[v] = in_buf[f_any]; }
+        __syncthreads();
+    }
 
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
@@ -367,7 +378,11 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
             }
         } else if (live[v]) {
             if (valid && grp == 0) a.hard_out[(int64_t)fr[v] * a.AZs + (int64_t)ca * Zs + i] = (uint8_t)xh[v];
-            if (ng > 0 && __any_sync(__activemask(), cx.bad[v] != 0) && (tid & 31) == 0) a.topbad[fr[v]] = 1;
+            if (PACK) {                                      // lanes of one frame: one address, one transaction
+                if (ng > 0 && cx.bad[v] != 0) a.topbad[fr[v]] = 1;
+            } else if (ng > 0 && __any_sync(__activemask(), cx.bad[v] != 0) && (tid & 31) == 0) {
+                a.topbad[fr[v]] = 1;
+            }
         }
     }
     if (FINAL) return;
@@ -404,7 +419,7 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     }
 }
 
-template <int TB, int G, int FV>
+template <int TB, int G, int FV, bool PACK>
 inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     args.tiles = (args.Z + TB - 1) / TB;
     args.max_dv = L.max_dv > 0 ? L.max_dv : 1;
@@ -414,13 +429,15 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     int dev = 0;
     cudaGetDevice(&dev);
     if (attr_dev != dev) {      // tables (<= 18.9 KB) + messages can exceed the 48 KB default
-        cudaFuncSetAttribute(k_pass<TB, G, FV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        cudaFuncSetAttribute(k_pass<TB, G, FV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(k_pass<TB, G, FV, true, PACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(k_pass<TB, G, FV, false, PACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         attr_dev = dev;
     }
     // the early-exit check of iteration t-2 rides in extra CTAs of the same grid (check.cuh): about four per SM
     const bool with_check = !L.final_mode && L.check_args != nullptr;
-    const int rows_y = (L.n_frames + FV - 1) / FV;
+    args.pack = PACK ? args.pack : 1;
+    const int per_row = FV * args.pack;                     // frames per CTA row
+    const int rows_y = (L.n_frames + per_row - 1) / per_row;
     const int extra = with_check ? std::max(1, std::min(args.tiles * L.n_cols, (4 * L.n_sm + rows_y - 1) / rows_y)) : 0;
     static const CheckTables no_tab{nullptr, nullptr};
     static const CheckArgs no_args{};
@@ -429,23 +446,44 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     args.cand_y = with_check ? args.tiles * L.n_cols : -1;
     const dim3 grid(args.tiles * L.n_cols + extra, rows_y), block(TB, G);
     const CheckTables& ctab = with_check ? *static_cast<const CheckTables*>(L.check_tab) : no_tab;
-    if (L.final_mode) k_pass<TB, G, FV, true><<<grid, block, smem, L.stream>>>(L.tab, args, ctab, chk);
-    else launch_pdl(k_pass<TB, G, FV, false>, grid, block, smem, L.stream, L.tab, args, ctab, chk);
+    if (L.final_mode) k_pass<TB, G, FV, true, PACK><<<grid, block, smem, L.stream>>>(L.tab, args, ctab, chk);
+    else launch_pdl(k_pass<TB, G, FV, false, PACK>, grid, block, smem, L.stream, L.tab, args, ctab, chk);
 }
 
 template <int TB>
 inline void launch_pass_z(const PassLaunch& L, const PassArgs& args) {
     const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
     const bool pair = L.n_frames >= 4;                      // batched: two frames per thread
-    if (split) { if (pair) launch_pass_tb<TB, 4, 2>(L, args); else launch_pass_tb<TB, 4, 1>(L, args); }
-    else { if (pair) launch_pass_tb<TB, 1, 2>(L, args); else launch_pass_tb<TB, 1, 1>(L, args); }
+    const bool pack = args.pack > 1;                        // several frames side by side in a tile
+    if (split) {
+        if (pair) { if (pack) launch_pass_tb<TB, 4, 2, true>(L, args); else launch_pass_tb<TB, 4, 2, false>(L, args); }
+        else { if (pack) launch_pass_tb<TB, 4, 1, true>(L, args); else launch_pass_tb<TB, 4, 1, false>(L, args); }
+    } else {
+        if (pair) { if (pack) launch_pass_tb<TB, 1, 2, true>(L, args); else launch_pass_tb<TB, 1, 2, false>(L, args); }
+        else { if (pack) launch_pass_tb<TB, 1, 1, true>(L, args); else launch_pass_tb<TB, 1, 1, false>(L, args); }
+    }
 }
 
 inline void launch_pass_any(const PassLaunch& L) {
     PassArgs args = L.args;
     args.table_bytes = (int)pass_any_table_bytes(L.max_np);
-    if (args.Z <= 32) launch_pass_z<32>(L, args);
-    else if (args.Z <= 64) launch_pass_z<64>(L, args);
+    // tile width: the one whose lanes are best used, frames packed side by side where the circulant is at most half a
+    // tile (kernel header); ties go to the narrower tile
+    const int Z = args.Z, fv = L.n_frames >= 4 ? 2 : 1;
+    const int rows = (L.n_frames + fv - 1) / fv;            // frames (or frame pairs) there are to pack
+    int best_tb = 128, best_pack = 1;
+    double best_use = -1.0;
+    for (int tb = 32; tb <= 128; tb *= 2) {
+        if (tb < Z && tb < 128) continue;
+        const int pack = 2 * Z <= tb ? std::min(tb / Z, rows) : 1;
+        const int tiles = (Z + tb - 1) / tb;
+        const double use = (double)pack * Z / ((double)tiles * tb);
+        if (use > best_use + 1e-9) { best_use = use; best_tb = tb; best_pack = pack; }
+    }
+    if (const char* pk = getenv("QCLDPC_PACK")) { if (atoi(pk) == 0) { best_pack = 1; best_tb = Z <= 32 ? 32 : Z <= 64 ? 64 : 128; } }
+    args.pack = best_pack;
+    if (best_tb == 32) launch_pass_z<32>(L, args);
+    else if (best_tb == 64) launch_pass_z<64>(L, args);
     else launch_pass_z<128>(L, args);
 }
 
