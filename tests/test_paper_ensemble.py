@@ -163,10 +163,11 @@ def _mixed_rows_code(rng, nc, kinds, q):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("case", ["triples only", "all kinds", "triples across chunks", "long columns", "tiny q"])
-@pytest.mark.parametrize("n_frames", [1, 5])
+@pytest.mark.parametrize("n_frames", [1, 5, 26])
 def test_gpu_row_kinds_of_the_generic_kernel(oracle_lib, case, n_frames):
     """Every chunk body of the generic pass (pair, triple, gen, mixed), with the boundaries between the edge classes of
-    a column falling at different places of the 4- and 8-edge chunks, one and two frames per thread."""
+    a column falling at different places of the 4- and 8-edge chunks, one and two frames per thread, and (26 frames) six
+    frames of q = 5 or three of q = 33 side by side in a tile."""
     from paper_1702_07740_b200 import binding as B
     rng = np.random.default_rng(sum(map(ord, case)))
     nc, q, sigma, kinds = {
@@ -201,17 +202,21 @@ def test_gpu_generic_kernel_frame_independence():
     spec = W.paper_ensemble_spec(400, 21)
     rows, cols, shifts, mb, nb = W.make_paper_ensemble(spec)
     code = B.QCLDPCCode.from_sparse(rows, cols, shifts, mb, nb, 21)
-    hi = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 3.0), 4, 555)
-    lo = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 0.3), 3, 556)
-    llr = np.concatenate([hi.llr[:2], lo.llr[:1], hi.llr[2:], lo.llr[1:]])          # 7 frames, converging and not
-    syn = np.concatenate([hi.syndrome[:2], lo.syndrome[:1], hi.syndrome[2:], lo.syndrome[1:]])
-    for early in (0, 1):
-        batch = _gpu_decode(code, llr, syn, 40, early)
-        assert early == 0 or (0 < batch[2].sum() < 7)                                # some stop early, some do not
-        for f in range(7):
-            alone = _gpu_decode(code, llr[f:f + 1], syn[f:f + 1], 40, early)
-            for a, b in zip(batch, alone):
-                np.testing.assert_array_equal(a[f], b[0])
+    hi = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 3.0), 8, 555)
+    lo = W.make_frames_sparse(rows, cols, shifts, mb, nb, 21, W.sigma_for_gap(0.02, 0.3), 5, 556)
+    order = [0, 1, 8, 2, 3, 9, 10, 4, 5, 6, 11, 7, 12]                                # converging and not, mixed
+    llr13, syn13 = np.concatenate([hi.llr, lo.llr])[order], np.concatenate([hi.syndrome, lo.syndrome])[order]
+    # 7 frames: two frames per thread; 13 frames: also three frames side by side in a tile (q = 21 in 64 lanes), the
+    # last CTA row with a single frame
+    for n in (7, 13):
+        llr, syn = llr13[:n], syn13[:n]
+        for early in (0, 1):
+            batch = _gpu_decode(code, llr, syn, 40, early)
+            assert early == 0 or (0 < batch[2].sum() < n)                            # some stop early, some do not
+            for f in range(n):
+                alone = _gpu_decode(code, llr[f:f + 1], syn[f:f + 1], 40, early)
+                for a_, b_ in zip(batch, alone):
+                    np.testing.assert_array_equal(a_[f], b_[0])
 
 
 def test_rate10_standin_structure():
