@@ -24,6 +24,7 @@ constexpr float kMsgMax2 = QCLDPC_MSG_MAX * kLog2e;   // the clamp S2 in log2 un
 //     w[e * Zs + i] = sgn(L_vc) * 2^-|L'_vc|          (sign in the IEEE sign bit; S3: -0 never occurs)
 // Zs = round_up(Z + kHalo, 32): the run [0,Z) is followed by a copy of its first kHalo entries, so that a tile of
 // consecutive variables reads its cyclically shifted window [a, a + tile) with a < Z WITHOUT a per-element wrap.
+// (Codes of the generic pass: compact runs, Zs = round_up(Z, 8), no halo, the reader wraps per element.)
 // Edges of "gen" rows (see below) carry the hard decision xhat_v of their variable in mantissa bit 0 (the reader
 // masks it off: the magnitude never depends on it).
 // Static per check c of base row R, index r:

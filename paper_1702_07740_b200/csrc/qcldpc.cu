@@ -358,7 +358,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     const bool exact = uniform && code->n_act_cols <= kMaxExactCols && code->col[0].ng == 3 &&
                        (code->col[0].dv == 11 || code->col[0].dv == 21);
     code->halo = exact ? 1 : 0;
-    code->Zs = (int)align_up((size_t)Z + (exact ? kHalo : 0), 32);
+    code->Zs = exact ? (int)align_up((size_t)Z + kHalo, 32) : (int)align_up((size_t)Z, 8);   // whole 32-byte sectors
     const int Zs = code->Zs;
     // run offsets are formed as 32-bit BYTE offsets in the kernels: a frame's edge state and its static terms must each
     // stay below 2^30 floats
