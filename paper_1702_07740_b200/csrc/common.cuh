@@ -71,6 +71,8 @@ struct PassArgs {
     int cand_y;                // exact kernels: blockIdx.y of the CTAs that run the early-exit check (check.cuh), or -1
     int64_t n, EZs, mZs, AZs;  // per-frame strides
     int pack;                  // generic pass: frames side by side in one tile (circulants of at most half a tile), >= 1
+    int flip;                  // 1: the grid walks the frames backwards (odd iterations: the frames the previous launch
+                               // wrote last, still in L2, are read first)
 };
 
 // Codes whose active columns all have the same shape (DV edges, the first NG of them gen edges; at most kMaxExactCols

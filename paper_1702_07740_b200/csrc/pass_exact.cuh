@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(kThreads, V == 1 ? 7 : 4) k_pass_exact(const _
         cand_work(ctab, chk, blockIdx.z * gridDim.x + blockIdx.x, gridDim.x * gridDim.z, threadIdx.x, kThreads);
         return;
     }
-    const int f = blockIdx.z;
+    const int f = a.flip ? gridDim.z - 1 - blockIdx.z : blockIdx.z;
     const int ca = blockIdx.y;                               // block-uniform active column
     const ExactCol<DV, NG, PCAP>& cd = T.c[ca];
     const int Z = a.Z, Zs = a.Zs;

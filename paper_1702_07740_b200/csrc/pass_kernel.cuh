@@ -261,11 +261,12 @@ __global__ void __launch_bounds__(TB * G, 1024 / (TB * G)) k_pass(const PassTabl
     const int i = i0 + li;
     const bool valid = PACK ? sub_raw < a.pack : i < Z;
     const int lane = valid ? li : 0;                         // idle threads read element 0 of every window
+    const int row = a.flip ? (int)gridDim.y - 1 - (int)blockIdx.y : (int)blockIdx.y;   // CTA row of frames
     int fr[FV], in_buf[FV], flag[FV];
     bool live[FV];
 #pragma unroll
     for (int v = 0; v < FV; ++v) {
-        fr[v] = PACK ? ((int)blockIdx.y * FV + v) * a.pack + (valid ? sub_raw : 0) : (int)blockIdx.y * FV + v;
+        fr[v] = PACK ? (row * FV + v) * a.pack + (valid ? sub_raw : 0) : row * FV + v;
         live[v] = fr[v] < a.n_frames;
         fr[v] = live[v] ? fr[v] : a.n_frames - 1;            // out of range: any valid frame, nothing of it is stored
         if (PACK) live[v] = live[v] && valid;
@@ -452,10 +453,15 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     else launch_pdl(k_pass<TB, G, FV, false, PACK>, grid, block, smem, L.stream, L.tab, args, ctab, chk);
 }
 
+inline int pass_any_fv(int n_frames) {                      // frames per thread; QCLDPC_FV=1|2 overrides (tuning knob)
+    if (const char* e = getenv("QCLDPC_FV")) { if (atoi(e) == 1 || atoi(e) == 2) return atoi(e); }
+    return n_frames >= 4 ? 2 : 1;
+}
+
 template <int TB>
 inline void launch_pass_z(const PassLaunch& L, const PassArgs& args) {
     const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
-    const bool pair = L.n_frames >= 4;                      // batched: two frames per thread
+    const bool pair = pass_any_fv(L.n_frames) == 2;         // batched: two frames per thread
     const bool pack = args.pack > 1;                        // several frames side by side in a tile
     if (split) {
         if (pair) { if (pack) launch_pass_tb<TB, 4, 2, true>(L, args); else launch_pass_tb<TB, 4, 2, false>(L, args); }
@@ -471,7 +477,7 @@ inline void launch_pass_any(const PassLaunch& L) {
     args.table_bytes = (int)pass_any_table_bytes(L.max_np);
     // tile width: the one whose lanes are best used, frames packed side by side where the circulant is at most half a
     // tile (kernel header); ties go to the narrower tile
-    const int Z = args.Z, fv = L.n_frames >= 4 ? 2 : 1;
+    const int Z = args.Z, fv = pass_any_fv(L.n_frames);
     const int rows = (L.n_frames + fv - 1) / fv;            // frames (or frame pairs) there are to pack
     int best_tb = 128, best_pack = 1;
     double best_use = -1.0;

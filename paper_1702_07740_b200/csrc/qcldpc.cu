@@ -536,6 +536,8 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         const char* v = getenv("QCLDPC_V");
         if (v && (atoi(v) == 1 || atoi(v) == 2)) V = atoi(v);
     }
+    const char* fl = getenv("QCLDPC_FLIP");                // tuning knob: 0 = every launch walks the frames forwards
+    const bool flip_frames = !(fl && atoi(fl) == 0);
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
@@ -579,6 +581,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         const bool merged = merge_check && check_wanted(t - 2) && code->n_act_cols > 0;
         if (code->n_act_cols > 0) {
             pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
+            pl.args.flip = flip_frames ? (t & 1) : 0;
             pl.args.hard_in = w.hardbuf[(t - 1) % 3]; pl.args.hard_out = w.hardbuf[t % 3];
             pl.args.topbad = topbad_slot(t - 1);
             pl.args.done = done_ver(t);
