@@ -94,3 +94,24 @@ def tanh_rule_bp_dense(H: np.ndarray, Q: np.ndarray, s: np.ndarray, n_iter: int,
         Lv = Q + M.sum(axis=0)
         Lvc = np.where(Hb, Lv[None, :] - M, 0.0)
     return Lv
+
+
+def tie_cases():
+    """Inputs whose posterior L_v is EXACTLY zero in any IEEE arithmetic, so that Step 4 ("0 if L_v >= 0") is
+    decided by the tie rule alone.  Each case: (base, Z, llr [n], syndrome [m], max_iter, variables that tie).
+      zero column        a variable without any check: L_v = Q_v = +0.0 or -0.0 (max_iter = 0 takes the decisions of
+                         Step 1, max_iter > 0 those of Step 4);
+      clamped checks     a variable whose only neighbours are two checks of degree 1: the exclusion set of a degree-1
+                         check is empty, S = 0, |m_cv| = Phi(0) = inf clamped to 30 (reading S2), sign (-1)^{s_c}; with
+                         Q_v = -/+60 the posterior is -60 + 30 + 30 = 0 (s = 0) or 60 - 30 - 30 = 0 (s = 1): all terms
+                         dyadic multiples, exact in float and double in any summation order."""
+    cases = []
+    one_check = np.array([[-1, 0, 0]], dtype=np.int32)               # column 0 is empty
+    for q0 in (0.0, -0.0):
+        for it in (0, 3):
+            cases.append((one_check, 1, np.array([q0, 1.0, -2.0], np.float32), np.zeros(1, np.uint8), it, [0]))
+    two_leaves = np.array([[0], [0]], dtype=np.int32)                # one variable, two degree-1 checks
+    for Z in (1, 5):
+        cases.append((two_leaves, Z, np.full(Z, -60.0, np.float32), np.zeros(2 * Z, np.uint8), 2, list(range(Z))))
+        cases.append((two_leaves, Z, np.full(Z, 60.0, np.float32), np.ones(2 * Z, np.uint8), 2, list(range(Z))))
+    return cases

@@ -23,7 +23,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 from paper_1702_07740_b200 import workloads as W  # noqa: E402
-from tests.helpers import bitwise_map_llr, dense_h, random_tree_code  # noqa: E402
+from tests.helpers import bitwise_map_llr, dense_h, random_tree_code, tie_cases  # noqa: E402
 
 TOL = 1e-3
 HARD_MIN = 1e-2
@@ -227,6 +227,23 @@ def test_gpu_noiseless_limit_and_max_iter_zero(B, A):
     hard, iters, passed, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, 0, 0)
     np.testing.assert_array_equal(hard, (fr.llr < 0).astype(np.uint8))
     np.testing.assert_array_equal(passed.astype(bool), (W.syndrome_of(base, Z, hard) == fr.syndrome).all(axis=1))
+
+
+@pytest.mark.parametrize("k", range(8))
+def test_gpu_decision_tie_rule(oracle_lib, B, k):
+    """P:361 (reading S4) through the C ABI: posteriors that are exactly zero decide bit 0 (tests/helpers.tie_cases:
+    a variable without checks at Q = +0.0 / -0.0, and a variable between two clamped degree-1 checks at Q = -/+60)."""
+    base, Z, llr, syn, max_iter, ties = tie_cases()[k]
+    ref = oracle_lib.decode(base, Z, llr[None], syn[None], max_iter, 0)
+    hard, iters, passed, post = gpu_decode(B, base, Z, llr[None], syn[None], max_iter, 0)
+    assert (post[0, ties] == 0.0).all()
+    assert (hard[0, ties] == 0).all()
+    np.testing.assert_array_equal(hard, ref.hard)
+    np.testing.assert_array_equal(passed, ref.passed)
+    if max_iter > 0 and base.shape[1] == 1 and syn[0] == 0:
+        below = (llr - np.float32(1e-3))
+        hard, iters, passed, post = gpu_decode(B, base, Z, below[None], syn[None], max_iter, 0)
+        assert (post[0] < 0).all() and (hard[0] == 1).all()
 
 
 def test_gpu_frame_independence_and_permutation(B):

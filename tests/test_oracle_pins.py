@@ -12,6 +12,7 @@ P7  noiseless limit                                                             
 P8  degree-1 variable invariant                                                       -> posterior sum
 P9  lifting rule against np.roll of the identity                                      -> H construction
 P10 frame independence                                                                        -> batching
+S4  decision tie rule (bit 0 iff L_v >= 0) at posteriors that are EXACTLY zero          -> Step 4, both places
 +   dense tanh-product BP (another formula, another data structure) on small cyclic codes     -> flooding schedule
 """
 import math
@@ -20,7 +21,8 @@ import numpy as np
 import pytest
 
 from paper_1702_07740_b200 import workloads as W
-from tests.helpers import (bitwise_map_llr, block_ml_word, dense_h, random_tree_code, tanh_rule_bp_dense)
+from tests.helpers import (bitwise_map_llr, block_ml_word, dense_h, random_tree_code, tanh_rule_bp_dense,
+                           tie_cases)
 
 BIG = 1e300  # msg_max "disabled"
 
@@ -112,6 +114,26 @@ def test_clamp_and_degenerate_inputs(oracle_lib):
     assert np.isfinite(r.posterior).all() and np.isfinite(r.msg_cv).all()
     np.testing.assert_array_equal(np.abs(r.msg_cv[0]), [30.0, 30.0, 30.0])
     np.testing.assert_array_equal(np.sign(r.msg_cv[0]), [-1.0, 1.0, -1.0])
+
+
+# ------------------------------------------------------------------------------------------- S4 (P:361 tie rule)
+@pytest.mark.parametrize("k", range(8))
+def test_decision_tie_rule(oracle_lib, k):
+    """P:361 as printed (reading S4): L_v >= 0 -> bit 0, also at L_v = +0.0 and -0.0.  A decoder that tests L_v > 0
+    instead gives bit 1 on every variable below."""
+    base, Z, llr, syn, max_iter, ties = tie_cases()[k]
+    for prec in (64, 32):
+        r = oracle_lib.decode(base, Z, llr[None], syn[None], max_iter, 0, precision=prec)
+        assert (r.posterior[0, ties] == 0.0).all()
+        assert (r.hard[0, ties] == 0).all()
+    if base.shape[1] == 1:
+        # the all-zero decision satisfies s = 0 but not s = 1; the flag follows the decisions (a ">" decoder would
+        # report the opposite in both cases)
+        assert r.passed[0] == (1 if syn[0] == 0 else 0)
+    # just below the tie the bit is 1
+    if max_iter > 0 and base.shape[1] == 1 and syn[0] == 0:
+        r = oracle_lib.decode(base, Z, (llr - np.float32(1e-3))[None], syn[None], max_iter, 0)
+        assert (r.posterior[0] < 0).all() and (r.hard[0] == 1).all()
 
 
 # ----------------------------------------------------------------------------------------------------------- P1
