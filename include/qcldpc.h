@@ -25,11 +25,12 @@ extern "C" {
 #endif
 
 #define QCLDPC_MSG_MAX 30.0f /* clamp on |m_cv| (reading S2); part of the definition of the result */
+#define QCLDPC_MAX_FRAMES 65535 /* frames per decode call (one grid dimension of the kernels); more: split the batch */
 
 enum {
     QCLDPC_OK = 0,
     QCLDPC_ERR_BAD_ARGUMENT = -1, /* NULL pointer, non-positive size, shift outside [-1, Z), max_iter < 0, ... */
-    QCLDPC_ERR_UNSUPPORTED = -2,  /* code outside the supported envelope (a column of degree > 64) */
+    QCLDPC_ERR_UNSUPPORTED = -2,  /* code outside the supported envelope, see qcldpc_code_create */
     QCLDPC_ERR_WORKSPACE = -3,    /* workspace NULL, misaligned (256 B) or smaller than qcldpc_workspace_bytes */
     QCLDPC_ERR_CUDA = -4,         /* a CUDA runtime call failed; qcldpc_last_cuda_error() has the text */
     QCLDPC_ERR_ALLOC = -5         /* host allocation failed */
@@ -47,7 +48,17 @@ typedef struct qcldpc_code qcldpc_code_t;
  * The handle owns small device tables (allocated with cudaMalloc on the current device) and is immutable: it may be
  * used concurrently from several streams with distinct workspaces.  At most one degree-1 column per base row is
  * "absorbed" into that row (such variables send Q_v forever and need no edge state); every other column is
- * "active" and carries one fp32 of state per edge.  Active columns may have degree 0..64.
+ * "active" and carries one fp32 of state per edge.
+ * Supported envelope (else QCLDPC_ERR_UNSUPPORTED): active columns of degree 0..64; at most 2048 partner entries per
+ * active column (the sum, over the column's edges into rows that are not "two active edges + one absorbed variable",
+ * of that row's other active edges); mb*Z and nb*Z at most 2^30; a frame's edge state (active base edges x Z rounded up
+ * to a multiple of 8, or Z + 256 rounded up to 32 for the BASELINE.json column shapes) and mb x that run length each
+ * below 2^30 floats (the kernels form 32-bit byte offsets inside a frame).
+ * Tuning knobs: qcldpc_code_create reads these environment variables ONCE and stores them in the handle; no decode
+ * call reads the environment.  Defaults are the measured best.  QCLDPC_V=1|2 variables per thread
+ * of the exact pass; QCLDPC_FLIP=0 every launch walks the frames forwards; QCLDPC_MERGE_CHECK=0 early-exit check as a
+ * separate launch; QCLDPC_CAND_PER_SM=k grid of that launch; QCLDPC_PACK=0 no lane packing and QCLDPC_FV=1|2 frames
+ * per thread in the generic pass.  None of them changes any result.
  */
 int qcldpc_code_create(const int32_t* base_shifts, int mb, int nb, int Z, qcldpc_code_t** out_code);
 void qcldpc_code_destroy(qcldpc_code_t* code);
@@ -70,8 +81,9 @@ int qcldpc_code_info(const qcldpc_code_t* code, int64_t* n, int64_t* m, int64_t*
 size_t qcldpc_workspace_bytes(const qcldpc_code_t* code, int n_frames);
 
 /*
- * Decode n_frames independent frames (Algorithm 1, syndrome form).  Only ENQUEUES work on `stream`; never
- * synchronises the device; allocates nothing.  All d_* are DEVICE pointers owned by the caller, frame-major and
+ * Decode n_frames independent frames (Algorithm 1, syndrome form), 1 <= n_frames <= QCLDPC_MAX_FRAMES.
+ * Only ENQUEUES work on `stream`; never synchronises the device; allocates no device memory (the first call of a
+ * process on a device sets kernel attributes).  All d_* are DEVICE pointers owned by the caller, frame-major and
  * contiguous:
  *   d_llr        const float   [n_frames][n]  Q_v = ln P(x_v=0)/P(x_v=1)
  *   d_syndrome   const uint8_t [n_frames][m]  s_c in {0,1} (only bit 0 is read)
@@ -115,6 +127,11 @@ size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int 
 int qcldpc_decode_host(const qcldpc_code_t* code, const float* h_llr, const uint8_t* h_syndrome, int n_frames,
                        int max_iter, int early_stop, uint8_t* h_hard, int32_t* h_iters, uint8_t* h_pass,
                        float* h_posterior, void* d_workspace, size_t workspace_bytes, void* stream);
+/* qcldpc_decode_host with the early-termination scheduling of qcldpc_decode_ex (check_from_iter >= 1). */
+int qcldpc_decode_host_ex(const qcldpc_code_t* code, const float* h_llr, const uint8_t* h_syndrome, int n_frames,
+                          int max_iter, int early_stop, int check_from_iter, uint8_t* h_hard, int32_t* h_iters,
+                          uint8_t* h_pass, float* h_posterior, void* d_workspace, size_t workspace_bytes,
+                          void* stream);
 
 /* Number of kernel launches the last qcldpc_decode / qcldpc_decode_host call of this thread enqueued. */
 int64_t qcldpc_last_launch_count(void);
@@ -126,7 +143,8 @@ int64_t qcldpc_last_launch_count(void);
  * early-exit check k_cand); stride = 0 switches it off.  qcldpc_profile_collect waits for the recorded events (host
  * blocks until they have completed), returns for each kind the summed duration in ms of the timed launches, how many
  * were timed and how many were launched since enable/collect, and clears the record.  ms_sum, timed, launched:
- * HOST arrays of 2 entries.
+ * HOST arrays of 2 entries.  The events live in a per-thread pool that grows on demand while profiling is on (the one
+ * place where a decode call creates CUDA objects) and is destroyed by qcldpc_profile_enable(0).
  */
 int qcldpc_profile_enable(int stride);
 int qcldpc_profile_collect(double* ms_sum, int64_t* timed, int64_t* launched);

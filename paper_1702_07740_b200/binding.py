@@ -18,7 +18,7 @@ SO_PATH = os.path.join(_HERE, "csrc", "libqcldpc.so")
 EXPORTED_SYMBOLS = (
     "qcldpc_code_create", "qcldpc_code_create_sparse", "qcldpc_code_destroy", "qcldpc_code_info", "qcldpc_workspace_bytes", "qcldpc_decode",
     "qcldpc_decode_ex",
-    "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_last_launch_count", "qcldpc_status_string",
+    "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_decode_host_ex", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
 )
 
@@ -48,6 +48,8 @@ _lib.qcldpc_decode_ex.restype = _i
 _lib.qcldpc_decode_ex.argtypes = [_vp, _vp, _vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.qcldpc_decode_host.restype = _i
 _lib.qcldpc_decode_host.argtypes = _DECODE_ARGS
+_lib.qcldpc_decode_host_ex.restype = _i
+_lib.qcldpc_decode_host_ex.argtypes = _lib.qcldpc_decode_ex.argtypes
 _lib.qcldpc_last_launch_count.restype = ctypes.c_int64
 _lib.qcldpc_last_launch_count.argtypes = []
 _lib.qcldpc_profile_enable.restype = _i
@@ -95,6 +97,38 @@ def qcldpc_profile_collect():
     return {name: (ms[k], timed[k], launched[k]) for k, name in enumerate(("pass", "cand"))}
 
 
+def _check_host_array(a, name, np_dtype, torch):
+    """A HOST array the C ABI can read as it is: right dtype, C-contiguous, not a device tensor."""
+    if isinstance(a, torch.Tensor):
+        want = {np.float32: torch.float32, np.uint8: torch.uint8, np.int32: torch.int32}[np_dtype]
+        if a.is_cuda or a.dtype != want or not a.is_contiguous():
+            raise ValueError(f"{name}: need a contiguous host tensor of dtype {want}, got {a.dtype} on {a.device}")
+    elif isinstance(a, np.ndarray):
+        if a.dtype != np_dtype or not a.flags["C_CONTIGUOUS"]:
+            raise ValueError(f"{name}: need a C-contiguous numpy array of dtype {np.dtype(np_dtype)}, got {a.dtype}")
+    else:
+        raise ValueError(f"{name}: need a numpy array or a host torch tensor")
+
+
+def _check_outputs(out, F, n, torch, cuda: bool):
+    """Caller-provided output buffers: shapes, dtypes, contiguity, residency."""
+    spec = (("hard", (F, n), np.uint8), ("iters", (F,), np.int32), ("passed", (F,), np.uint8),
+            ("posterior", (F, n), np.float32))
+    for (name, shape, dt), a in zip(spec, out):
+        if a is None:
+            if name != "posterior":
+                raise ValueError(f"out.{name} is missing")
+            continue
+        if tuple(a.shape) != shape:
+            raise ValueError(f"out.{name}: shape {tuple(a.shape)}, need {shape}")
+        if cuda:
+            want = {np.float32: torch.float32, np.uint8: torch.uint8, np.int32: torch.int32}[dt]
+            if not (isinstance(a, torch.Tensor) and a.is_cuda and a.dtype == want and a.is_contiguous()):
+                raise ValueError(f"out.{name}: need a contiguous CUDA tensor of dtype {want}")
+        else:
+            _check_host_array(a, f"out.{name}", dt, torch)
+
+
 class DecodeResult(NamedTuple):
     hard: "object"        # uint8  [F][n]
     iters: "object"       # int32  [F]
@@ -115,6 +149,19 @@ class QCLDPCCode:
         _check(_lib.qcldpc_code_create(base.ctypes.data, self.mb, self.nb, self.Z, ctypes.byref(self._handle)),
                "qcldpc_code_create")
         self._read_info()
+        self._device = self._current_device()
+
+    @staticmethod
+    def _current_device():
+        """The CUDA device the handle's tables were allocated on (the one current at creation)."""
+        import torch
+        return torch.device("cuda", torch.cuda.current_device())
+
+    def _require_device(self, dev):
+        import torch
+        dev = torch.device(dev)
+        if dev.type != "cuda" or (dev.index if dev.index is not None else torch.cuda.current_device()) != self._device.index:
+            raise ValueError(f"this code handle lives on {self._device}; got buffers on {dev}")
 
     def _read_info(self):
         n, m, e = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
@@ -136,6 +183,7 @@ class QCLDPCCode:
         _check(_lib.qcldpc_code_create_sparse(r.ctypes.data, c.ctypes.data, p.ctypes.data, len(r), self.mb, self.nb,
                                               self.Z, ctypes.byref(self._handle)), "qcldpc_code_create_sparse")
         self._read_info()
+        self._device = self._current_device()
         return self
 
     def __del__(self):
@@ -169,15 +217,29 @@ class QCLDPCCode:
             raise ValueError(f"shapes {tuple(llr.shape)} / {tuple(syndrome.shape)} do not match n={self.n}, m={self.m}")
         F = llr.shape[0]
         dev = llr.device
+        self._require_device(dev)
+        if syndrome.device != dev:
+            raise ValueError("llr and syndrome must live on one device")
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
         need = self.workspace_bytes(F)
+        own = []                                        # tensors allocated here and used on `st`
         if workspace is None:
             workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+            own.append(workspace)
+        else:
+            self._require_device(workspace.device)
         if out is None:
             out = DecodeResult(torch.empty((F, self.n), dtype=torch.uint8, device=dev),
                                torch.empty(F, dtype=torch.int32, device=dev),
                                torch.empty(F, dtype=torch.uint8, device=dev),
                                torch.empty((F, self.n), dtype=torch.float32, device=dev) if want_posterior else None)
-        st = stream if stream is not None else torch.cuda.current_stream(dev)
+            own.extend(t for t in out if t is not None)
+        else:
+            _check_outputs(out, F, self.n, torch, cuda=True)
+        # the call only enqueues: tell the caching allocator that these blocks are in use on `st`, so that a block
+        # dropped by the caller (the internal workspace on return) is not handed out again before the decode has run
+        for t in own + [llr, syndrome]:
+            t.record_stream(st)
         with torch.cuda.device(dev):
             rc = _lib.qcldpc_decode_ex(self._handle, llr.data_ptr(), syndrome.data_ptr(), F, int(max_iter),
                                        int(early_stop), int(check_from_iter), out.hard.data_ptr(),
@@ -188,8 +250,9 @@ class QCLDPCCode:
         return out
 
     def decode_host(self, llr: np.ndarray, syndrome: np.ndarray, max_iter: int, early_stop: int,
-                    want_posterior: bool = False, workspace=None, out=None, stream=None):
-        """qcldpc_decode_host on HOST arrays (numpy or pinned torch CPU tensors); returns host outputs.
+                    want_posterior: bool = False, workspace=None, out=None, stream=None, check_from_iter: int = 1):
+        """qcldpc_decode_host_ex on HOST arrays (numpy or pinned torch CPU tensors; float32 / uint8, C-contiguous);
+        returns host outputs.
 
         Host<->device copies happen inside the call; it returns after the stream has drained."""
         import torch
@@ -197,23 +260,28 @@ class QCLDPCCode:
         def ptr(a):
             return a.data_ptr() if isinstance(a, torch.Tensor) else a.ctypes.data
 
+        _check_host_array(llr, "llr", np.float32, torch)
+        _check_host_array(syndrome, "syndrome", np.uint8, torch)
         F = llr.shape[0]
         if tuple(llr.shape) != (F, self.n) or tuple(syndrome.shape) != (F, self.m):
             raise ValueError("bad host shapes")
         need = self.host_workspace_bytes(F, want_posterior)
         if workspace is None:
-            workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+            workspace = torch.empty(need, dtype=torch.uint8, device=self._device)
+        self._require_device(workspace.device)
         if out is None:
             out = DecodeResult(np.empty((F, self.n), dtype=np.uint8), np.empty(F, dtype=np.int32),
                                np.empty(F, dtype=np.uint8),
                                np.empty((F, self.n), dtype=np.float32) if want_posterior else None)
+        else:
+            _check_outputs(out, F, self.n, torch, cuda=False)
         st = stream if stream is not None else torch.cuda.current_stream(workspace.device)
         with torch.cuda.device(workspace.device):
-            rc = _lib.qcldpc_decode_host(self._handle, ptr(llr), ptr(syndrome), F, int(max_iter), int(early_stop),
-                                         ptr(out.hard), ptr(out.iters), ptr(out.passed),
-                                         ptr(out.posterior) if out.posterior is not None else None,
-                                         workspace.data_ptr(), workspace.numel(), st.cuda_stream)
-        _check(rc, "qcldpc_decode_host")
+            rc = _lib.qcldpc_decode_host_ex(self._handle, ptr(llr), ptr(syndrome), F, int(max_iter), int(early_stop),
+                                            int(check_from_iter), ptr(out.hard), ptr(out.iters), ptr(out.passed),
+                                            ptr(out.posterior) if out.posterior is not None else None,
+                                            workspace.data_ptr(), workspace.numel(), st.cuda_stream)
+        _check(rc, "qcldpc_decode_host_ex")
         return out
 
 

@@ -97,6 +97,8 @@ struct PassLaunch {
     const void* check_args;    //       (exact families; NULL: none)
     int n_cols, n_frames, max_np, max_dv;
     int n_sm;                  // multiprocessors of the device
+    int fv;                    // generic pass: frames per thread (1 or 2)
+    int pack_ok;               // generic pass: lane packing allowed
 };
 using PassLauncher = void (*)(const PassLaunch&);
 using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only

@@ -31,18 +31,19 @@ __global__ void __launch_bounds__(kThreads, V == 1 ? 7 : 4) k_pass_exact(const _
     const int i0 = blockIdx.x * (kThreads * V);
 
     // preamble: window starts of this tile as byte offsets, one thread per stream
-    __shared__ int2 s_eo[DV];
-    __shared__ int s_po[NGS * PCAP];
+    // byte offsets are formed in UNSIGNED arithmetic: a frame's runs stay below 2^30 floats (qcldpc_code_create)
+    __shared__ uint2 s_eo[DV];
+    __shared__ unsigned s_po[NGS * PCAP];
     static_assert(DV <= kThreads && NGS * PCAP <= kThreads, "one preamble thread per stream");
     if (tid < DV) {
         int r0 = i0 - cd.shift[tid]; r0 += (r0 < 0) ? Z : 0;  // check index of the tile's first variable
         int x = i0 + cd.delta[tid]; x -= (x >= Z) ? Z : 0;
-        s_eo[tid] = make_int2(4 * (cd.p_off[tid] + x), 4 * (cd.t_off[tid] + r0));
+        s_eo[tid] = make_uint2(4u * (unsigned)(cd.p_off[tid] + x), 4u * (unsigned)(cd.t_off[tid] + r0));
     }
     if (NG > 0 && tid >= kThreads - NG * PCAP) {             // slot (g, j): partner j of gen edge g, or -1
         const int sl = tid - (kThreads - NG * PCAP);
         int x = i0 + cd.g_delta[sl]; x -= (x >= Z) ? Z : 0;
-        s_po[sl] = cd.g_off[sl] >= 0 ? 4 * (cd.g_off[sl] + x) : -1;
+        s_po[sl] = cd.g_off[sl] >= 0 ? 4u * (unsigned)(cd.g_off[sl] + x) : 0xffffffffu;   // no partner in this slot
     }
     pdl_wait();                                              // from here on: memory the previous launch wrote
     int in_buf;
@@ -75,16 +76,16 @@ __global__ void __launch_bounds__(kThreads, V == 1 ? 7 : 4) k_pass_exact(const _
     for (int g = 0; g < NG; ++g) {
 #pragma unroll
         for (int j = 0; j < PCAP; ++j) {
-            const int po = s_po[g * PCAP + j];               // -1: the row has fewer partners
+            const unsigned po = s_po[g * PCAP + j];          // 0xffffffff: the row has fewer partners
 #pragma unroll
             for (int v = 0; v < V; ++v)
-                pw[g][j][v] = (po != -1) ? __ldg(byte_ptr(qP, po) + v * kThreads) : 0.0f;
+                pw[g][j][v] = (po != 0xffffffffu) ? __ldg(byte_ptr(qP, po) + v * kThreads) : 0.0f;
         }
     }
     float tv[DV][V], wv[DV][V];
 #pragma unroll
     for (int k = 0; k < DV; ++k) {
-        const int2 o = s_eo[k];
+        const uint2 o = s_eo[k];
 #pragma unroll
         for (int v = 0; v < V; ++v) tv[k][v] = __ldg(byte_ptr(tP, o.y) + v * kThreads);
         if (k >= NG) {

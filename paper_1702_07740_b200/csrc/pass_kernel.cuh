@@ -26,7 +26,6 @@
 #include "common.cuh"
 
 #include <algorithm>
-#include <cstdlib>
 
 namespace qc {
 
@@ -453,15 +452,10 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
     else launch_pdl(k_pass<TB, G, FV, false, PACK>, grid, block, smem, L.stream, L.tab, args, ctab, chk);
 }
 
-inline int pass_any_fv(int n_frames) {                      // frames per thread; QCLDPC_FV=1|2 overrides (tuning knob)
-    if (const char* e = getenv("QCLDPC_FV")) { if (atoi(e) == 1 || atoi(e) == 2) return atoi(e); }
-    return n_frames >= 4 ? 2 : 1;
-}
-
 template <int TB>
 inline void launch_pass_z(const PassLaunch& L, const PassArgs& args) {
     const bool split = L.max_dv > 2 * kChunk;               // long columns: four edge groups per variable
-    const bool pair = pass_any_fv(L.n_frames) == 2;         // batched: two frames per thread
+    const bool pair = L.fv == 2;                            // batched: two frames per thread
     const bool pack = args.pack > 1;                        // several frames side by side in a tile
     if (split) {
         if (pair) { if (pack) launch_pass_tb<TB, 4, 2, true>(L, args); else launch_pass_tb<TB, 4, 2, false>(L, args); }
@@ -477,7 +471,7 @@ inline void launch_pass_any(const PassLaunch& L) {
     args.table_bytes = (int)pass_any_table_bytes(L.max_np);
     // tile width: the one whose lanes are best used, frames packed side by side where the circulant is at most half a
     // tile (kernel header); ties go to the narrower tile
-    const int Z = args.Z, fv = pass_any_fv(L.n_frames);
+    const int Z = args.Z, fv = L.fv;
     const int rows = (L.n_frames + fv - 1) / fv;            // frames (or frame pairs) there are to pack
     int best_tb = 128, best_pack = 1;
     double best_use = -1.0;
@@ -490,7 +484,7 @@ inline void launch_pass_any(const PassLaunch& L) {
         const double use = (double)pack * Z / ((double)tiles * tb);
         if (use > best_use + 1e-9) { best_use = use; best_tb = tb; best_pack = pack; }
     }
-    if (const char* pk = getenv("QCLDPC_PACK")) { if (atoi(pk) == 0) { best_pack = 1; best_tb = Z <= 32 ? 32 : Z <= 64 ? 64 : 128; } }
+    if (!L.pack_ok) { best_pack = 1; best_tb = Z <= 32 ? 32 : Z <= 64 ? 64 : 128; }
     args.pack = best_pack;
     if (best_tb == 32) launch_pass_z<32>(L, args);
     else if (best_tb == 64) launch_pass_z<64>(L, args);

@@ -63,6 +63,22 @@ thread_local Profile g_prof;
 
 }  // namespace
 
+// Tuning knobs (defaults are the measured best).  Part of the immutable handle: the decode calls read no
+// environment variable and keep no state outside the handle and the caller's workspace.
+struct Tuning {
+    int V = 0;                            // QCLDPC_V=1|2: variables per thread of k_pass_exact (0: by grid size)
+    int flip = 1;                         // QCLDPC_FLIP=0: every launch walks the frames forwards
+    int merge_check = 1;                  // QCLDPC_MERGE_CHECK=0: the early-exit check is a separate k_cand launch
+    int cand_per_sm = 0;                  // QCLDPC_CAND_PER_SM=k: grid of a separate k_cand launch (0: by batch size)
+    int pack = 1;                         // QCLDPC_PACK=0: no lane packing in the generic pass
+    int fv = 0;                           // QCLDPC_FV=1|2: frames per thread of the generic pass (0: by batch size)
+};
+
+static int env_int(const char* name, int dflt) {
+    const char* e = getenv(name);
+    return (e && *e) ? atoi(e) : dflt;
+}
+
 struct qcldpc_code {
     int mb, nb, Z, Zs, tiles;             // tiles = ceil(Z / kThreads)
     int halo = 0, max_np = 0;             // halo: runs are followed by kHalo wrapped entries (exact families)
@@ -80,6 +96,7 @@ struct qcldpc_code {
     PassLauncher launcher = nullptr;
     std::vector<char> exact;              // kernel-parameter table of the exact family (empty: generic kernel)
     int n_sm = 148;
+    Tuning tune;                          // read ONCE from the environment by qcldpc_code_create (include/qcldpc.h)
 };
 
 namespace {
@@ -430,6 +447,17 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         fill(ht, code->exact.data());
     }
     code->tiles = (Z + kThreads - 1) / kThreads;
+    {
+        Tuning& tn = code->tune;
+        const int v = env_int("QCLDPC_V", 0);
+        tn.V = (v == 1 || v == 2) ? v : 0;
+        tn.flip = env_int("QCLDPC_FLIP", 1) != 0;
+        tn.merge_check = env_int("QCLDPC_MERGE_CHECK", 1) != 0;
+        tn.cand_per_sm = std::max(0, env_int("QCLDPC_CAND_PER_SM", 0));
+        tn.pack = env_int("QCLDPC_PACK", 1) != 0;
+        const int fv = env_int("QCLDPC_FV", 0);
+        tn.fv = (fv == 1 || fv == 2) ? fv : 0;
+    }
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
         const size_t bytes = std::max<size_t>(vec.size(), 1) * sizeof(vec[0]);
@@ -502,7 +530,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     g_launches = 0;
     if (check_from_iter < 1) return QCLDPC_ERR_BAD_ARGUMENT;
     if (!code || !d_llr || !d_syndrome || !d_hard || !d_iters || !d_pass) return QCLDPC_ERR_BAD_ARGUMENT;
-    if (n_frames <= 0 || n_frames > 65535 || max_iter < 0) return QCLDPC_ERR_BAD_ARGUMENT;
+    if (n_frames <= 0 || n_frames > QCLDPC_MAX_FRAMES || max_iter < 0) return QCLDPC_ERR_BAD_ARGUMENT;
     if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255) ||
         workspace_bytes < qcldpc_workspace_bytes(code, n_frames))
         return QCLDPC_ERR_WORKSPACE;
@@ -528,30 +556,28 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     ++g_launches;
 
     // exact families: two variables per thread (1 KB windows) once the grid still fills the chip several times over;
-    // small batches keep one variable per thread (more CTAs in flight).  QCLDPC_V=1|2 overrides (tuning knob).
+    // small batches keep one variable per thread (more CTAs in flight).  Tuning::V overrides.
     int V = 1;
     if (!code->exact.empty()) {
         const int64_t ctas_v2 = (int64_t)((Z + 2 * kThreads - 1) / (2 * kThreads)) * code->n_act_cols * n_frames;
         if (ctas_v2 >= (int64_t)4 * 8 * code->n_sm) V = 2;
-        const char* v = getenv("QCLDPC_V");
-        if (v && (atoi(v) == 1 || atoi(v) == 2)) V = atoi(v);
+        if (code->tune.V) V = code->tune.V;
     }
-    const char* fl = getenv("QCLDPC_FLIP");                // tuning knob: 0 = every launch walks the frames forwards
-    const bool flip_frames = !(fl && atoi(fl) == 0);
+    const bool flip_frames = code->tune.flip != 0;
+    const int fv = code->tune.fv ? code->tune.fv : (n_frames >= 4 ? 2 : 1);   // generic pass: frames per thread
     PassLaunch pl{ptab,
                   PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
                            w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
                   st, V, false,
                   code->exact.empty() ? nullptr : code->exact.data(), nullptr, nullptr, code->n_act_cols, n_frames,
-                  code->max_np, code->max_dv, code->n_sm};
+                  code->max_np, code->max_dv, code->n_sm, fv, code->tune.pack};
     CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
                  {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
                  d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
                  n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
     // early-exit grid: persistent; small batches are launch-bound and almost never have a candidate, so a smaller grid
     // (less to schedule and retire between two passes) wins there
-    const char* cb = getenv("QCLDPC_CAND_PER_SM");
-    const int cand_per_sm = cb ? std::max(1, atoi(cb)) : (n_frames <= 8 ? 1 : 4);
+    const int cand_per_sm = code->tune.cand_per_sm ? code->tune.cand_per_sm : (n_frames <= 8 ? 1 : 4);
     const int cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * tiles1));
 
     // Launch t = pass t, then the early-exit check of iteration t-2 (check.cuh explains the lag): the check reads the
@@ -572,8 +598,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     // the check is launched for iterations T >= check_from_iter - 2: the filter slot of iteration I is dirty from pass
     // I-2 and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
     auto check_wanted = [&](int T) { return early_stop && T >= 1 && T >= check_from_iter - 2; };
-    const char* mc = getenv("QCLDPC_MERGE_CHECK");        // tuning knob: 0 = always a separate k_cand launch
-    const bool merge_check = !(mc && atoi(mc) == 0);
+    const bool merge_check = code->tune.merge_check != 0;
     pl.check_tab = nullptr; pl.check_args = nullptr;
     int t_last = 0;                                      // last launch issued
     for (int t = 1; t <= max_iter; ++t) {
@@ -641,9 +666,18 @@ size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int 
 int qcldpc_decode_host(const qcldpc_code_t* code, const float* h_llr, const uint8_t* h_syndrome, int n_frames,
                        int max_iter, int early_stop, uint8_t* h_hard, int32_t* h_iters, uint8_t* h_pass,
                        float* h_posterior, void* d_workspace, size_t workspace_bytes, void* stream) {
+    return qcldpc_decode_host_ex(code, h_llr, h_syndrome, n_frames, max_iter, early_stop, 1, h_hard, h_iters, h_pass,
+                                 h_posterior, d_workspace, workspace_bytes, stream);
+}
+
+int qcldpc_decode_host_ex(const qcldpc_code_t* code, const float* h_llr, const uint8_t* h_syndrome, int n_frames,
+                          int max_iter, int early_stop, int check_from_iter, uint8_t* h_hard, int32_t* h_iters,
+                          uint8_t* h_pass, float* h_posterior, void* d_workspace, size_t workspace_bytes,
+                          void* stream) {
     g_launches = 0;
     if (!code || !h_llr || !h_syndrome || !h_hard || !h_iters || !h_pass) return QCLDPC_ERR_BAD_ARGUMENT;
-    if (n_frames <= 0 || max_iter < 0) return QCLDPC_ERR_BAD_ARGUMENT;
+    if (n_frames <= 0 || n_frames > QCLDPC_MAX_FRAMES || max_iter < 0 || check_from_iter < 1)
+        return QCLDPC_ERR_BAD_ARGUMENT;
     if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255) ||
         workspace_bytes < qcldpc_host_workspace_bytes(code, n_frames, h_posterior != nullptr))
         return QCLDPC_ERR_WORKSPACE;
@@ -662,8 +696,8 @@ int qcldpc_decode_host(const qcldpc_code_t* code, const float* h_llr, const uint
     if (h_posterior) { d_post = reinterpret_cast<float*>(p + off); off += align_up(llr_b, 256); }
     CUDA_TRY(cudaMemcpyAsync(d_llr, h_llr, llr_b, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_syn, h_syndrome, syn_b, cudaMemcpyHostToDevice, st));
-    const int rc = decode_impl(code, d_llr, d_syn, n_frames, max_iter, early_stop, 1, d_hard, d_iters, d_pass, d_post,
-                               d_workspace, core, stream, true);
+    const int rc = decode_impl(code, d_llr, d_syn, n_frames, max_iter, early_stop, check_from_iter, d_hard, d_iters,
+                               d_pass, d_post, d_workspace, core, stream, true);
     if (rc != QCLDPC_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(h_hard, d_hard, hard_b, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(h_iters, d_iters, (size_t)n_frames * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -680,6 +714,11 @@ int qcldpc_profile_enable(int stride) {
     g_prof.stride = stride;
     g_prof.kind.clear();
     g_prof.launched[0] = g_prof.launched[1] = 0;
+    if (stride == 0) {                                     // switching it off releases the event pool
+        for (cudaEvent_t ev : g_prof.pool) cudaEventDestroy(ev);
+        g_prof.pool.clear();
+        g_prof.pool.shrink_to_fit();
+    }
     return QCLDPC_OK;
 }
 
@@ -703,7 +742,8 @@ const char* qcldpc_status_string(int status) {
     switch (status) {
         case QCLDPC_OK: return "ok";
         case QCLDPC_ERR_BAD_ARGUMENT: return "bad argument";
-        case QCLDPC_ERR_UNSUPPORTED: return "unsupported code (active column degree > 64 or size out of range)";
+        case QCLDPC_ERR_UNSUPPORTED:
+            return "unsupported code (active column degree > 64, gen-row partner table or size out of range)";
         case QCLDPC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case QCLDPC_ERR_CUDA: return "CUDA runtime error";
         case QCLDPC_ERR_ALLOC: return "host allocation failed";
