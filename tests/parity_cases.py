@@ -1,0 +1,150 @@
+"""Comparison routines shared by the GPU parity tests (tests/test_gpu_parity.py) and the parity report
+(tests/parity_report.py).  Expected values come from `oracle/` only; the CUDA path is called through the C ABI binding.
+
+Bar (BASELINE.json north_star): fixed iteration count, early stop off:
+    |L_gpu - L_oracle| <= TOL * max(1, |L_oracle|)  for every variable,     TOL = 1e-3
+    hard bits identical wherever |L_oracle| > HARD_MIN,                     HARD_MIN = 1e-2
+early stop on: per-frame pass flags and iteration counts against the oracle on the same inputs.
+
+fp32 floor: the oracle's float instantiation (the same text with REAL = float) against
+its double instantiation on the same inputs measures what ANY fp32 evaluation of the iteration loses.  A frame is
+UNPINNED only where that floor itself leaves half the tolerance (floor > TOL / 2): there a comparison with the fp64
+oracle cannot separate kernel error from fp32 rounding; the GPU deviation must then stay within UNPINNED_FACTOR x the
+floor, and the frame is reported.  Everywhere else the stated tolerance is asserted as it stands.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import List, Optional
+
+import numpy as np
+
+from paper_1702_07740_b200 import workloads as W
+
+TOL = 1e-3
+HARD_MIN = 1e-2
+UNPINNED_AT = TOL / 2          # "if oracle32 itself leaves the tolerance" -- taken at half of it
+UNPINNED_FACTOR = 4.0          # GPU deviation allowed on an unpinned frame, in units of the measured floor
+HARD_PINNED_ERR = HARD_MIN / 2  # below this deviation the hard bits with |L| > HARD_MIN are asserted, above it (only possible on
+                               # an unpinned frame) the mismatch count is reported
+
+
+def rel_err(post, post_ref):
+    return np.abs(post.astype(np.float64) - post_ref) / np.maximum(1.0, np.abs(post_ref))
+
+
+@dataclass
+class FrameParity:
+    frame: int
+    err: float                 # max_v |L_gpu - L_64| / max(1, |L_64|)
+    floor: Optional[float]     # the same for the oracle's float instantiation (None: not needed, err <= TOL / 2)
+    decided: int               # variables with |L_64| > HARD_MIN
+    hard_mismatch: int         # of those, hard bits that differ
+    unpinned: bool
+
+    @property
+    def ok(self) -> bool:
+        bound = max(TOL, UNPINNED_FACTOR * self.floor) if self.unpinned else TOL
+        hard_ok = self.hard_mismatch == 0 or self.err > HARD_PINNED_ERR
+        return self.err <= bound and hard_ok
+
+
+@dataclass
+class CaseParity:
+    label: str
+    n_iter: int
+    frames: List[FrameParity] = field(default_factory=list)
+
+    @property
+    def ok(self) -> bool:
+        return all(f.ok for f in self.frames)
+
+    def failures(self) -> str:
+        return "; ".join(f"frame {f.frame}: err {f.err:.3e} floor {f.floor if f.floor is None else f'{f.floor:.2e}'} "
+                         f"hard mismatches {f.hard_mismatch}" for f in self.frames if not f.ok)
+
+
+def gpu_decode(B, code_or_base, Z, llr, syn, max_iter, early_stop, want_posterior=True, check_from_iter=1):
+    """(hard, iters, passed, posterior) as numpy arrays; code_or_base is a base matrix or a ready QCLDPCCode."""
+    import torch
+    code = code_or_base if hasattr(code_or_base, "decode") else B.QCLDPCCode(code_or_base, Z)
+    d_llr = torch.from_numpy(np.ascontiguousarray(llr, dtype=np.float32)).cuda()
+    d_syn = torch.from_numpy(np.ascontiguousarray(syn, dtype=np.uint8)).cuda()
+    out = code.decode(d_llr, d_syn, max_iter, early_stop, want_posterior=want_posterior,
+                      check_from_iter=check_from_iter)
+    torch.cuda.synchronize()
+    post = out.posterior.cpu().numpy() if out.posterior is not None else None
+    return out.hard.cpu().numpy(), out.iters.cpu().numpy(), out.passed.cpu().numpy(), post
+
+
+def compare_fixed(oracle_lib, base, Z, llr, syn, n_iter, label, hard, post, always_floor=False,
+                  frame_ids=None) -> CaseParity:
+    """GPU outputs (hard, post) of a fixed-count decode against the oracle on the same inputs.  The float
+    instantiation runs only for the frames that need it (err > TOL / 2) unless always_floor."""
+    ref = oracle_lib.decode(base, Z, llr, syn, n_iter, 0)
+    err = rel_err(post, ref.posterior).max(axis=1)
+    need = np.nonzero((err > UNPINNED_AT) | always_floor)[0]
+    floor = np.full(len(err), np.nan)
+    if len(need):
+        ref32 = oracle_lib.decode(base, Z, llr[need], syn[need], n_iter, 0, precision=32)
+        floor[need] = rel_err(ref32.posterior, ref.posterior[need]).max(axis=1)
+    case = CaseParity(label, n_iter)
+    for f in range(len(err)):
+        decided = np.abs(ref.posterior[f]) > HARD_MIN
+        mism = int((hard[f][decided] != ref.hard[f][decided]).sum())
+        fl = None if np.isnan(floor[f]) else float(floor[f])
+        unpinned = fl is not None and fl > UNPINNED_AT
+        case.frames.append(FrameParity(int(frame_ids[f]) if frame_ids is not None else f, float(err[f]), fl,
+                                       int(decided.sum()), mism, unpinned))
+    return case
+
+
+def run_fixed(oracle_lib, B, base, Z, llr, syn, n_iter, label, always_floor=False) -> CaseParity:
+    hard, iters, passed, post = gpu_decode(B, base, Z, llr, syn, n_iter, 0)
+    assert np.isfinite(post).all(), f"{label}: non-finite posterior"
+    assert (iters == n_iter).all(), f"{label}: iteration counts {iters} with early stop off"
+    s_gpu = W.syndrome_of(base, Z, hard)
+    assert (passed.astype(bool) == (s_gpu == syn).all(axis=1)).all(), f"{label}: pass flag does not describe the GPU's own decisions"
+    return compare_fixed(oracle_lib, base, Z, llr, syn, n_iter, label, hard, post, always_floor)
+
+
+@dataclass
+class StopParity:
+    label: str
+    n_frames: int
+    gpu_pass: int
+    oracle_pass: int
+    discordant_pass: int                      # frames whose pass flags differ
+    discordant_iters: int                     # frames whose iteration counts differ
+    diff_hist: dict                           # iters_gpu - iters_oracle -> count
+    hard_mismatch_frames: int                 # frames passed on both sides whose words differ
+    gpu_words_valid: bool                     # every word the GPU reports as passed satisfies H x = s
+
+    @property
+    def fer_gpu(self) -> float:
+        return 1.0 - self.gpu_pass / self.n_frames
+
+    @property
+    def fer_oracle(self) -> float:
+        return 1.0 - self.oracle_pass / self.n_frames
+
+
+def binomial_band_95(n: int, p_hat: float):
+    """Two-sided 95 % Clopper-Pearson interval of a binomial proportion observed as p_hat over n trials."""
+    from scipy.stats import beta
+    k = round(p_hat * n)
+    lo = 0.0 if k == 0 else float(beta.ppf(0.025, k, n - k + 1))
+    hi = 1.0 if k == n else float(beta.ppf(0.975, k + 1, n - k))
+    return lo, hi
+
+
+def compare_stop(oracle_lib, base, Z, llr, syn, max_iter, label, hard, iters, passed, syndrome_of=None) -> StopParity:
+    ref = oracle_lib.decode(base, Z, llr, syn, max_iter, 1)
+    diff = iters.astype(np.int64) - ref.iters.astype(np.int64)
+    vals, counts = np.unique(diff, return_counts=True)
+    both = passed.astype(bool) & ref.passed.astype(bool)
+    words_bad = int((hard[both] != ref.hard[both]).any(axis=1).sum()) if both.any() else 0
+    ok = passed.astype(bool)
+    valid = bool((W.syndrome_of(base, Z, hard[ok]) == syn[ok]).all()) if ok.any() else True
+    return StopParity(label, len(iters), int(passed.sum()), int(ref.passed.sum()), int((passed != ref.passed).sum()),
+                      int((diff != 0).sum()), {int(v): int(c) for v, c in zip(vals, counts)}, words_bad, valid)

@@ -8,12 +8,12 @@ early stop on: per-frame pass flags and iteration counts agree with the oracle (
 on the same inputs, so the comparison is per frame).
 
 fp32 noise floor: flooding BP on a frame that does not converge is a chaotic
-map; 1-ulp differences grow ~1.2x per iteration (config 1, frames 1 and 2: 1e-6 at iteration 5, 1e-4..1e-3 at
-iteration 50 for ANY fp32 evaluation, including the oracle's own float instantiation).  The oracle's float
-instantiation (same text, REAL = float) measures that floor on the same inputs.  Where the floor itself exceeds a
-tenth of the tolerance, the comparison with the fp64 oracle is unpinned by construction (the deviation is a property
-of fp32, not of the kernel): there the test prints both numbers and requires the GPU deviation to stay within
-16x the floor.  Everywhere else the stated tolerance is asserted as is.
+map; 1-ulp differences grow ~1.2x per iteration for ANY fp32 evaluation, including the oracle's own float
+instantiation, which measures that floor on the same inputs.  A frame is UNPINNED only where the floor itself exceeds
+HALF the tolerance (tests/parity_cases.py); there the GPU deviation must stay within UNPINNED_FACTOR x the floor and the
+frame is printed.  Everywhere else the stated tolerance is asserted as it stands.  profiles/r02_parity_report.md
+(written on the B200 by tests/parity_report.py) records err, floor and hard-bit mismatches per config / frame /
+iteration count.
 """
 import numpy as np
 import pytest
@@ -24,9 +24,8 @@ torch = pytest.importorskip("torch")
 
 from paper_1702_07740_b200 import workloads as W  # noqa: E402
 from tests.helpers import bitwise_map_llr, dense_h, random_tree_code, tie_cases  # noqa: E402
-
-TOL = 1e-3
-HARD_MIN = 1e-2
+from tests import parity_cases as PC  # noqa: E402
+from tests.parity_cases import HARD_MIN, TOL, rel_err  # noqa: E402
 
 
 @pytest.fixture(scope="module")
@@ -38,42 +37,20 @@ def B():
 
 
 def gpu_decode(B, base, Z, llr, syn, max_iter, early_stop, want_posterior=True, check_from_iter=1):
-    code = B.QCLDPCCode(base, Z)
-    d_llr = torch.from_numpy(np.ascontiguousarray(llr, dtype=np.float32)).cuda()
-    d_syn = torch.from_numpy(np.ascontiguousarray(syn, dtype=np.uint8)).cuda()
-    out = code.decode(d_llr, d_syn, max_iter, early_stop, want_posterior=want_posterior,
-                      check_from_iter=check_from_iter)
-    torch.cuda.synchronize()
-    post = out.posterior.cpu().numpy() if out.posterior is not None else None
-    return out.hard.cpu().numpy(), out.iters.cpu().numpy(), out.passed.cpu().numpy(), post
-
-
-def rel_err(post_gpu, post_ref):
-    return np.abs(post_gpu.astype(np.float64) - post_ref) / np.maximum(1.0, np.abs(post_ref))
+    return PC.gpu_decode(B, base, Z, llr, syn, max_iter, early_stop, want_posterior, check_from_iter)
 
 
 def assert_parity(oracle_lib, B, base, Z, llr, syn, n_iter, label):
-    """Fixed iteration count, early stop off. Returns (max rel err per frame, fp32 floor per frame)."""
-    ref = oracle_lib.decode(base, Z, llr, syn, n_iter, 0)
-    ref32 = oracle_lib.decode(base, Z, llr, syn, n_iter, 0, precision=32)
-    hard, iters, passed, post = gpu_decode(B, base, Z, llr, syn, n_iter, 0)
-    assert np.isfinite(post).all()
-    err = rel_err(post, ref.posterior).max(axis=1)
-    floor = rel_err(ref32.posterior, ref.posterior).max(axis=1)
-    for f in range(len(err)):
-        if floor[f] <= TOL / 10:
-            assert err[f] <= TOL, f"{label}: frame {f} iter {n_iter}: err {err[f]:.3e} (fp32 floor {floor[f]:.1e})"
-        else:
-            print(f"{label}: frame {f} iter {n_iter}: UNPINNED (fp32 floor {floor[f]:.2e} > tol/10), gpu err {err[f]:.2e}")
-            assert err[f] <= max(TOL, 16 * floor[f]), f"{label}: frame {f}: err {err[f]:.3e} vs floor {floor[f]:.1e}"
-    decided = np.abs(ref.posterior) > HARD_MIN
-    pinned = (err <= HARD_MIN / 2)[:, None] & decided        # |dL| <= 5e-3 max(1,|L|) cannot flip a bit with |L| > 1e-2
-    assert (hard[pinned] == ref.hard[pinned]).all(), f"{label}: hard-bit mismatch where |L| > 1e-2"
-    np.testing.assert_array_equal(iters, n_iter)
-    # pass flag must describe the GPU's own decisions
-    s_gpu = W.syndrome_of(base, Z, hard)
-    np.testing.assert_array_equal(passed.astype(bool), (s_gpu == syn).all(axis=1))
-    return err, floor
+    """Fixed iteration count, early stop off (tests/parity_cases.py has the rule).  Returns (max rel err per frame,
+    fp32 floor per frame where it was needed, else nan)."""
+    case = PC.run_fixed(oracle_lib, B, base, Z, llr, syn, n_iter, label)
+    for f in case.frames:
+        if f.unpinned:
+            print(f"{label}: frame {f.frame} iter {n_iter}: UNPINNED (fp32 floor {f.floor:.2e} > tol/2), gpu err "
+                  f"{f.err:.2e}, hard-bit mismatches where |L| > 1e-2: {f.hard_mismatch} of {f.decided}")
+    assert case.ok, f"{label} iter {n_iter}: {case.failures()}"
+    return (np.array([f.err for f in case.frames]),
+            np.array([np.nan if f.floor is None else f.floor for f in case.frames]))
 
 
 # ------------------------------------------------------------------------------------------------ config 1 (full)
@@ -81,7 +58,7 @@ def assert_parity(oracle_lib, B, base, Z, llr, syn, n_iter, label):
 def test_config1_fixed_iterations(oracle_lib, B, n_iter):
     cfg, base, Z, fr = W.make_config(1)
     err, floor = assert_parity(oracle_lib, B, base, Z, fr.llr, fr.syndrome, n_iter, "cfg1")
-    print(f"cfg1 iter {n_iter}: max err {err.max():.2e}, median {np.median(err):.2e}, floor max {floor.max():.2e}")
+    print(f"cfg1 iter {n_iter}: max err {err.max():.2e}, median {np.median(err):.2e}, floor max {np.nanmax(floor) if np.isfinite(floor).any() else float('nan'):.2e}")
 
 
 def test_config1_early_stop_matches_oracle(oracle_lib, B):
@@ -118,7 +95,7 @@ def test_config1_check_from_iter_matches_oracle(oracle_lib, B, check_from):
 def test_reduced_configs_fixed_iterations(oracle_lib, B, cfg_index, Z, n_iter):
     cfg, base, Z, fr = W.make_config(cfg_index, Z=Z, n_frames=4)
     err, floor = assert_parity(oracle_lib, B, base, Z, fr.llr, fr.syndrome, n_iter, f"cfg{cfg_index}/Z{Z}")
-    print(f"cfg{cfg_index} Z={Z} iter {n_iter}: max err {err.max():.2e} floor {floor.max():.2e}")
+    print(f"cfg{cfg_index} Z={Z} iter {n_iter}: max err {err.max():.2e}")
 
 
 @pytest.mark.parametrize("cfg_index,snr_point,Z", [(5, 5, 2000), (5, 3, 2000), (3, 0, 500)])
@@ -136,12 +113,22 @@ def test_reduced_configs_early_stop(oracle_lib, B, cfg_index, snr_point, Z):
 
 
 # --------------------------------------------------------------------------------- full-size configs (n = 1e6)
-@pytest.mark.parametrize("cfg_index,n_iter", [(2, 25), (3, 25)])
+@pytest.mark.parametrize("cfg_index,n_iter", [(2, 50), (3, 50)])
 def test_full_size_single_frame(oracle_lib, B, cfg_index, n_iter):
+    """Configs 2 and 3 at full size, parity mode: 50 fixed iterations, early stop off."""
     cfg, base, Z, fr = W.make_config(cfg_index)
     assert fr.llr.shape == (1, 1000000)
     err, floor = assert_parity(oracle_lib, B, base, Z, fr.llr, fr.syndrome, n_iter, f"cfg{cfg_index}")
-    print(f"cfg{cfg_index} full size iter {n_iter}: max err {err.max():.2e} floor {floor.max():.2e}")
+    print(f"cfg{cfg_index} full size iter {n_iter}: max err {err.max():.2e}")
+
+
+@pytest.mark.parametrize("cfg_index,Z,n_iter", [(3, 1000, 200), (1, 32, 120)])
+def test_long_fixed_count(oracle_lib, B, cfg_index, Z, n_iter):
+    """Fixed-count posterior comparison well past 50 iterations (stalled frames of config 3's structure: errors do not
+    accumulate; config 1: converged frames settle, the chaotic ones are reported against their floor)."""
+    cfg, base, Z, fr = W.make_config(cfg_index, Z=Z, n_frames=4 if cfg_index != 1 else None)
+    err, floor = assert_parity(oracle_lib, B, base, Z, fr.llr, fr.syndrome, n_iter, f"cfg{cfg_index}/Z{Z}")
+    print(f"cfg{cfg_index} Z={Z} iter {n_iter}: max err {err.max():.2e}")
 
 
 def test_config4_batch_sampled_frames(oracle_lib, B):
@@ -157,28 +144,62 @@ def test_config4_batch_sampled_frames(oracle_lib, B):
     post = out.posterior.cpu().numpy()
     hard = out.hard.cpu().numpy()
     assert (out.iters.cpu().numpy() == n_iter).all() and (out.passed.cpu().numpy() == 0).all()
+    sample = np.array([0, 9, 18, 27, 37, 45, 54, 63])
+    ref = oracle_lib.decode(base, Z, fr.llr[sample], fr.syndrome[sample], n_iter, 1)
+    assert (ref.passed == 0).all() and (ref.iters == n_iter).all()
+    case = PC.compare_fixed(oracle_lib, base, Z, fr.llr[sample], fr.syndrome[sample], n_iter, "cfg4 batch",
+                            hard[sample], post[sample], frame_ids=sample)
+    assert case.ok and not any(f.unpinned for f in case.frames), case.failures()
+    print("cfg4 sampled frames: max err", max(f.err for f in case.frames))
     for f in (0, 37, 63):
-        ref = oracle_lib.decode(base, Z, fr.llr[f:f + 1], fr.syndrome[f:f + 1], n_iter, 1)
-        assert ref.passed[0] == 0 and ref.iters[0] == n_iter
-        e = rel_err(post[f:f + 1], ref.posterior).max()
-        assert e <= TOL, f"frame {f}: {e:.3e}"
-        decided = np.abs(ref.posterior[0]) > HARD_MIN
-        np.testing.assert_array_equal(hard[f][decided], ref.hard[0][decided])
         one = code.decode(d_llr[f:f + 1], d_syn[f:f + 1], n_iter, 1, want_posterior=True)
         torch.cuda.synchronize()
         assert torch.equal(one.posterior[0], out.posterior[f]) and torch.equal(one.hard[0], out.hard[f])
+    # frame independence inside the batch, for EVERY frame: the batch reversed gives the reversed outputs bit for bit
+    rev = code.decode(d_llr.flip(0).contiguous(), d_syn.flip(0).contiguous(), n_iter, 1, want_posterior=True)
+    torch.cuda.synchronize()
+    assert torch.equal(rev.posterior.flip(0), out.posterior) and torch.equal(rev.hard.flip(0), out.hard)
 
 
-def test_config5_full_size_sampled(oracle_lib, B):
-    """Config 5 at full Z: the highest-SNR point converges quickly; pass flags and iteration counts must agree."""
-    cfg, base, Z, fr = W.make_config(5, snr_point=5, n_frames=2)
-    ref = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, 60, 1)
-    hard, iters, passed, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, 60, 1)
-    print(f"cfg5 snr5 full: oracle pass {ref.passed} iters {ref.iters}; gpu {passed} {iters}")
-    np.testing.assert_array_equal(passed, ref.passed)
-    np.testing.assert_array_equal(iters, ref.iters)
-    ok = ref.passed.astype(bool)
-    np.testing.assert_array_equal(hard[ok], ref.hard[ok])
+def assert_stop_parity(sp, n_frames):
+    """north_star: "with early stop enabled the frame-error rate must be statistically consistent with the oracle".
+    Both sides decode the SAME inputs, so the comparison is per frame: discordant pass flags per point must lie inside
+    the binomial 95 % band around zero disagreement (expected 0, at most 1 of 32), every word the GPU
+    reports as decoded must satisfy H x = s, and frames decoded on both sides must give the same word."""
+    print(f"{sp.label}: FER gpu {sp.fer_gpu:.3f} oracle {sp.fer_oracle:.3f}; discordant pass flags "
+          f"{sp.discordant_pass}/{n_frames}, discordant iteration counts {sp.discordant_iters}/{n_frames}, "
+          f"iters_gpu - iters_oracle histogram {sp.diff_hist}")
+    lo, hi = PC.binomial_band_95(n_frames, sp.fer_oracle)
+    assert lo <= sp.fer_gpu <= hi, f"{sp.label}: GPU FER {sp.fer_gpu} outside the 95 % band [{lo:.3f}, {hi:.3f}]"
+    assert sp.discordant_pass <= 1, f"{sp.label}: {sp.discordant_pass} discordant pass flags"
+    assert sp.gpu_words_valid and sp.hard_mismatch_frames == 0
+    assert sp.discordant_iters <= max(1, n_frames // 16), f"{sp.label}: iteration counts differ on {sp.discordant_iters} frames"
+
+
+@pytest.mark.parametrize("snr_point", [0, 1, 2, 3, 4, 5])
+def test_config5_fer_vs_oracle(oracle_lib, B, snr_point):
+    """Config 5 as specified (32 frames per point, six SNR points, max 300 iterations, early stop on) on its base
+    graph lifted by Z = 2000 (the oracle finishes 192 frames in minutes): per-frame pass flags and iteration counts."""
+    cfg, base, Z, fr = W.make_config(5, snr_point=snr_point, Z=2000)
+    assert fr.llr.shape[0] == 32 and cfg.max_iter == 300
+    hard, iters, passed, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, want_posterior=False)
+    sp = PC.compare_stop(oracle_lib, base, Z, fr.llr, fr.syndrome, cfg.max_iter, f"cfg5 Z=2000 point {snr_point}",
+                         hard, iters, passed)
+    assert_stop_parity(sp, 32)
+
+
+@pytest.mark.parametrize("snr_point", [3, 4, 5])
+def test_config5_full_size_sampled(oracle_lib, B, snr_point):
+    """Config 5 at full Z = 10,000 inside the benched batch of 32 frames: the oracle decodes 4 sampled frames of the
+    waterfall points one by one (the frames run concurrently on the host cores)."""
+    cfg, base, Z, fr = W.make_config(5, snr_point=snr_point)
+    sample = np.array([0, 11, 21, 31])
+    hard, iters, passed, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, want_posterior=False)
+    sp = PC.compare_stop(oracle_lib, base, Z, fr.llr[sample], fr.syndrome[sample], cfg.max_iter,
+                         f"cfg5 full size point {snr_point} frames {sample.tolist()}", hard[sample], iters[sample],
+                         passed[sample])
+    print(f"  batch of 32: gpu pass {int(passed.sum())}/32, iterations {iters.min()}..{iters.max()}")
+    assert sp.discordant_pass == 0 and sp.discordant_iters == 0 and sp.gpu_words_valid and sp.hard_mismatch_frames == 0
 
 
 # ------------------------------------------------------------------------------------ pins applied to the GPU
@@ -338,6 +359,24 @@ def test_decode_host_matches_device_path(B):
     np.testing.assert_array_equal(out3.passed, p2)
     np.testing.assert_array_equal(out3.posterior, post2)
     assert n_host < n_dev // 3
+
+
+def test_decode_host_check_from_iter(oracle_lib, B):
+    """qcldpc_decode_host_ex: the early-termination scheduling on the host-buffer path."""
+    cfg, base, Z, fr = W.make_config(1)
+    code = B.QCLDPCCode(base, Z)
+    for check_from in (1, 9, 60):
+        ref = oracle_lib.decode(base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from=check_from)
+        out = code.decode_host(fr.llr, fr.syndrome, cfg.max_iter, 1, want_posterior=True, check_from_iter=check_from)
+        np.testing.assert_array_equal(out.iters, ref.iters)
+        np.testing.assert_array_equal(out.passed, ref.passed)
+        dev = gpu_decode(B, base, Z, fr.llr, fr.syndrome, cfg.max_iter, 1, check_from_iter=check_from)
+        np.testing.assert_array_equal(out.hard, dev[0])
+        np.testing.assert_array_equal(out.posterior, dev[3])
+    with pytest.raises(ValueError):
+        code.decode_host(fr.llr.astype(np.float64), fr.syndrome, 5, 0)        # wrong dtype must not be read as fp32
+    with pytest.raises(ValueError):
+        code.decode_host(fr.llr[:, ::2], fr.syndrome, 5, 0)                     # non-contiguous
 
 
 def test_gpu_argument_errors(B):
