@@ -133,6 +133,48 @@ int qcldpc_decode_host_ex(const qcldpc_code_t* code, const float* h_llr, const u
                           uint8_t* h_pass, float* h_posterior, void* d_workspace, size_t workspace_bytes,
                           void* stream);
 
+/*
+ * ---- The steps either side of the decoder (device pointers; each call only enqueues on `stream`) ----
+ *
+ * LLR front end, Step 1 of Algorithm 1: sigma^2_{N_v} <- sigma^2_Z / ||X_v||, Q_v <- 2 R_v / sigma^2_{N_v}.
+ *   d_r, d_x     const float [n_frames][n]  Alice's received values R_v = M_v / X_v (Eq. 1) and her own X_v
+ *   d_sigma2_z   const float [n_frames]     channel noise variance sigma^2_Z of each frame
+ *   dim          0: no side information, sigma^2_N = sigma^2_Z for every symbol (d_x may be NULL; this is the BIAWGN
+ *                   recipe LLR = 2 y / sigma^2 of BASELINE.json's configs)
+ *                1: the d = 1 scheme: sigma^2_{N_v} = sigma^2_Z / ||X_v||^norm_power.  norm_power = 2 is the
+ *                   variance Eq. 1 implies (noise term Z_v / X_v) and the one under which Q_v is the log-likelihood
+ *                   ratio Step 1 says it is; norm_power = 1 is the formula as printed at P:97 / P:344 (reading G5)
+ *                2: the d = 2 scheme: successive pairs (2i, 2i+1), 0-based, n even:
+ *                   a = (X_2i + X_2i+1) / (X_2i^2 + X_2i+1^2), b = (X_2i+1 - X_2i) / (same), sigma^2_N = (a^2 + b^2) sigma^2_Z
+ *                   (the d = 4 and d = 8 noise terms are not in the paper)
+ *   d_llr        float [n_frames][n]        Q_v, the input of qcldpc_decode
+ * IEEE single-precision arithmetic in the printed order (X_v = 0: infinite variance, Q_v = +-0).
+ */
+int qcldpc_llr_init(const float* d_r, const float* d_x, const float* d_sigma2_z, int n_frames, int64_t n, int dim,
+                    int norm_power, float* d_llr, void* stream);
+
+/*
+ * Bit-packed outputs (Step 5, keeps the first k bits of the decoded word): the first n_bits <= n hard decisions
+ * of every frame of d_hard (uint8 [n_frames][n], one byte per bit, only bit 0 is read) as (n_bits + 7) / 8 bytes per
+ * frame in d_packed (uint8 [n_frames][(n_bits + 7) / 8]); bit v of a frame is bit 7 - (v mod 8) of byte v / 8 (most
+ * significant bit first, reading G8); unused low bits of the last byte are zero.
+ */
+int qcldpc_pack_bits(const uint8_t* d_hard, int n_frames, int64_t n, int64_t n_bits, uint8_t* d_packed, void* stream);
+
+/*
+ * 32-bit CRC of each decoded message against the CRC that travels in the frame (Fig. 7: the k information
+ * bits are k - 32 message bits followed by N_CRC = 32 CRC bits; run it on the frames whose parity check
+ * passed).  CRC-32 of IEEE 802.3 (reading G7: polynomial 0x04C11DB7 bit-reflected, initial value and final XOR
+ * 0xFFFFFFFF; "123456789" -> 0xCBF43926) over the first (k_bits - 32) / 8 bytes of every row of d_packed; the stored
+ * CRC is the big-endian 32-bit number in the next 4 bytes.
+ *   d_packed      const uint8_t [n_frames][stride_bytes], stride_bytes >= k_bits / 8 (qcldpc_pack_bits output)
+ *   k_bits        a multiple of 8, >= 32
+ *   d_crc         uint32_t [n_frames]  the computed CRC (may be NULL)
+ *   d_ok          uint8_t  [n_frames]  1 iff computed == stored (may be NULL; not both NULL)
+ */
+int qcldpc_crc32_check(const uint8_t* d_packed, int n_frames, int64_t stride_bytes, int64_t k_bits, uint32_t* d_crc,
+                       uint8_t* d_ok, void* stream);
+
 /* Number of kernel launches the last qcldpc_decode / qcldpc_decode_host call of this thread enqueued. */
 int64_t qcldpc_last_launch_count(void);
 

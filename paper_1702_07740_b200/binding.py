@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = (
     "qcldpc_decode_ex",
     "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_decode_host_ex", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
+    "qcldpc_llr_init", "qcldpc_pack_bits", "qcldpc_crc32_check",
 )
 
 if not os.path.exists(SO_PATH):
@@ -57,6 +58,12 @@ _lib.qcldpc_profile_enable.argtypes = [_i]
 _lib.qcldpc_profile_collect.restype = _i
 _lib.qcldpc_profile_collect.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64),
                                         ctypes.POINTER(ctypes.c_int64)]
+_lib.qcldpc_llr_init.restype = _i
+_lib.qcldpc_llr_init.argtypes = [_vp, _vp, _vp, _i, ctypes.c_int64, _i, _i, _vp, _vp]
+_lib.qcldpc_pack_bits.restype = _i
+_lib.qcldpc_pack_bits.argtypes = [_vp, _i, ctypes.c_int64, ctypes.c_int64, _vp, _vp]
+_lib.qcldpc_crc32_check.restype = _i
+_lib.qcldpc_crc32_check.argtypes = [_vp, _i, ctypes.c_int64, ctypes.c_int64, _vp, _vp, _vp]
 _lib.qcldpc_status_string.restype = ctypes.c_char_p
 _lib.qcldpc_status_string.argtypes = [_i]
 _lib.qcldpc_last_cuda_error.restype = ctypes.c_char_p
@@ -283,6 +290,66 @@ class QCLDPCCode:
                                             workspace.data_ptr(), workspace.numel(), st.cuda_stream)
         _check(rc, "qcldpc_decode_host_ex")
         return out
+
+
+def _cuda_tensor(t, name, dtype, torch):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise ValueError(f"{name}: need a contiguous CUDA tensor of dtype {dtype}")
+    return t
+
+
+def llr_init(r, x, sigma2_z, dim: int = 1, norm_power: int = 2, out=None, stream=None):
+    """qcldpc_llr_init (P:344 Step 1): Q = 2 R / sigma_N^2 on device tensors r, x float32 [F][n] (x may be None for
+    dim = 0), sigma2_z float32 [F].  Returns Q float32 [F][n]; only enqueues on `stream`."""
+    import torch
+    _cuda_tensor(r, "r", torch.float32, torch)
+    _cuda_tensor(sigma2_z, "sigma2_z", torch.float32, torch)
+    if x is not None:
+        _cuda_tensor(x, "x", torch.float32, torch)
+        if x.shape != r.shape:
+            raise ValueError("r and x must have one shape")
+    if r.dim() != 2 or sigma2_z.numel() != r.shape[0]:
+        raise ValueError("r must be [F][n] and sigma2_z [F]")
+    if out is None:
+        out = torch.empty_like(r)
+    _cuda_tensor(out, "out", torch.float32, torch)
+    st = stream if stream is not None else torch.cuda.current_stream(r.device)
+    with torch.cuda.device(r.device):
+        rc = _lib.qcldpc_llr_init(r.data_ptr(), x.data_ptr() if x is not None else None, sigma2_z.data_ptr(),
+                                  r.shape[0], r.shape[1], int(dim), int(norm_power), out.data_ptr(), st.cuda_stream)
+    _check(rc, "qcldpc_llr_init")
+    return out
+
+
+def pack_bits(hard, n_bits: int, out=None, stream=None):
+    """qcldpc_pack_bits: the first n_bits of every row of hard (uint8 [F][n], one byte per bit) as bits, most
+    significant first; returns uint8 [F][(n_bits + 7) // 8]."""
+    import torch
+    _cuda_tensor(hard, "hard", torch.uint8, torch)
+    F, n = hard.shape
+    if out is None:
+        out = torch.empty((F, (int(n_bits) + 7) // 8), dtype=torch.uint8, device=hard.device)
+    _cuda_tensor(out, "out", torch.uint8, torch)
+    st = stream if stream is not None else torch.cuda.current_stream(hard.device)
+    with torch.cuda.device(hard.device):
+        rc = _lib.qcldpc_pack_bits(hard.data_ptr(), F, n, int(n_bits), out.data_ptr(), st.cuda_stream)
+    _check(rc, "qcldpc_pack_bits")
+    return out
+
+
+def crc32_check(packed, k_bits: int, stream=None):
+    """qcldpc_crc32_check on packed frames uint8 [F][>= k_bits / 8]: (crc uint32-as-int64 [F], ok uint8 [F])."""
+    import torch
+    _cuda_tensor(packed, "packed", torch.uint8, torch)
+    F, stride = packed.shape
+    crc = torch.empty(F, dtype=torch.int32, device=packed.device)
+    ok = torch.empty(F, dtype=torch.uint8, device=packed.device)
+    st = stream if stream is not None else torch.cuda.current_stream(packed.device)
+    with torch.cuda.device(packed.device):
+        rc = _lib.qcldpc_crc32_check(packed.data_ptr(), F, stride, int(k_bits), crc.data_ptr(), ok.data_ptr(),
+                                     st.cuda_stream)
+    _check(rc, "qcldpc_crc32_check")
+    return crc.to(torch.int64) & 0xFFFFFFFF, ok
 
 
 def raw_lib():

@@ -28,7 +28,8 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 
 def _units():
     units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), []),
-             (os.path.join(CSRC, "pass_generic.cu"), os.path.join(OBJDIR, "pass_generic.o"), [])]
+             (os.path.join(CSRC, "pass_generic.cu"), os.path.join(OBJDIR, "pass_generic.o"), []),
+             (os.path.join(CSRC, "frontend.cu"), os.path.join(OBJDIR, "frontend.o"), [])]
     for name, dv, ng, pcap in PASS_INSTANCES:
         units.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJDIR, f"{name}.o"),
                       [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={pcap}"]))
