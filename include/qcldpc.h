@@ -58,7 +58,8 @@ typedef struct qcldpc_code qcldpc_code_t;
  * call reads the environment.  Defaults are the measured best.  QCLDPC_V=1|2 variables per thread
  * of the exact pass; QCLDPC_FLIP=0 every launch walks the frames forwards; QCLDPC_MERGE_CHECK=0 early-exit check as a
  * separate launch; QCLDPC_CAND_PER_SM=k grid of that launch; QCLDPC_PACK=0 no lane packing and QCLDPC_FV=1|2 frames
- * per thread in the generic pass.  None of them changes any result.
+ * per thread in the generic pass; QCLDPC_LOOP=stream and QCLDPC_BODY=k (body of 12 k iterations) for the iteration
+ * loop (see qcldpc_iterations_issued).  None of them changes any result.
  */
 int qcldpc_code_create(const int32_t* base_shifts, int mb, int nb, int Z, qcldpc_code_t** out_code);
 void qcldpc_code_destroy(qcldpc_code_t* code);
@@ -82,8 +83,9 @@ size_t qcldpc_workspace_bytes(const qcldpc_code_t* code, int n_frames);
 
 /*
  * Decode n_frames independent frames (Algorithm 1, syndrome form), 1 <= n_frames <= QCLDPC_MAX_FRAMES.
- * Only ENQUEUES work on `stream`; never synchronises the device; allocates no device memory (the first call of a
- * process on a device sets kernel attributes).  All d_* are DEVICE pointers owned by the caller, frame-major and
+ * Only ENQUEUES work on `stream`; never synchronises the device; allocates no device memory of its own (the first call
+ * of a process on a device sets kernel attributes; the first call with a new argument tuple instantiates a CUDA graph,
+ * see qcldpc_iterations_issued).  All d_* are DEVICE pointers owned by the caller, frame-major and
  * contiguous:
  *   d_llr        const float   [n_frames][n]  Q_v = ln P(x_v=0)/P(x_v=1)
  *   d_syndrome   const uint8_t [n_frames][m]  s_c in {0,1} (only bit 0 is read)
@@ -118,9 +120,9 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
 /*
  * Same decode with HOST buffers (h_* are HOST pointers, same shapes; pinned memory makes the copies asynchronous):
  * copies inputs host->device, decodes, copies outputs device->host on `stream`, then WAITS for the stream so that the
- * h_* outputs are valid on return.  Because this call waits anyway, it reads the number of live frames back every 32
- * iterations and stops launching once every frame has stopped (same results; qcldpc_decode, which never waits, issues
- * all max_iter iterations and the leftover ones are empty grids).  h_posterior may be NULL.  The device staging area is part of d_workspace, which
+ * h_* outputs are valid on return.  The iteration loop ends on the device as in qcldpc_decode (with QCLDPC_LOOP=stream
+ * this call reads the number of live frames back every 32 iterations and stops launching once every frame has stopped).
+ * h_posterior may be NULL.  The device staging area is part of d_workspace, which
  * must hold qcldpc_host_workspace_bytes(code, n_frames, h_posterior != NULL) bytes.
  */
 size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int want_posterior);
@@ -175,8 +177,25 @@ int qcldpc_pack_bits(const uint8_t* d_hard, int n_frames, int64_t n, int64_t n_b
 int qcldpc_crc32_check(const uint8_t* d_packed, int n_frames, int64_t stride_bytes, int64_t k_bits, uint32_t* d_crc,
                        uint8_t* d_ok, void* stream);
 
-/* Number of kernel launches the last qcldpc_decode / qcldpc_decode_host call of this thread enqueued. */
+/* Number of kernel launches (graph path: kernel nodes, the loop body counted once) the last qcldpc_decode /
+ * qcldpc_decode_host call of this thread enqueued. */
 int64_t qcldpc_last_launch_count(void);
+
+/*
+ * The iteration loop runs on the DEVICE: by default a decode call builds (first call with a given argument tuple) and
+ * launches ONE CUDA graph whose conditional WHILE node repeats a body of 12 iterations until max_iter is reached or
+ * every frame of the batch has stopped ("Go to Step 5"), so a batch that has stopped costs at most one more body
+ * of empty launches although the call never waits.  Instantiated graphs are cached in the handle, keyed by all pointer
+ * and scalar arguments (the one place where the handle changes after creation; guarded by a mutex; building a graph
+ * allocates driver memory).  QCLDPC_LOOP=stream (read by qcldpc_code_create) keeps one launch per iteration from the
+ * host; so do decodes of fewer than 14 iterations and calls made while qcldpc_profile_enable is on.
+ *   qcldpc_iterations_issued  how many iterations' launches the last decode in d_workspace actually issued (reads one
+ *                             int back from the workspace on `stream` and WAITS for it; h_iterations: HOST pointer)
+ *   qcldpc_last_loop_mode     1 if the last decode call of this thread ran as a graph, 0 if as stream launches
+ */
+int qcldpc_iterations_issued(const qcldpc_code_t* code, int n_frames, const void* d_workspace, void* stream,
+                             int* h_iterations);
+int qcldpc_last_loop_mode(void);
 
 /*
  * Optional launch timing for roofline reports (bench.py).  qcldpc_profile_enable(stride) with stride > 0 makes the

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = (
     "qcldpc_decode_ex",
     "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_decode_host_ex", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
-    "qcldpc_llr_init", "qcldpc_pack_bits", "qcldpc_crc32_check",
+    "qcldpc_llr_init", "qcldpc_pack_bits", "qcldpc_crc32_check", "qcldpc_iterations_issued", "qcldpc_last_loop_mode",
 )
 
 if not os.path.exists(SO_PATH):
@@ -64,6 +64,10 @@ _lib.qcldpc_pack_bits.restype = _i
 _lib.qcldpc_pack_bits.argtypes = [_vp, _i, ctypes.c_int64, ctypes.c_int64, _vp, _vp]
 _lib.qcldpc_crc32_check.restype = _i
 _lib.qcldpc_crc32_check.argtypes = [_vp, _i, ctypes.c_int64, ctypes.c_int64, _vp, _vp, _vp]
+_lib.qcldpc_iterations_issued.restype = _i
+_lib.qcldpc_iterations_issued.argtypes = [_vp, _i, _vp, _vp, ctypes.POINTER(_i)]
+_lib.qcldpc_last_loop_mode.restype = _i
+_lib.qcldpc_last_loop_mode.argtypes = []
 _lib.qcldpc_status_string.restype = ctypes.c_char_p
 _lib.qcldpc_status_string.argtypes = [_i]
 _lib.qcldpc_last_cuda_error.restype = ctypes.c_char_p
@@ -89,6 +93,11 @@ def qcldpc_status_string(status: int) -> str:
 
 def qcldpc_last_launch_count() -> int:
     return int(_lib.qcldpc_last_launch_count())
+
+
+def qcldpc_last_loop_mode() -> int:
+    """1: the last decode of this thread ran as one graph with the loop on the device; 0: one launch per iteration."""
+    return int(_lib.qcldpc_last_loop_mode())
 
 
 def qcldpc_profile_enable(stride: int) -> None:
@@ -205,6 +214,16 @@ class QCLDPCCode:
 
     def host_workspace_bytes(self, n_frames: int, want_posterior: bool) -> int:
         return int(_lib.qcldpc_host_workspace_bytes(self._handle, int(n_frames), int(bool(want_posterior))))
+
+    def iterations_issued(self, n_frames: int, workspace, stream=None) -> int:
+        """qcldpc_iterations_issued: iterations whose launches the last decode in `workspace` issued (waits)."""
+        import torch
+        st = stream if stream is not None else torch.cuda.current_stream(workspace.device)
+        n = _i(0)
+        with torch.cuda.device(workspace.device):
+            _check(_lib.qcldpc_iterations_issued(self._handle, int(n_frames), workspace.data_ptr(), st.cuda_stream,
+                                                 ctypes.byref(n)), "qcldpc_iterations_issued")
+        return n.value
 
     # ---------------------------------------------------------------------------------------------- decode
     def decode(self, llr, syndrome, max_iter: int, early_stop: int, want_posterior: bool = True,

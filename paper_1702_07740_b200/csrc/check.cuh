@@ -25,6 +25,10 @@ struct CheckArgs {
     int* topbad_clear;           // the slot the next pass will write
     int* fullbad; int* unsat; unsigned* ticket;
     int n_frames, mb, Z, Zs, tiles, t, check_from; int64_t n, m, EZs, AZs;
+    // Device-side iteration loop (qcldpc.cu, LoopCtl): the iteration checked is t + *t_base (t_base = NULL: t itself);
+    // the last worker publishes the number of frames still iterating in *n_live; a launch issued after the loop
+    // has ended early (every frame stopped) does nothing when *skip is set.
+    const int* t_base; int* n_live; const int* skip;
 };
 
 #ifdef __CUDACC__
@@ -75,10 +79,13 @@ __device__ __forceinline__ unsigned check_one(const CheckTables& tab, const Chec
 __device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArgs& a, const int worker, const int n_workers,
                                           const int tid, const int nthr) {
     __shared__ unsigned s_last;
+    __shared__ int s_live;
+    if (a.skip && *a.skip) return;                                       // the loop ended early: nothing left to check
     const int units = a.mb * a.tiles;
+    const int t_now = a.t + (a.t_base ? *a.t_base : 0);                  // the iteration whose decisions are checked
     if (worker == 0)
         for (int f = tid; f < a.n_frames; f += nthr) a.topbad_clear[f] = 0;
-    if (a.t < a.check_from) return;                                      // launched only to clear the filter slot
+    if (t_now < a.check_from) return;                                    // launched only to clear the filter slot
     bool any = false;
     for (int f0 = 0; f0 < a.n_frames; f0 += nthr) {
         const int f = f0 + tid;
@@ -94,7 +101,7 @@ __device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArg
                 const int R = u / a.tiles;
                 const int r = (u - R * a.tiles) * nthr + tid;
                 unsigned bad = 0;
-                if (r < a.Z) bad = check_one<false>(tab, a, g, R, r, a.t);
+                if (r < a.Z) bad = check_one<false>(tab, a, g, R, r, t_now);
                 if (__syncthreads_or(bad != 0) && tid == 0) a.fullbad[g] = 1;
             }
         }
@@ -110,15 +117,21 @@ __device__ __forceinline__ void cand_work(const CheckTables& tab, const CheckArg
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    if (tid == 0) s_live = 0;
+    __syncthreads();
+    int live = 0;
     for (int f = tid; f < a.n_frames; f += nthr) {
         int d = a.done_r[f];
         if (!d && !a.topbad[f]) {
-            if (*((volatile int*)(a.fullbad + f)) == 0) { d = 1; a.iters[f] = a.t; a.pass[f] = 1; }
+            if (*((volatile int*)(a.fullbad + f)) == 0) { d = 1; a.iters[f] = t_now; a.pass[f] = 1; }
             a.fullbad[f] = 0;
         }
         a.done_w[f] = d;
+        live += d ? 0 : 1;
     }
-    if (tid == 0) *a.ticket = 0;
+    if (live) atomicAdd(&s_live, live);
+    __syncthreads();
+    if (tid == 0) { *a.n_live = s_live; *a.ticket = 0; }
 }
 #endif
 

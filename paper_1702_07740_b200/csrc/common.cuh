@@ -99,6 +99,7 @@ struct PassLaunch {
     int n_sm;                  // multiprocessors of the device
     int fv;                    // generic pass: frames per thread (1 or 2)
     int pack_ok;               // generic pass: lane packing allowed
+    int prepare_only;          // 1: set the kernel attributes of the instantiation this launch would use, launch nothing
 };
 using PassLauncher = void (*)(const PassLaunch&);
 using ExactBuilder = size_t (*)(const HostTables&, void* out);   // out = NULL: size only

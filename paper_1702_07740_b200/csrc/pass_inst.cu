@@ -59,6 +59,7 @@ static void launch_exact(const PassLaunch& L) {
 }
 
 void PASS_NAME(const PassLaunch& L) {
+    if (L.prepare_only) return;                          // no attributes to set: static shared memory only
     if (L.V == 2) { if (L.final_mode) launch_exact<2, true>(L); else launch_exact<2, false>(L); }
     else { if (L.final_mode) launch_exact<1, true>(L); else launch_exact<1, false>(L); }
 }

@@ -435,6 +435,7 @@ inline void launch_pass_tb(const PassLaunch& L, PassArgs args) {
         cudaFuncSetAttribute(k_pass<TB, G, FV, false, PACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         attr_dev = dev;
     }
+    if (L.prepare_only) return;
     // the early-exit check of iteration t-2 rides in extra CTAs of the same grid (check.cuh): about four per SM
     const bool with_check = !L.final_mode && L.check_args != nullptr;
     args.pack = PACK ? args.pack : 1;

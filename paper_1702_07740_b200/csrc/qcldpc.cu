@@ -33,6 +33,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -51,6 +52,7 @@ namespace {
 
 thread_local char g_cuda_error[512] = "";
 thread_local int64_t g_launches = 0;
+thread_local int g_loop_mode = 0;         // 1: the last decode of this thread ran as a graph with a device-side loop
 
 // Optional launch timing (qcldpc_profile_enable): CUDA event pairs around sampled launches, on the decode stream.
 struct Profile {
@@ -72,7 +74,16 @@ struct Tuning {
     int cand_per_sm = 0;                  // QCLDPC_CAND_PER_SM=k: grid of a separate k_cand launch (0: by batch size)
     int pack = 1;                         // QCLDPC_PACK=0: no lane packing in the generic pass
     int fv = 0;                           // QCLDPC_FV=1|2: frames per thread of the generic pass (0: by batch size)
+    int loop_graph = 1;                   // QCLDPC_LOOP=stream: one launch per iteration from the host, no graph
+    int body_mult = 1;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations
 };
+
+// One instantiated decode graph per argument tuple (the kernel parameters are baked into the graph's nodes).
+struct GraphKey {
+    const void *llr, *syn, *hard, *iters, *pass, *post, *ws;
+    int n_frames, max_iter, early_stop, check_from, device;
+};
+struct GraphEntry { GraphKey key; cudaGraphExec_t exec; uint64_t stamp; };
 
 static int env_int(const char* name, int dflt) {
     const char* e = getenv(name);
@@ -97,6 +108,11 @@ struct qcldpc_code {
     std::vector<char> exact;              // kernel-parameter table of the exact family (empty: generic kernel)
     int n_sm = 148;
     Tuning tune;                          // read ONCE from the environment by qcldpc_code_create (include/qcldpc.h)
+    // graph cache: the only mutable part of the handle, guarded by graph_mu (decode calls take a const handle)
+    std::mutex graph_mu;
+    std::vector<GraphEntry> graphs;
+    uint64_t graph_clock = 0;
+    cudaStream_t cap_main = nullptr, cap_body = nullptr;   // capture-only streams: nothing ever executes on them
 };
 
 namespace {
@@ -188,15 +204,40 @@ __global__ void k_live_count(const int* done, int n_frames, int* n_live) {
     if (threadIdx.x == 0) *n_live = s_c;
 }
 
+// Device-side state of the iteration loop: ints behind the grid ticket in the workspace.
+enum LoopCtl { kCtlLive = 16,        // host-polling path: frames still iterating, read back every kPollEvery launches
+               kCtlIterBase = 32,    // graph path: iterations the WHILE loop has completed (a multiple of the body length)
+               kCtlNLive = 33,       // frames still iterating, as of the last early-exit check that ran (cand_work)
+               kCtlStopped = 34,     // the loop ended because every frame had stopped (not because of max_iter)
+               kCtlIssued = 35 };    // passes launched by the decode call (qcldpc_iterations_issued)
+
 __global__ void k_reset(int* done2, int* unsat, int* topbad3, int* fullbad, unsigned* ticket, int32_t* iters,
                         uint8_t* pass, int n_frames, int max_iter) {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
-    if (f == 0) *ticket = 0;
+    if (f == 0) {
+        *ticket = 0;
+        int* ctl = reinterpret_cast<int*>(ticket);
+        ctl[kCtlIterBase] = 0; ctl[kCtlNLive] = n_frames; ctl[kCtlStopped] = 0; ctl[kCtlIssued] = 0;
+    }
     if (f >= n_frames) return;
     done2[f] = 0; done2[n_frames + f] = 0; unsat[f] = 0; fullbad[f] = 0;
     topbad3[f] = 0; topbad3[n_frames + f] = 0; topbad3[2 * n_frames + f] = 0;
     iters[f] = max_iter; pass[f] = 0;
 }
+
+// End of one body of the graph WHILE loop (`body` iterations): advance the iteration base and decide whether the loop
+// runs again: iterations remain AND some frame is still iterating ("Go to Step 5" for the whole batch).
+__global__ void k_loop_ctl(cudaGraphConditionalHandle handle, int* ctl, int body, int loop_iters, int pre_iters) {
+    const int completed = ctl[kCtlIterBase] + body;
+    ctl[kCtlIterBase] = completed;
+    ctl[kCtlIssued] = pre_iters + completed;
+    const bool more = completed < loop_iters;
+    const bool live = ctl[kCtlNLive] > 0;
+    if (more && !live) ctl[kCtlStopped] = 1;
+    cudaGraphSetConditional(handle, (more && live) ? 1u : 0u);
+}
+
+__global__ void k_set_int(int* p, int v) { *p = v; }
 
 // ---------------------------------------------------------------------------------------------------------------
 // host side
@@ -457,6 +498,9 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         tn.pack = env_int("QCLDPC_PACK", 1) != 0;
         const int fv = env_int("QCLDPC_FV", 0);
         tn.fv = (fv == 1 || fv == 2) ? fv : 0;
+        const char* lp = getenv("QCLDPC_LOOP");
+        tn.loop_graph = !(lp && strcmp(lp, "stream") == 0);
+        tn.body_mult = std::min(16, std::max(1, env_int("QCLDPC_BODY", 1)));
     }
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
@@ -482,6 +526,9 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
 
 void qcldpc_code_destroy(qcldpc_code_t* code) {
     if (!code) return;
+    for (GraphEntry& ge : code->graphs) cudaGraphExecDestroy(ge.exec);
+    if (code->cap_main) cudaStreamDestroy(code->cap_main);
+    if (code->cap_body) cudaStreamDestroy(code->cap_body);
     cudaFree(code->d_edge); cudaFree(code->d_gen); cudaFree(code->d_partner); cudaFree(code->d_col);
     cudaFree(code->d_row); cudaFree(code->d_redge);
     delete code;
@@ -507,9 +554,203 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
                             d_posterior, d_workspace, workspace_bytes, stream);
 }
 
-// host_poll: the caller waits for the stream anyway (qcldpc_decode_host), so every kPollEvery iterations the number of
-// live frames is read back and the launch sequence ends once every frame has stopped.  The device-pointer API never
-// waits: there the leftover launches of a fully stopped batch are empty grids.
+// Two ways to run the iteration loop (same kernels, same results):
+//   graph   (default) one CUDA graph per decode: prologue, the first few iterations, a conditional WHILE node whose
+//           body is kLoopBody iterations + k_loop_ctl, epilogue.  The loop ends on the DEVICE when max_iter is reached or
+//           when every frame has stopped, so a batch that has stopped issues at most one more body of (empty)
+//           launches and the call still only enqueues.  Buffer rotation has period 12 (4 state buffers, 3 decision
+//           buffers, 2 flag versions), so the body's kernel parameters are static; only the iteration NUMBER is read
+//           from device memory (CheckArgs::t_base).  Instantiated graphs are cached in the handle by argument tuple.
+//   stream  (QCLDPC_LOOP=stream, profiling on, or fewer iterations than one body) one launch per iteration from the
+//           host; qcldpc_decode_host then polls the number of live frames every kPollEvery launches (host_poll).
+namespace {
+
+constexpr int kLoopBody = 12;
+
+struct DecodePlan {
+    const qcldpc_code* code;
+    Workspace w;
+    PassTables ptab; CheckTables ctab;
+    InitArgs ia;
+    PassLaunch pl;
+    CheckArgs ca;
+    int n_frames, max_iter, early_stop, check_from, cand_blocks, tiles1, fblocks;
+    bool merge_check, flip;
+    int* ctl;
+    int32_t* d_iters; uint8_t* d_pass;
+
+    int* done_ver(int t) const { return w.done + (size_t)(t & 1) * n_frames; }
+    int* topbad_slot(int T) const { return w.topbad + (size_t)(((T % 3) + 3) % 3) * n_frames; }
+    // the check is launched for iterations T >= check_from - 2: the filter slot of iteration I is dirty from pass I-2
+    // and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
+    bool check_wanted(int T) const { return early_stop && T >= 1 && T >= check_from - 2; }
+};
+
+void issue_prologue(DecodePlan& P, cudaStream_t st) {
+    k_reset<<<P.fblocks, 128, 0, st>>>(P.w.done, P.w.unsat, P.w.topbad, P.w.fullbad, P.w.ticket, P.d_iters, P.d_pass,
+                                       P.n_frames, P.max_iter);
+    ++g_launches;
+    if (P.code->n_act_cols > 0) {
+        k_init_cols<<<dim3(P.tiles1 * P.code->n_act_cols, P.n_frames), kThreads, 0, st>>>(P.ptab, P.ia);
+        ++g_launches;
+    }
+    k_init_rows<<<dim3(P.tiles1 * P.code->mb, P.n_frames), kThreads, 0, st>>>(P.ctab, P.ia);
+    ++g_launches;
+}
+
+// check of iteration T (+ *t_base), issued with launch t: reads the stopped-frame flags of version t & 1 (the ones pass
+// t reads) and writes version (t + 1) & 1 for pass t+1
+void set_check(DecodePlan& P, int T, int t, const int* t_base, const int* skip) {
+    P.ca.t = T;
+    P.ca.t_base = t_base;
+    P.ca.skip = skip;
+    P.ca.topbad = P.topbad_slot(T);
+    P.ca.topbad_clear = P.topbad_slot(t);                // the slot pass t+1 writes (filter of iteration t)
+    P.ca.done_r = P.done_ver(t);
+    P.ca.done_w = P.done_ver(t + 1);
+}
+
+void launch_check(DecodePlan& P, cudaStream_t st, int T, int t, const int* t_base, const int* skip) {
+    set_check(P, T, t, t_base, skip);
+    const int pk = prof_begin(1, st);
+    launch_pdl(k_cand, dim3(P.cand_blocks), dim3(kThreads), 0, st, P.ctab, P.ca);
+    prof_end(pk, st);
+    ++g_launches;
+}
+
+// Launch t = pass t carrying (or followed by) the early-exit check of iteration t-2 (check.cuh explains the lag).
+// t_base != NULL: inside the WHILE body; t is then the launch's number in the FIRST trip of the loop, the real number is
+// t + *t_base (the same modulo 12), and the check is always issued (the device decides whether it is due).
+void issue_iteration(DecodePlan& P, cudaStream_t st, int t, const int* t_base) {
+    const qcldpc_code* code = P.code;
+    const bool want = t_base ? (P.early_stop != 0) : P.check_wanted(t - 2);
+    const bool merged = P.merge_check && want && code->n_act_cols > 0;
+    if (code->n_act_cols > 0) {
+        PassLaunch& pl = P.pl;
+        pl.stream = st;
+        pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
+        pl.args.flip = P.flip ? (t & 1) : 0;
+        pl.args.hard_in = P.w.hardbuf[(t - 1) % 3]; pl.args.hard_out = P.w.hardbuf[t % 3];
+        pl.args.topbad = P.topbad_slot(t - 1);
+        pl.args.done = P.done_ver(t);
+        pl.check_tab = nullptr; pl.check_args = nullptr;
+        if (merged) {
+            set_check(P, t - 2, t, t_base, nullptr);
+            pl.check_tab = &P.ctab; pl.check_args = &P.ca;
+        }
+        const int pk = prof_begin(0, st);
+        code->launcher(pl);
+        prof_end(pk, st);
+        ++g_launches;
+    }
+    if (want && !merged) launch_check(P, st, t - 2, t, t_base, nullptr);
+}
+
+// after the last launch t_last: the check of the last but one executed iteration (the last one is settled by
+// k_check_final), then the outputs from each frame's frozen state: iteration d_iters[f] (= max_iter for the frames that
+// did not stop)
+void issue_epilogue(DecodePlan& P, cudaStream_t st, int t_last, const int* skip) {
+    if (t_last >= 2 && P.check_wanted(t_last - 1)) launch_check(P, st, t_last - 1, t_last + 1, nullptr, skip);
+    if (P.code->n_act_cols > 0 && P.max_iter > 0) {
+        P.pl.stream = st;
+        P.pl.final_mode = true;
+        P.pl.check_tab = nullptr; P.pl.check_args = nullptr;
+        P.code->launcher(P.pl);
+        P.pl.final_mode = false;
+        ++g_launches;
+    }
+    set_check(P, 0, 0, nullptr, nullptr);
+    k_check_final<<<dim3(P.tiles1 * P.code->mb, P.n_frames), kThreads, 0, st>>>(P.ctab, P.ca);
+    k_flags_final<<<P.fblocks, 128, 0, st>>>(P.w.unsat, P.d_pass, P.n_frames);
+    g_launches += 2;
+}
+
+// Captures the whole decode into a graph with a conditional WHILE node around the bulk of the iterations.
+// Returns cudaSuccess and the instantiated graph, or the error (the caller then runs the stream path).
+cudaError_t build_decode_graph(DecodePlan& P, cudaGraphExec_t* exec_out) {
+    qcldpc_code* code = const_cast<qcldpc_code*>(P.code);          // the capture streams live in the handle (under graph_mu)
+    cudaError_t e = cudaSuccess;
+    if (!code->cap_main) e = cudaStreamCreateWithFlags(&code->cap_main, cudaStreamNonBlocking);
+    if (e == cudaSuccess && !code->cap_body) e = cudaStreamCreateWithFlags(&code->cap_body, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return e;
+    if (code->n_act_cols > 0) {                                   // kernel attributes are set outside the capture
+        P.pl.prepare_only = 1;
+        P.pl.final_mode = false; code->launcher(P.pl);
+        P.pl.final_mode = true; code->launcher(P.pl);
+        P.pl.final_mode = false;
+        P.pl.prepare_only = 0;
+    }
+    const int body = kLoopBody * code->tune.body_mult;
+    int pre = P.max_iter % body;
+    if (pre < 2) pre += body;                                     // every launch of the body carries a check of T >= 1
+    const int loops = (P.max_iter - pre) / body;                  // > 0: the caller made sure
+    int* const iter_base = P.ctl + kCtlIterBase;
+    const int* const stopped = P.ctl + kCtlStopped;
+
+    cudaStream_t cm = code->cap_main, cb = code->cap_body;
+    e = cudaStreamBeginCapture(cm, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return e;
+    cudaGraph_t graph = nullptr;
+    bool body_open = false;
+    auto bail = [&](cudaError_t err) {
+        cudaGraph_t g = nullptr;
+        if (body_open) cudaStreamEndCapture(cb, &g);
+        g = nullptr;
+        cudaStreamEndCapture(cm, &g);
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        return err;
+    };
+    issue_prologue(P, cm);
+    for (int t = 1; t <= pre; ++t) issue_iteration(P, cm, t, nullptr);
+    {
+        cudaStreamCaptureStatus status;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t n_deps = 0;
+        e = cudaStreamGetCaptureInfo(cm, &status, nullptr, &graph, &deps, &n_deps);
+        if (e != cudaSuccess || status != cudaStreamCaptureStatusActive) return bail(e != cudaSuccess ? e : cudaErrorUnknown);
+        cudaGraphConditionalHandle handle;
+        e = cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault);
+        if (e != cudaSuccess) return bail(e);
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t loop_node;
+        e = cudaGraphAddNode(&loop_node, graph, deps, n_deps, &np);
+        if (e != cudaSuccess) return bail(e);
+        cudaGraph_t body_graph = np.conditional.phGraph_out[0];
+        e = cudaStreamUpdateCaptureDependencies(cm, &loop_node, 1, cudaStreamSetCaptureDependencies);
+        if (e != cudaSuccess) return bail(e);
+        e = cudaStreamBeginCaptureToGraph(cb, body_graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) return bail(e);
+        body_open = true;
+        for (int j = 1; j <= body; ++j) issue_iteration(P, cb, pre + j, iter_base);
+        k_loop_ctl<<<1, 1, 0, cb>>>(handle, P.ctl, body, loops * body, pre);
+        ++g_launches;
+        cudaGraph_t g2 = nullptr;
+        e = cudaStreamEndCapture(cb, &g2);
+        body_open = false;
+        if (e != cudaSuccess) return bail(e);
+    }
+    issue_epilogue(P, cm, P.max_iter, stopped);
+    e = cudaStreamEndCapture(cm, &graph);
+    if (e != cudaSuccess) { cudaGetLastError(); return e; }
+    e = cudaGraphInstantiate(exec_out, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) cudaGetLastError();
+    return e;
+}
+
+bool same_key(const GraphKey& a, const GraphKey& b) {
+    return a.llr == b.llr && a.syn == b.syn && a.hard == b.hard && a.iters == b.iters && a.pass == b.pass &&
+           a.post == b.post && a.ws == b.ws && a.n_frames == b.n_frames && a.max_iter == b.max_iter &&
+           a.early_stop == b.early_stop && a.check_from == b.check_from && a.device == b.device;
+}
+
+}  // namespace
+
 static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                        int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
                        uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream,
@@ -535,25 +776,22 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         workspace_bytes < qcldpc_workspace_bytes(code, n_frames))
         return QCLDPC_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const Workspace w = carve(code, n_frames, d_workspace);
+    DecodePlan P;
+    P.code = code;
+    P.w = carve(code, n_frames, d_workspace);
+    const Workspace& w = P.w;
     const int Z = code->Z, Zs = code->Zs;
     const int64_t EZs = (int64_t)code->n_act_edges * Zs, mZs = (int64_t)code->mb * Zs;
     const int64_t AZs = (int64_t)code->n_act_cols * Zs;
-    const int tiles1 = (Z + kThreads - 1) / kThreads;
-    const int fblocks = (n_frames + 127) / 128;
-    const PassTables ptab{code->d_edge, code->d_gen, code->d_partner, code->d_col};
-    const CheckTables ctab{code->d_row, code->d_redge};
-
-    k_reset<<<fblocks, 128, 0, st>>>(w.done, w.unsat, w.topbad, w.fullbad, w.ticket, d_iters, d_pass, n_frames, max_iter);
-    ++g_launches;
-    const InitArgs ia{d_llr, d_syndrome, w.qbuf[0], w.t, w.hardbuf[0], d_hard, d_posterior,
-                      Z, Zs, tiles1, code->halo, code->n, code->m, EZs, mZs, AZs};
-    if (code->n_act_cols > 0) {
-        k_init_cols<<<dim3(tiles1 * code->n_act_cols, n_frames), kThreads, 0, st>>>(ptab, ia);
-        ++g_launches;
-    }
-    k_init_rows<<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(ctab, ia);
-    ++g_launches;
+    P.tiles1 = (Z + kThreads - 1) / kThreads;
+    P.fblocks = (n_frames + 127) / 128;
+    P.ptab = PassTables{code->d_edge, code->d_gen, code->d_partner, code->d_col};
+    P.ctab = CheckTables{code->d_row, code->d_redge};
+    P.n_frames = n_frames; P.max_iter = max_iter; P.early_stop = early_stop; P.check_from = check_from_iter;
+    P.d_iters = d_iters; P.d_pass = d_pass;
+    P.ctl = reinterpret_cast<int*>(w.ticket);
+    P.ia = InitArgs{d_llr, d_syndrome, w.qbuf[0], w.t, w.hardbuf[0], d_hard, d_posterior,
+                    Z, Zs, P.tiles1, code->halo, code->n, code->m, EZs, mZs, AZs};
 
     // exact families: two variables per thread (1 KB windows) once the grid still fills the chip several times over;
     // small batches keep one variable per thread (more CTAs in flight).  Tuning::V overrides.
@@ -563,93 +801,98 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         if (ctas_v2 >= (int64_t)4 * 8 * code->n_sm) V = 2;
         if (code->tune.V) V = code->tune.V;
     }
-    const bool flip_frames = code->tune.flip != 0;
+    P.flip = code->tune.flip != 0;
     const int fv = code->tune.fv ? code->tune.fv : (n_frames >= 4 ? 2 : 1);   // generic pass: frames per thread
-    PassLaunch pl{ptab,
-                  PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
-                           w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
-                  st, V, false,
-                  code->exact.empty() ? nullptr : code->exact.data(), nullptr, nullptr, code->n_act_cols, n_frames,
-                  code->max_np, code->max_dv, code->n_sm, fv, code->tune.pack};
-    CheckArgs ca{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
-                 {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
-                 d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
-                 n_frames, code->mb, Z, Zs, tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs};
+    P.pl = PassLaunch{P.ptab,
+                      PassArgs{d_llr, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]}, w.t, nullptr, nullptr, d_hard, d_posterior,
+                               w.done, d_iters, nullptr, 0, 0, Z, Zs, code->tiles, 0, 0, n_frames, -1, code->n, EZs, mZs, AZs},
+                      st, V, false,
+                      code->exact.empty() ? nullptr : code->exact.data(), nullptr, nullptr, code->n_act_cols, n_frames,
+                      code->max_np, code->max_dv, code->n_sm, fv, code->tune.pack, 0};
+    P.ca = CheckArgs{d_llr, d_syndrome, {w.qbuf[0], w.qbuf[1], w.qbuf[2], w.qbuf[3]},
+                     {w.hardbuf[0], w.hardbuf[1], w.hardbuf[2]}, d_hard,
+                     d_posterior, w.done, w.done, d_iters, d_pass, nullptr, nullptr, w.fullbad, w.unsat, w.ticket,
+                     n_frames, code->mb, Z, Zs, P.tiles1, 0, check_from_iter, code->n, code->m, EZs, AZs,
+                     nullptr, P.ctl + kCtlNLive, nullptr};
     // early-exit grid: persistent; small batches are launch-bound and almost never have a candidate, so a smaller grid
     // (less to schedule and retire between two passes) wins there
     const int cand_per_sm = code->tune.cand_per_sm ? code->tune.cand_per_sm : (n_frames <= 8 ? 1 : 4);
-    const int cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * tiles1));
+    P.cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * P.tiles1));
+    P.merge_check = code->tune.merge_check != 0;
 
-    // Launch t = pass t, then the early-exit check of iteration t-2 (check.cuh explains the lag): the check reads the
-    // stopped-frame flags of version t & 1 (the ones pass t reads) and writes version (t + 1) & 1 for pass t+1.
-    auto done_ver = [&](int t) { return w.done + (size_t)(t & 1) * n_frames; };
-    auto topbad_slot = [&](int T) { return w.topbad + (size_t)(((T % 3) + 3) % 3) * n_frames; };
-    auto launch_check = [&](int T, int t) {              // check of iteration T, issued with launch t
-        ca.t = T;
-        ca.topbad = topbad_slot(T);
-        ca.topbad_clear = topbad_slot(t);                // the slot pass t+1 writes (filter of iteration t)
-        ca.done_r = done_ver(t);
-        ca.done_w = done_ver(t + 1);
-        const int pk = prof_begin(1, st);
-        launch_pdl(k_cand, dim3(cand_blocks), dim3(kThreads), 0, st, ctab, ca);
-        prof_end(pk, st);
-        ++g_launches;
-    };
-    // the check is launched for iterations T >= check_from_iter - 2: the filter slot of iteration I is dirty from pass
-    // I-2 and is cleared by the launch of iteration I-2, so the two launches before the first checked iteration only clear
-    auto check_wanted = [&](int T) { return early_stop && T >= 1 && T >= check_from_iter - 2; };
-    const bool merge_check = code->tune.merge_check != 0;
-    pl.check_tab = nullptr; pl.check_args = nullptr;
+    // ---- graph path
+    const int body = kLoopBody * code->tune.body_mult;
+    if (code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2) {
+        int dev = 0;
+        CUDA_TRY(cudaGetDevice(&dev));
+        const GraphKey key{d_llr, d_syndrome, d_hard, d_iters, d_pass, d_posterior, d_workspace,
+                           n_frames, max_iter, early_stop, check_from_iter, dev};
+        qcldpc_code* mc = const_cast<qcldpc_code*>(code);
+        std::lock_guard<std::mutex> lock(mc->graph_mu);
+        cudaGraphExec_t exec = nullptr;
+        for (GraphEntry& ge : mc->graphs)
+            if (same_key(ge.key, key)) { exec = ge.exec; ge.stamp = ++mc->graph_clock; break; }
+        if (!exec) {
+            const cudaError_t e = build_decode_graph(P, &exec);
+            if (e != cudaSuccess) {
+                exec = nullptr;
+                snprintf(g_cuda_error, sizeof(g_cuda_error), "graph loop unavailable (%s): stream loop used",
+                         cudaGetErrorString(e));
+                g_launches = 0;
+            } else {
+                if (mc->graphs.size() >= 8) {                    // evict the least recently used entry
+                    size_t old = 0;
+                    for (size_t k = 1; k < mc->graphs.size(); ++k)
+                        if (mc->graphs[k].stamp < mc->graphs[old].stamp) old = k;
+                    cudaGraphExecDestroy(mc->graphs[old].exec);  // a launch in flight completes first
+                    mc->graphs.erase(mc->graphs.begin() + old);
+                }
+                mc->graphs.push_back(GraphEntry{key, exec, ++mc->graph_clock});
+            }
+        }
+        if (exec) {
+            CUDA_TRY(cudaGraphLaunch(exec, st));
+            g_loop_mode = 1;
+            return QCLDPC_OK;
+        }
+    }
+
+    // ---- stream path
+    g_loop_mode = 0;
+    issue_prologue(P, st);
     int t_last = 0;                                      // last launch issued
     for (int t = 1; t <= max_iter; ++t) {
-        // the check of iteration t-2 rides in the grid of pass t (one launch per iteration)
-        const bool merged = merge_check && check_wanted(t - 2) && code->n_act_cols > 0;
-        if (code->n_act_cols > 0) {
-            pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
-            pl.args.flip = flip_frames ? (t & 1) : 0;
-            pl.args.hard_in = w.hardbuf[(t - 1) % 3]; pl.args.hard_out = w.hardbuf[t % 3];
-            pl.args.topbad = topbad_slot(t - 1);
-            pl.args.done = done_ver(t);
-            pl.check_tab = nullptr; pl.check_args = nullptr;
-            if (merged) {
-                ca.t = t - 2;
-                ca.topbad = topbad_slot(t - 2);
-                ca.topbad_clear = topbad_slot(t);
-                ca.done_r = done_ver(t);
-                ca.done_w = done_ver(t + 1);
-                pl.check_tab = &ctab; pl.check_args = &ca;
-            }
-            const int pk = prof_begin(0, st);
-            code->launcher(pl);
-            prof_end(pk, st);
-            ++g_launches;
-        }
-        if (check_wanted(t - 2) && !merged) launch_check(t - 2, t);
+        issue_iteration(P, st, t, nullptr);
         t_last = t;
         if (host_poll && early_stop && t % kPollEvery == 0 && t < max_iter) {
-            int* const d_live = reinterpret_cast<int*>(w.ticket) + 16;
+            int* const d_live = P.ctl + kCtlLive;
             int live = 1;
-            k_live_count<<<1, 128, 0, st>>>(check_wanted(t - 2) ? done_ver(t + 1) : done_ver(t), n_frames, d_live);
+            k_live_count<<<1, 128, 0, st>>>(P.check_wanted(t - 2) ? P.done_ver(t + 1) : P.done_ver(t), n_frames, d_live);
             ++g_launches;
             CUDA_TRY(cudaMemcpyAsync(&live, d_live, sizeof(int), cudaMemcpyDeviceToHost, st));
             CUDA_TRY(cudaStreamSynchronize(st));
             if (live == 0) break;                        // every frame is frozen: the remaining launches would be empty
         }
     }
-    // the check of the last but one executed iteration (the last one is settled by k_check_final below)
-    if (t_last >= 2 && check_wanted(t_last - 1)) launch_check(t_last - 1, t_last + 1);
-    // outputs from each frame's frozen state: iteration d_iters[f] (= max_iter for the frames that did not stop)
-    if (code->n_act_cols > 0 && max_iter > 0) {
-        pl.final_mode = true;
-        code->launcher(pl);
-        ++g_launches;
-    }
-    k_check_final<<<dim3(tiles1 * code->mb, n_frames), kThreads, 0, st>>>(ctab, ca);
-    k_flags_final<<<fblocks, 128, 0, st>>>(w.unsat, d_pass, n_frames);
-    g_launches += 2;
+    k_set_int<<<1, 1, 0, st>>>(P.ctl + kCtlIssued, t_last);
+    ++g_launches;
+    issue_epilogue(P, st, t_last, nullptr);
     CUDA_TRY(cudaGetLastError());
     return QCLDPC_OK;
 }
+
+int qcldpc_iterations_issued(const qcldpc_code_t* code, int n_frames, const void* d_workspace, void* stream,
+                             int* h_iterations) {
+    if (!code || n_frames <= 0 || !d_workspace || !h_iterations) return QCLDPC_ERR_BAD_ARGUMENT;
+    const Workspace w = carve(code, n_frames, const_cast<void*>(d_workspace));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CUDA_TRY(cudaMemcpyAsync(h_iterations, reinterpret_cast<const int*>(w.ticket) + kCtlIssued, sizeof(int),
+                             cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return QCLDPC_OK;
+}
+
+int qcldpc_last_loop_mode(void) { return g_loop_mode; }
 
 size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int want_posterior) {
     if (!code || n_frames <= 0) return 0;

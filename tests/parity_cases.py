@@ -24,7 +24,8 @@ from paper_1702_07740_b200 import workloads as W
 TOL = 1e-3
 HARD_MIN = 1e-2
 UNPINNED_AT = TOL / 2          # "if oracle32 itself leaves the tolerance" -- taken at half of it
-UNPINNED_FACTOR = 4.0          # GPU deviation allowed on an unpinned frame, in units of the measured floor
+UNPINNED_FACTOR = 6.0          # GPU deviation allowed on an unpinned frame, in units of its floor: measured ratios on the
+                               # chaotic frames of config 1 reach 3.9 (profiles/r02_parity_report.md), + 50 % margin
 HARD_PINNED_ERR = HARD_MIN / 2  # below this deviation the hard bits with |L| > HARD_MIN are asserted, above it (only possible on
                                # an unpinned frame) the mismatch count is reported
 

@@ -334,7 +334,7 @@ def test_degenerate_and_general_codes(oracle_lib, B, case):
     np.testing.assert_array_equal(iters, ref.iters)
 
 
-def test_decode_host_matches_device_path(B):
+def test_decode_host_matches_device_path(B, monkeypatch):
     cfg, base, Z, fr = W.make_config(1)
     code = B.QCLDPCCode(base, Z)
     h, i, p, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, 30, 1)
@@ -346,18 +346,27 @@ def test_decode_host_matches_device_path(B):
     out2 = code.decode_host(fr.llr, fr.syndrome, 30, 1, want_posterior=False)
     np.testing.assert_array_equal(out2.hard, h)
     assert B.qcldpc_last_launch_count() > 0
-    # a batch whose frames all stop early: the host path ends the launch sequence once nothing is live (it waits for
-    # the stream anyway), the device path enqueues all max_iter iterations; same outputs, far fewer launches
+    # a batch whose frames all stop early: same outputs from both paths, and with the host-driven loop
+    # (QCLDPC_LOOP=stream) the host path ends the launch sequence once nothing is live while the device-pointer path
+    # enqueues all max_iter iterations (with the default graph loop both end on the device:
+    # test_device_loop_stops_issuing_when_the_batch_has_stopped)
     conv = np.nonzero(p)[0][:6]
     h2, i2, p2, post2 = gpu_decode(B, base, Z, fr.llr[conv], fr.syndrome[conv], 400, 1)
-    n_dev = B.qcldpc_last_launch_count()
     out3 = code.decode_host(fr.llr[conv], fr.syndrome[conv], 400, 1, want_posterior=True)
-    n_host = B.qcldpc_last_launch_count()
     assert p2.all() and i2.max() < 64
     np.testing.assert_array_equal(out3.hard, h2)
     np.testing.assert_array_equal(out3.iters, i2)
     np.testing.assert_array_equal(out3.passed, p2)
     np.testing.assert_array_equal(out3.posterior, post2)
+    monkeypatch.setenv("QCLDPC_LOOP", "stream")
+    code_s = B.QCLDPCCode(base, Z)
+    monkeypatch.delenv("QCLDPC_LOOP")
+    PC.gpu_decode(B, code_s, Z, fr.llr[conv], fr.syndrome[conv], 400, 1)
+    n_dev = B.qcldpc_last_launch_count()
+    out4 = code_s.decode_host(fr.llr[conv], fr.syndrome[conv], 400, 1, want_posterior=True)
+    n_host = B.qcldpc_last_launch_count()
+    np.testing.assert_array_equal(out4.iters, i2)
+    np.testing.assert_array_equal(out4.posterior, post2)
     assert n_host < n_dev // 3
 
 
@@ -377,6 +386,64 @@ def test_decode_host_check_from_iter(oracle_lib, B):
         code.decode_host(fr.llr.astype(np.float64), fr.syndrome, 5, 0)        # wrong dtype must not be read as fp32
     with pytest.raises(ValueError):
         code.decode_host(fr.llr[:, ::2], fr.syndrome, 5, 0)                     # non-contiguous
+
+
+@pytest.mark.parametrize("max_iter", [14, 15, 25, 26, 27, 37, 38, 39, 49, 61, 120])
+def test_device_loop_matches_stream_loop_and_oracle(oracle_lib, B, max_iter, monkeypatch):
+    """The iteration loop as a graph WHILE node (default) against one launch per iteration from the host
+    (QCLDPC_LOOP=stream, read at handle creation) and against the oracle, for budgets on both sides of every body
+    boundary (pre-loop 2..13 iterations, bodies of 12), early stop on and off."""
+    cfg, base, Z, fr = W.make_config(1)
+    llr = np.concatenate([fr.llr, 25.0 * (1.0 - 2.0 * fr.x[:2].astype(np.float32))])   # + two noiseless frames
+    syn = np.concatenate([fr.syndrome, fr.syndrome[:2]])
+    code_g = B.QCLDPCCode(base, Z)
+    monkeypatch.setenv("QCLDPC_LOOP", "stream")
+    code_s = B.QCLDPCCode(base, Z)
+    monkeypatch.delenv("QCLDPC_LOOP")
+    for early in (1, 0):
+        g = PC.gpu_decode(B, code_g, Z, llr, syn, max_iter, early)
+        assert B.qcldpc_last_loop_mode() == 1
+        s_ = PC.gpu_decode(B, code_s, Z, llr, syn, max_iter, early)
+        assert B.qcldpc_last_loop_mode() == 0
+        for a, b in zip(g, s_):
+            np.testing.assert_array_equal(a, b)
+        ref = oracle_lib.decode(base, Z, llr, syn, max_iter, early)
+        np.testing.assert_array_equal(g[1], ref.iters)
+        np.testing.assert_array_equal(g[2], ref.passed)
+        ok = ref.passed.astype(bool)
+        np.testing.assert_array_equal(g[0][ok], ref.hard[ok])
+
+
+def test_device_loop_stops_issuing_when_the_batch_has_stopped(B):
+    """qcldpc_decode only enqueues, yet a batch whose frames have all stopped must not pay for max_iter launches: the
+    WHILE loop ends on the device.  Also: a second call with the same arguments re-launches the cached graph."""
+    cfg, base, Z, fr = W.make_config(1)
+    code = B.QCLDPCCode(base, Z)
+    h, i, p, post = gpu_decode(B, base, Z, fr.llr, fr.syndrome, 50, 1)
+    conv = np.nonzero(p)[0][:6]
+    d_llr = torch.from_numpy(fr.llr[conv]).cuda()
+    d_syn = torch.from_numpy(fr.syndrome[conv]).cuda()
+    ws = torch.empty(code.workspace_bytes(len(conv)), dtype=torch.uint8, device="cuda")
+    out = code.decode(d_llr, d_syn, 4000, 1, want_posterior=True, workspace=ws)
+    assert B.qcldpc_last_loop_mode() == 1
+    issued = code.iterations_issued(len(conv), ws)
+    iters = out.iters.cpu().numpy()
+    assert out.passed.cpu().numpy().all() and iters.max() < 64
+    np.testing.assert_array_equal(iters, i[conv])
+    # the last check that can stop a frame runs two launches after its iteration; the loop looks at the count of live
+    # frames once per body of 12, and the first 2..13 iterations run before the loop
+    assert iters.max() + 2 <= issued <= iters.max() + 2 + 12 + 13, (issued, iters.max())
+    out2 = code.decode(d_llr, d_syn, 4000, 1, want_posterior=True, workspace=ws, out=out)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(out2.iters.cpu().numpy(), iters)
+    np.testing.assert_array_equal(out2.posterior.cpu().numpy()[:, :64], post[conv][:, :64])
+    # a batch that never stops issues exactly max_iter iterations
+    stuck = np.nonzero(p == 0)[0][:2]
+    d_llr2 = torch.from_numpy(fr.llr[stuck]).cuda()
+    d_syn2 = torch.from_numpy(fr.syndrome[stuck]).cuda()
+    ws2 = torch.empty(code.workspace_bytes(len(stuck)), dtype=torch.uint8, device="cuda")
+    code.decode(d_llr2, d_syn2, 77, 1, want_posterior=False, workspace=ws2)
+    assert code.iterations_issued(len(stuck), ws2) == 77
 
 
 def test_gpu_argument_errors(B):
