@@ -158,6 +158,12 @@ __device__ __forceinline__ unsigned sign_of(float x) { return __float_as_uint(x)
 // XOR, not OR: the approximate lg2/rcp can make a magnitude that should be +0 come out as -tiny, and the result must
 // stay an odd function of the signs (the syndrome <-> codeword equivalence is bit-exact, tests P5)
 __device__ __forceinline__ float with_sign(float mag, unsigned sg) { return __uint_as_float(__float_as_uint(mag) ^ sg); }
+// check-node rule of a row with one other active edge: partner [+] static term; the sign product includes
+// (-1)^{s_c} via t
+__device__ __forceinline__ float cn_rule(float wv, float tv) {
+    const float qa = fabsf(wv), tt = fabsf(tv);
+    return with_sign(mag_of(qa + tt, fmaf(qa, tt, 1.0f)), sign_of(wv) ^ sign_of(tv));
+}
 #endif
 
 }  // namespace qc

@@ -200,10 +200,11 @@ int qcldpc_llr_init(const float* d_r, const float* d_x, const float* d_sigma2_z,
 }
 
 int qcldpc_pack_bits(const uint8_t* d_hard, int n_frames, int64_t n, int64_t n_bits, uint8_t* d_packed, void* stream) {
-    if (!d_hard || !d_packed || n_frames <= 0 || n_frames > QCLDPC_MAX_FRAMES || n <= 0 || n_bits < 0 || n_bits > n)
+    if (!d_hard || n_frames <= 0 || n_frames > QCLDPC_MAX_FRAMES || n <= 0 || n_bits < 0 || n_bits > n)
         return QCLDPC_ERR_BAD_ARGUMENT;
     const int64_t n_bytes = (n_bits + 7) / 8;
-    if (n_bytes == 0) return QCLDPC_OK;
+    if (n_bytes == 0) return QCLDPC_OK;                          // nothing to write: d_packed may be NULL
+    if (!d_packed) return QCLDPC_ERR_BAD_ARGUMENT;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const dim3 grid((unsigned)((n_bytes + kFrontThreads - 1) / kFrontThreads), (unsigned)n_frames);
     if (n % 8 == 0 && aligned(d_hard, 8)) k_pack_bits<true><<<grid, kFrontThreads, 0, st>>>(d_hard, n, n_bits, n_bytes, d_packed);

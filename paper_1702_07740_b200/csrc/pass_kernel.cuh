@@ -53,12 +53,6 @@ __device__ __forceinline__ unsigned stream_off(const StreamDesc sd, unsigned lan
     return 4u * (sd.base + min(idx, idx - Z));               // idx - Z wraps to a huge value when idx < Z
 }
 
-// check-node rule: partner [+] static term; the sign product includes (-1)^{s_c} via t
-__device__ __forceinline__ float cn_rule(float wv, float tv) {
-    const float qa = fabsf(wv), tt = fabsf(tv);
-    return with_sign(mag_of(qa + tt, fmaf(qa, tt, 1.0f)), sign_of(wv) ^ sign_of(tv));
-}
-
 // One chunk of CH edges starting at edge k0: loads back to back, then the check-node rule, messages to shared memory.
 // MODE 1: all edges are pair edges (k0 >= ng, k0 + CH <= dv); MODE 3: all are edges of triple rows (k0 >= ngh,
 // k0 + CH <= ng); MODE 2: all are gen edges (k0 + CH <= ng); MODE 0: anything (per-edge predicates).

@@ -75,7 +75,7 @@ struct Tuning {
     int pack = 1;                         // QCLDPC_PACK=0: no lane packing in the generic pass
     int fv = 0;                           // QCLDPC_FV=1|2: frames per thread of the generic pass (0: by batch size)
     int loop_graph = 1;                   // QCLDPC_LOOP=stream: one launch per iteration from the host, no graph
-    int body_mult = 1;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations
+    int body_mult = 0;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations (0: by batch size)
 };
 
 // One instantiated decode graph per argument tuple (the kernel parameters are baked into the graph's nodes).
@@ -500,7 +500,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         tn.fv = (fv == 1 || fv == 2) ? fv : 0;
         const char* lp = getenv("QCLDPC_LOOP");
         tn.loop_graph = !(lp && strcmp(lp, "stream") == 0);
-        tn.body_mult = std::min(16, std::max(1, env_int("QCLDPC_BODY", 1)));
+        tn.body_mult = std::min(16, std::max(0, env_int("QCLDPC_BODY", 0)));
     }
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
@@ -566,6 +566,12 @@ int qcldpc_decode(const qcldpc_code_t* code, const float* d_llr, const uint8_t* 
 namespace {
 
 constexpr int kLoopBody = 12;
+// A trip of the WHILE loop costs ~6 us on top of its launches (measured, B200): small batches, whose iterations take
+// about that long, run bodies of 24 iterations, large ones bodies of 12 (a stopped batch then issues fewer empty launches).
+inline int loop_body_len(const qcldpc_code* code, int n_frames) {
+    const int mult = code->tune.body_mult ? code->tune.body_mult : (n_frames <= 8 ? 2 : 1);
+    return kLoopBody * mult;
+}
 
 struct DecodePlan {
     const qcldpc_code* code;
@@ -680,7 +686,7 @@ cudaError_t build_decode_graph(DecodePlan& P, cudaGraphExec_t* exec_out) {
         P.pl.final_mode = false;
         P.pl.prepare_only = 0;
     }
-    const int body = kLoopBody * code->tune.body_mult;
+    const int body = loop_body_len(code, P.n_frames);
     int pre = P.max_iter % body;
     if (pre < 2) pre += body;                                     // every launch of the body carries a check of T >= 1
     const int loops = (P.max_iter - pre) / body;                  // > 0: the caller made sure
@@ -821,7 +827,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     P.merge_check = code->tune.merge_check != 0;
 
     // ---- graph path
-    const int body = kLoopBody * code->tune.body_mult;
+    const int body = loop_body_len(code, n_frames);
     if (code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2) {
         int dev = 0;
         CUDA_TRY(cudaGetDevice(&dev));

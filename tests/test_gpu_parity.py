@@ -408,9 +408,14 @@ def test_device_loop_matches_stream_loop_and_oracle(oracle_lib, B, max_iter, mon
         for a, b in zip(g, s_):
             np.testing.assert_array_equal(a, b)
         ref = oracle_lib.decode(base, Z, llr, syn, max_iter, early)
-        np.testing.assert_array_equal(g[1], ref.iters)
-        np.testing.assert_array_equal(g[2], ref.passed)
-        ok = ref.passed.astype(bool)
+        # past ~50 iterations the two chaotic frames of config 1 stop (or not) on rounding noise: frames on which the
+        # oracle's own float instantiation disagrees with its double one are compared between the two loops only
+        ref32 = oracle_lib.decode(base, Z, llr, syn, max_iter, early, precision=32)
+        stable = (ref32.iters == ref.iters) & (ref32.passed == ref.passed)
+        assert stable.sum() >= len(stable) - 2
+        np.testing.assert_array_equal(g[1][stable], ref.iters[stable])
+        np.testing.assert_array_equal(g[2][stable], ref.passed[stable])
+        ok = ref.passed.astype(bool) & stable
         np.testing.assert_array_equal(g[0][ok], ref.hard[ok])
 
 
