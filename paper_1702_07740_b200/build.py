@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"), os.path.join(CSRC, "check.cuh"),
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"), os.path.join(CSRC, "check.cuh"), os.path.join(CSRC, "pass_il.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
 # (symbol, DV, NG, PCAP): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
 # 11 or 21 edges, 3 of them into the top rows); pass_generic.cu takes any column of degree <= 64
@@ -29,7 +29,8 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 def _units():
     units = [(os.path.join(CSRC, "qcldpc.cu"), os.path.join(OBJDIR, "qcldpc.o"), []),
              (os.path.join(CSRC, "pass_generic.cu"), os.path.join(OBJDIR, "pass_generic.o"), []),
-             (os.path.join(CSRC, "frontend.cu"), os.path.join(OBJDIR, "frontend.o"), [])]
+             (os.path.join(CSRC, "frontend.cu"), os.path.join(OBJDIR, "frontend.o"), []),
+             (os.path.join(CSRC, "pass_il.cu"), os.path.join(OBJDIR, "pass_il.o"), [])]
     for name, dv, ng, pcap in PASS_INSTANCES:
         units.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJDIR, f"{name}.o"),
                       [f"-DPASS_NAME={name}", f"-DPASS_DV={dv}", f"-DPASS_NG={ng}", f"-DPASS_PCAP={pcap}"]))

@@ -18,6 +18,8 @@
 // k_il_check_final (a4; transposes back to the frame-major outputs).
 #pragma once
 
+#include <type_traits>
+
 #include "check.cuh"
 #include "common.cuh"
 
@@ -35,14 +37,32 @@ struct IlArgs {
     unsigned* hardm_final;     // FINAL: decisions of each frame's last iteration, same shape
     uint8_t* d_hard; float* d_post;
     const int* done; const int32_t* iters; int* topbad; int* unsat;
-    int in_buf, out_buf, hin, hout;
-    int Z, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv;
+    const float* q_in; float* q_out;           // regular pass: qb[(t - 1) % 4] -> qb[t % 4]
+    const unsigned* hard_in; unsigned* hard_out;   // hardm[(t - 1) % 3] -> hardm[t % 3]
+    int Z, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;
     int64_t n, m, EZ, mZ, AZ;  // E*Z, mb*Z, A*Z (per group, in lines of 32)
 };
 
-#ifdef __CUDACC__
+struct IlEdgeA { int shift, t_off, p_off, delta; };           // first 16 bytes of EdgeDesc (16-byte aligned copy)
+struct IlEdgeB { int p2_off, delta2; };
+__host__ __device__ inline size_t il_table_bytes(int max_dv, int max_np) {
+    return (size_t)(max_dv > 0 ? max_dv : 1) * (sizeof(IlEdgeA) + sizeof(IlEdgeB) + sizeof(GenDesc)) +
+           (size_t)(max_np > 0 ? max_np : 1) * sizeof(PartnerDesc);
+}
+inline size_t il_smem_bytes(int max_dv, int max_np, int W) {
+    return (il_table_bytes(max_dv, max_np) + 127) / 128 * 128 + (size_t)W * (max_dv > 0 ? max_dv : 1) * kIlGroup * sizeof(float);
+}
+
+
+// kernels and their launcher: only in the family's own translation unit (pass_il.cu defines QC_IL_IMPL)
+#if defined(__CUDACC__) && defined(QC_IL_IMPL)
 __device__ __forceinline__ int il_warp_id() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
 __device__ __forceinline__ int il_wrap(int x, int Z) { return x >= Z ? x - Z : x; }
+// p[idx] of a small kernel-parameter array without indexing the parameter space dynamically
+template <class T>
+__device__ __forceinline__ T il_pick(T const (&p)[4], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : idx == 2 ? p[2] : p[3]; }
+template <class T>
+__device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : p[2]; }
 // line index -> pointer to this lane's float
 __device__ __forceinline__ const float* il_line(const float* base, unsigned line, unsigned lane) {
     return byte_ptr(base, (line * kIlGroup + lane) * 4u);
@@ -122,8 +142,8 @@ __device__ __forceinline__ unsigned il_check_one(const CheckTables& tab, const C
     const RowDesc rd = tab.row[R];
     const int Z = a.Z;
     const int f = min(g * kIlGroup + lane, a.n_frames - 1);
-    const float* __restrict__ qprev = a.qb[(T + 3) % 4] + (int64_t)g * a.EZ * kIlGroup;
-    const unsigned* __restrict__ hm = a.hardm[T % 3] + (int64_t)g * a.AZ;
+    const float* __restrict__ qprev = il_pick(a.qb, (T + 3) % 4) + (int64_t)g * a.EZ * kIlGroup;
+    const unsigned* __restrict__ hm = il_pick(a.hardm, T % 3) + (int64_t)g * a.AZ;
     unsigned par = want ? (c.syn[(int64_t)f * c.m + (int64_t)R * Z + r] & 1u) : 0u;
     unsigned sg = par << 31;
     float num = 0.0f, den = 1.0f;
@@ -213,13 +233,11 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 
 // ---- a1 + a2: the fused pass ------------------------------------------------------------------------------------------
 // CTA = W warps = W consecutive variables of one active column; grid = (columns * tiles [+ check workers], groups).
-// Shared memory: the column's tables (edge, gen, partner descriptors), then the messages m'[W][dv][32].
-// The summation groups of the generic pass: block b = k / 8 of a column's edges belongs to partial sum
-// ((b / G) odd ? G - 1 - b % G : b % G) with G = a.split (4 for long columns, else 1); inside a group increasing k.
+// Shared memory: the column's tables, then the messages m'[W][max_dv][32].
 template <bool FINAL>
 __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                  const CheckArgs chk) {
-    extern __shared__ __align__(16) unsigned char smem_il[];
+    extern __shared__ __align__(128) unsigned char smem_il[];
     pdl_launch();
     if (!FINAL && a.cand_x >= 0 && (int)blockIdx.x >= a.cand_x) {
         pdl_wait();
@@ -231,53 +249,287 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
     const int ca = blockIdx.x / a.tiles;
     const int warp = il_warp_id(), lane = threadIdx.x & 31;
     const int i = (blockIdx.x - ca * a.tiles) * a.W + warp;
-    const ColDesc cd = tab.col[ca];
+    const ColDesc cd = tab.col[ca];                           // tables: constant, not the previous launch's output
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
-    EdgeDesc* const s_e = reinterpret_cast<EdgeDesc*>(smem_il);
-    GenDesc* const s_g = reinterpret_cast<GenDesc*>(s_e + a.max_dv);
-    PartnerDesc* const s_p = reinterpret_cast<PartnerDesc*>(s_g + a.max_dv);
-    for (int k = threadIdx.x; k < dv; k += blockDim.x) s_e[k] = tab.edge[cd.ebeg + k];
+    const int mdv = a.max_dv;
+    IlEdgeA* const s_a = reinterpret_cast<IlEdgeA*>(smem_il);
+    IlEdgeB* const s_b = reinterpret_cast<IlEdgeB*>(s_a + mdv);
+    GenDesc* const s_g = reinterpret_cast<GenDesc*>(s_b + mdv);
+    PartnerDesc* const s_p = reinterpret_cast<PartnerDesc*>(s_g + mdv);
+    for (int k = threadIdx.x; k < dv; k += blockDim.x) {
+        const EdgeDesc d = tab.edge[cd.ebeg + k];
+        s_a[k] = IlEdgeA{d.shift, d.t_off, d.p_off, d.delta};
+        s_b[k] = IlEdgeB{d.p2_off, d.delta2};
+    }
     for (int k = threadIdx.x; k < ng; k += blockDim.x) s_g[k] = tab.gen[cd.gbeg + k];
     for (int k = threadIdx.x; k < cd.np; k += blockDim.x) s_p[k] = tab.partner[cd.pbeg + k];
     const int f = g * kIlGroup + lane;
     const bool in_range = f < a.n_frames;
     const int fc = in_range ? f : a.n_frames - 1;
-    pdl_wait();
+    pdl_wait();                                               // from here on: memory the previous launch wrote
     const int flag = FINAL ? a.iters[fc] : a.done[fc];
     __syncthreads();
     if (i >= Z) return;
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
-    if (!FINAL && !__any_sync(0xffffffffu, live)) return;
+    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped
     const unsigned line_v = (unsigned)(ca * Z + i);
-    const unsigned hm_in = FINAL ? 0u : a.hardm[a.hin][(int64_t)g * a.AZ + line_v];
-    const unsigned xb = (hm_in >> lane) & 1u;
+    const unsigned xb = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v] >> lane) & 1u;
     const float Q = a.qc[((int64_t)g * a.AZ + line_v) * kIlGroup + lane];
     // FINAL: every frame reads the state of its own last iteration, w^(T-1) in buffer (T - 1) mod 4
-    const float* __restrict__ qP = a.qb[FINAL ? ((flag > 0 ? flag : 1) + 3) % 4 : a.in_buf] + (int64_t)g * a.EZ * kIlGroup;
+    const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup;
     const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup;
-    float* const s_m = reinterpret_cast<float*>(smem_il + (size_t)a.max_dv * (sizeof(EdgeDesc) + sizeof(GenDesc)) +
-                                                (size_t)(a.max_dv > 0 ? kMaxPartners : 0) * 0) ;
-    (void)s_m;
-    float* const msg = reinterpret_cast<float*>(s_p + a.split * 0 + (tab.partner ? 0 : 0)) ;
-    (void)msg;
-    // messages of this warp: m[k][lane]
-    float* const m_w = reinterpret_cast<float*>(smem_il + a.cand_x * 0) ;
-    (void)m_w;
-    float* const mm = a_msg_base(smem_il, a) + ((size_t)warp * a.max_dv) * kIlGroup + lane;
-
-    float part[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    float* const mm = reinterpret_cast<float*>(smem_il + (il_table_bytes(mdv, a.max_np) + 127) / 128 * 128) +
+                      (size_t)warp * mdv * kIlGroup + lane;
+    const unsigned ulane = (unsigned)lane;
     unsigned bad = 0;
-    const int G = a.split;
-    auto add_msg = [&](int k, float mk) {
-        mm[k * kIlGroup] = mk;
-        const int b = k / kIlChunk, pos = b % G;
-        const int grp = ((b / G) & 1) ? G - 1 - pos : pos;
-        part[0] += grp == 0 ? mk : 0.0f;
-        part[1] += grp == 1 ? mk : 0.0f;
-        part[2] += grp == 2 ? mk : 0.0f;
-        part[3] += grp == 3 ? mk : 0.0f;
+
+    auto t_line = [&](const IlEdgeA& d) { int r = i - d.shift; r += r < 0 ? Z : 0; return (unsigned)(d.t_off + r); };
+    auto p_line = [&](int off, int delta) { return (unsigned)(off + il_wrap(i + delta, Z)); };
+
+    int k = 0;
+    // gen edges [0, ngh): fold every other edge of the row (the rule is associative); bit 0 of a gen edge's state is its
+    // variable's hard decision: the XOR of the raw words carries sign AND parity
+#pragma unroll 1
+    for (; k < ngh; ++k) {
+        const IlEdgeA d = s_a[k];
+        const GenDesc gd = s_g[k];
+        const float tv = __ldg(il_line(tP, t_line(d), ulane));
+        float num = 0.0f, den = 1.0f;
+        unsigned xa = 0u;
+#pragma unroll 1
+        for (int jb = 0; jb < gd.np; jb += 4) {
+            float pm[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const bool have = jb + u < gd.np;
+                const PartnerDesc p = s_p[gd.pbeg + (have ? jb + u : 0)];
+                pm[u] = have ? __ldg(il_line(qP, p_line(p.off, p.delta), ulane)) : 0.0f;   // +0.0: the identity
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned wb = __float_as_uint(pm[u]);
+                xa ^= wb;
+                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
+            }
+        }
+        if (!FINAL && gd.counter)            // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
+            bad |= (xa ^ xb ^ (__float_as_uint(tv) >> 31)) & 1u;
+        boxplus_acc(fabsf(tv), num, den);
+        mm[k * kIlGroup] = with_sign(mag_of(num, den), (xa ^ __float_as_uint(tv)) & 0x80000000u);
+    }
+    // edges of triple rows [ngh, ng): two partners and an absorbed variable, one fraction, no reciprocal in between
+    auto triple = [&](auto CHc, int k0) {
+        constexpr int CH = decltype(CHc)::value;
+        float tv[CH], pa[CH], pb[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            const IlEdgeA d = s_a[k0 + j];
+            const IlEdgeB e = s_b[k0 + j];
+            tv[j] = __ldg(il_line(tP, t_line(d), ulane));
+            pa[j] = __ldg(il_line(qP, p_line(d.p_off, d.delta), ulane));
+            pb[j] = __ldg(il_line(qP, p_line(e.p2_off, e.delta2), ulane));
+        }
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            const unsigned ua = __float_as_uint(pa[j]), ub = __float_as_uint(pb[j]);
+            const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
+            float num = qa + qb, den = fmaf(qa, qb, 1.0f);
+            boxplus_acc(fabsf(tv[j]), num, den);
+            mm[(k0 + j) * kIlGroup] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j])) & 0x80000000u);
+        }
     };
-    (void)add_msg;
+#pragma unroll 1
+    for (; k + 4 <= ng; k += 4) triple(std::integral_constant<int, 4>{}, k);
+#pragma unroll 1
+    for (; k < ng; ++k) triple(std::integral_constant<int, 1>{}, k);
+    // pair edges [ng, dv): one partner and an absorbed variable
+    auto pair = [&](auto CHc, int k0) {
+        constexpr int CH = decltype(CHc)::value;
+        float tv[CH], wv[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            const IlEdgeA d = s_a[k0 + j];
+            tv[j] = __ldg(il_line(tP, t_line(d), ulane));
+            wv[j] = __ldg(il_line(qP, p_line(d.p_off, d.delta), ulane));
+        }
+#pragma unroll
+        for (int j = 0; j < CH; ++j) mm[(k0 + j) * kIlGroup] = cn_rule(wv[j], tv[j]);
+    };
+#pragma unroll 1
+    for (; k + 8 <= dv; k += 8) pair(std::integral_constant<int, 8>{}, k);
+    if (k + 4 <= dv) { pair(std::integral_constant<int, 4>{}, k); k += 4; }
+#pragma unroll 1
+    for (; k < dv; ++k) pair(std::integral_constant<int, 1>{}, k);
+
+    // variable-node rule.  The messages are added in the order of the generic pass: block b = k / 8 belongs
+    // to partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = a.split; inside a partial sum k increases; the partial
+    // sums meet in the order 0 .. G-1.
+    float sum = 0.0f;
+    const int G = a.split;
+#pragma unroll 1
+    for (int grp = 0; grp < G; ++grp) {
+        float acc = 0.0f;
+#pragma unroll 1
+        for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
+            const int kb = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk;
+            const int ke = min(kb + kIlChunk, dv);
+            for (int kk = kb; kk < ke; ++kk) acc += mm[kk * kIlGroup];
+        }
+        sum = (G == 1) ? acc : sum + acc;
+    }
+    const float L = Q + sum;                                  // L'_v
+    unsigned xh = __float_as_uint(L) >> 31;                   // 0 iff L_v >= 0
+    if (FINAL) {
+        if (live) {
+            const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + i;
+            a.d_hard[vv] = (uint8_t)xh;
+            if (a.d_post) a.d_post[vv] = L * kLn2;
+        } else {
+            xh = (a.hardm[0][(int64_t)g * a.AZ + line_v] >> lane) & 1u;   // t = 0: the decisions of the channel values
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
+        if (lane == 0) a.hardm_final[(int64_t)g * a.AZ + line_v] = mask;
+        return;
+    }
+    const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
+    if (lane == 0) a.hard_out[(int64_t)g * a.AZ + line_v] = mask;
+    if (ng > 0 && bad != 0 && live) a.topbad[f] = 1;
+
+    const bool single = dv == 1;                              // a single edge sends Q itself
+    float* const sp = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * Z + i) * kIlGroup + lane;
+    const unsigned step = (unsigned)Z * kIlGroup * 4u;
+#pragma unroll 4
+    for (int kk = 0; kk < dv; ++kk) {
+        const float Lvc = single ? Q : L - mm[kk * kIlGroup];   // Q + sum_{k' != k} m_k'
+        unsigned wb = __float_as_uint(w_of(Lvc));
+        if (kk < ng) wb = (wb & 0xfffffffeu) | xh;            // gen edge: tag with the hard decision
+        if (live) *byte_ptr(sp, (unsigned)kk * step) = __uint_as_float(wb);
+    }
+}
+
+// ---- a4: every check of every frame on the frame's frozen state (iteration d_iters[f]) -------------------------------
+// Tile = 32 checks of one base row x 32 frames.  Phase 1 (lane = check): frame-major loads of the absorbed variable's
+// LLR and the syndrome bit; phase 2 (lane = frame): the parity, the absorbed variable's decision (L_j = Q_j + m_cj,
+// P:330); phase 3 (lane = check): frame-major stores of that variable's outputs.
+__global__ void __launch_bounds__(256) k_il_check_final(const CheckTables tab, const IlArgs a) {
+    __shared__ float s_q[kIlGroup][33];
+    __shared__ float s_post[kIlGroup][33];
+    __shared__ unsigned char s_syn[kIlGroup][36];
+    __shared__ unsigned char s_xj[kIlGroup][36];
+    const int g = blockIdx.y, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int Z = a.Z;
+    const int tiles32 = (Z + 31) / 32;
+    const int R = blockIdx.x / tiles32, r0 = (blockIdx.x - R * tiles32) * 32;
+    const RowDesc rd = tab.row[R];
+    for (int fl = w; fl < kIlGroup; fl += 8) {
+        const int f = g * kIlGroup + fl, r = r0 + lane;
+        float Qj = 0.0f;
+        unsigned s = 0;
+        if (f < a.n_frames && r < Z) {
+            if (rd.abs_col >= 0)
+                Qj = __ldg(a.llr + (int64_t)f * a.n + (int64_t)rd.abs_col * Z + il_wrap(r + rd.abs_shift, Z));
+            s = a.syn[(int64_t)f * a.m + (int64_t)R * Z + r] & 1u;
+        }
+        s_q[fl][lane] = Qj;
+        s_syn[fl][lane] = (unsigned char)s;
+    }
+    __syncthreads();
+    {
+        const int f = g * kIlGroup + lane;
+        const bool in_range = f < a.n_frames;
+        const int T = a.iters[in_range ? f : a.n_frames - 1];
+        const float* __restrict__ qprev = il_pick(a.qb, ((T > 0 ? T : 1) + 3) % 4) + (int64_t)g * a.EZ * kIlGroup;   // w^(T-1)
+        const unsigned* __restrict__ hm = a.hardm_final + (int64_t)g * a.AZ;
+        int nbad = 0;
+        for (int rl = w; rl < 32; rl += 8) {
+            const int r = r0 + rl;
+            if (r >= Z) break;
+            unsigned par = s_syn[lane][rl];
+            unsigned sg = par << 31;
+            float num = 0.0f, den = 1.0f;
+            for (int k = 0; k < rd.ne; ++k) {
+                const RowEdge re = tab.redge[rd.ebeg + k];
+                const int iv = il_wrap(r + re.shift, Z);
+                par ^= (hm[re.ca * Z + iv] >> lane) & 1u;
+                if (rd.abs_col >= 0) {
+                    unsigned wb = __float_as_uint(__ldg(il_line(qprev, (unsigned)(re.edge * Z + iv), (unsigned)lane)));
+                    sg ^= wb & 0x80000000u;
+                    wb &= rd.gen ? 0x7ffffffeu : 0x7fffffffu;         // gen edges carry a tag in bit 0
+                    boxplus_acc(__uint_as_float(wb), num, den);
+                }
+            }
+            if (rd.abs_col >= 0) {
+                const float Qj = s_q[lane][rl];
+                float Lj = llr_to_log2(Qj);
+                if (T > 0) Lj += with_sign(mag_of(num, den), sg);       // L'_j = Q'_j + m'_cj
+                const unsigned xj = __float_as_uint(Lj) >> 31;
+                s_xj[lane][rl] = (unsigned char)xj;
+                s_post[lane][rl] = T > 0 ? Lj * kLn2 : Qj;
+                par ^= xj;
+            }
+            nbad += in_range ? (int)par : 0;
+        }
+        if (nbad) atomicAdd(a.unsat + f, nbad);
+    }
+    if (rd.abs_col < 0) return;                               // block-uniform
+    __syncthreads();
+    for (int fl = w; fl < kIlGroup; fl += 8) {
+        const int f = g * kIlGroup + fl, r = r0 + lane;
+        if (f < a.n_frames && r < Z) {
+            const int64_t v = (int64_t)f * a.n + (int64_t)rd.abs_col * Z + il_wrap(r + rd.abs_shift, Z);
+            a.d_hard[v] = s_xj[fl][lane];
+            if (a.d_post) a.d_post[v] = s_post[fl][lane];
+        }
+    }
+}
+#endif
+
+// ---- host side --------------------------------------------------------------------------------------------------------
+struct IlLaunch {
+    PassTables tab; CheckTables ctab; IlArgs args; cudaStream_t stream;
+    const CheckArgs* check;    // the early-exit check this launch carries in its grid (NULL: none)
+    bool final_mode; int n_sm, prepare_only;
+};
+
+// warps per CTA: the width whose last tile idles the fewest warps, near 8, within the shared-memory budget
+inline int il_pick_w(int Z, int max_dv, int max_np) {
+    int best = 1;
+    double best_cost = 1e30;
+    for (int w = 2; w <= 16; ++w) {
+        if (il_smem_bytes(max_dv, max_np, w) > 200 * 1024) break;
+        const int tiles = (Z + w - 1) / w;
+        const double waste = (double)(tiles * w - Z) / (double)(tiles * w);
+        const double cost = waste + 0.01 * (w > 8 ? w - 8 : 8 - w);   // ties: close to 8 warps
+        if (cost < best_cost - 1e-12) { best_cost = cost; best = w; }
+    }
+    return best;
+}
+
+#ifdef QC_IL_IMPL
+inline void launch_pass_il(const IlLaunch& L) {
+    IlArgs args = L.args;
+    const size_t smem = il_smem_bytes(args.max_dv, args.max_np, args.W);
+    static thread_local int attr_dev = -1;                  // the attribute is per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (attr_dev != dev) {
+        cudaFuncSetAttribute(k_pass_il<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        attr_dev = dev;
+    }
+    if (L.prepare_only) return;
+    const bool with_check = !L.final_mode && L.check != nullptr;
+    const int work = args.n_cols * args.tiles;
+    const int extra = with_check ? (2 * L.n_sm + args.n_groups - 1) / args.n_groups : 0;
+    args.cand_x = with_check ? work : -1;
+    static const CheckTables no_tab{nullptr, nullptr};
+    static const CheckArgs no_args{};
+    const dim3 grid(work + extra, args.n_groups), block(32 * args.W);
+    if (L.final_mode)
+        k_pass_il<true><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
+    else
+        launch_pdl(k_pass_il<false>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
+                   with_check ? *L.check : no_args);
 }
 #endif
 

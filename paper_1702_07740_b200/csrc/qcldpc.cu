@@ -28,6 +28,7 @@
 // pass t and touches nothing that pass writes: check.cuh has the timeline.
 #include "check.cuh"
 #include "common.cuh"
+#include "pass_il.cuh"
 
 #include <algorithm>
 #include <cstdio>
@@ -44,6 +45,11 @@ void launch_pass_dv21_ng3(const PassLaunch&);
 void launch_pass_generic(const PassLaunch&);
 size_t launch_pass_dv11_ng3_table(const HostTables&, void*);
 size_t launch_pass_dv21_ng3_table(const HostTables&, void*);
+// the frame-interleaved family (pass_il.cu)
+void launch_pass_il_entry(const IlLaunch&);
+void launch_il_init(const PassTables&, const CheckTables&, const IlArgs&, cudaStream_t);
+void launch_il_cand(const CheckTables&, const CheckArgs&, const IlArgs&, int blocks, cudaStream_t);
+void launch_il_check_final(const CheckTables&, const IlArgs&, cudaStream_t);
 }  // namespace qc
 
 using namespace qc;
@@ -76,6 +82,7 @@ struct Tuning {
     int fv = 0;                           // QCLDPC_FV=1|2: frames per thread of the generic pass (0: by batch size)
     int loop_graph = 1;                   // QCLDPC_LOOP=stream: one launch per iteration from the host, no graph
     int body_mult = 0;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations (0: by batch size)
+    int il = 1;                           // QCLDPC_IL=0: never the frame-interleaved family; 2: for every batch size
 };
 
 // One instantiated decode graph per argument tuple (the kernel parameters are baked into the graph's nodes).
@@ -104,6 +111,11 @@ struct qcldpc_code {
     std::vector<RowEdge> redge;
     EdgeDesc* d_edge = nullptr; GenDesc* d_gen = nullptr; PartnerDesc* d_partner = nullptr; ColDesc* d_col = nullptr;
     RowDesc* d_row = nullptr; RowEdge* d_redge = nullptr;
+    // frame-interleaved family (pass_il.cuh): the same tables with run length Z (a run is Z lines of 32 frames)
+    std::vector<EdgeDesc> edge_il; std::vector<PartnerDesc> partner_il;
+    EdgeDesc* d_edge_il = nullptr; PartnerDesc* d_partner_il = nullptr;
+    bool il_ok = false;                   // the code fits the family's 32-bit byte offsets
+    int il_w = 8;                         // warps per CTA of k_pass_il
     PassLauncher launcher = nullptr;
     std::vector<char> exact;              // kernel-parameter table of the exact family (empty: generic kernel)
     int n_sm = 148;
@@ -276,20 +288,47 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Workspace {
     float* qbuf[4]; float* t; uint8_t* hardbuf[3]; int* done; int* unsat; int* topbad; int* fullbad; unsigned* ticket;
+    // frame-interleaved family: LLRs of the active variables, decisions as one word per variable (3 + the final ones)
+    bool il; int n_groups; float* qc; unsigned* hardm[4];
     size_t bytes;
 };
+
+// The frame-interleaved family decodes batches that fill its groups of 32 frames (codes outside the exact families).
+bool use_il(const qcldpc_code* code, int n_frames) {
+    if (!code->il_ok || code->tune.il == 0) return false;
+    if (code->tune.il == 2) return true;
+    const int groups = (n_frames + kIlGroup - 1) / kIlGroup;
+    return n_frames >= 24 && 4 * n_frames >= 3 * groups * kIlGroup;      // at least 3/4 of the lanes carry a frame
+}
 
 Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
     Workspace w;
     char* p = static_cast<char*>(base);
     size_t off = 0;
+    w.il = use_il(code, n_frames);
+    w.n_groups = (n_frames + kIlGroup - 1) / kIlGroup;
+    w.qc = nullptr;
+    for (int b = 0; b < 4; ++b) w.hardm[b] = nullptr;
+    for (int b = 0; b < 3; ++b) w.hardbuf[b] = nullptr;
+    const size_t fbytes = align_up((size_t)n_frames * sizeof(int), 256);
+    if (w.il) {
+        const size_t lines = (size_t)w.n_groups * kIlGroup * sizeof(float);            // bytes per line index
+        const size_t qbytes = align_up(lines * code->n_act_edges * code->Z, 256);
+        const size_t tbytes = align_up(lines * code->mb * code->Z, 256);
+        const size_t cbytes = align_up(lines * code->n_act_cols * code->Z, 256);
+        const size_t hbytes = align_up((size_t)w.n_groups * code->n_act_cols * code->Z * sizeof(unsigned), 256);
+        for (int b = 0; b < 4; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
+        w.t = reinterpret_cast<float*>(p + off); off += tbytes;
+        w.qc = reinterpret_cast<float*>(p + off); off += cbytes;
+        for (int b = 0; b < 4; ++b) { w.hardm[b] = reinterpret_cast<unsigned*>(p + off); off += hbytes; }
+    } else {
     const size_t qbytes = align_up((size_t)n_frames * code->n_act_edges * code->Zs * sizeof(float), 256);
     const size_t tbytes = align_up((size_t)n_frames * code->mb * code->Zs * sizeof(float), 256);
     const size_t hbytes = align_up((size_t)n_frames * code->n_act_cols * code->Zs, 256);
-    const size_t fbytes = align_up((size_t)n_frames * sizeof(int), 256);
     for (int b = 0; b < 4; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
     w.t = reinterpret_cast<float*>(p + off); off += tbytes;
     for (int b = 0; b < 3; ++b) { w.hardbuf[b] = reinterpret_cast<uint8_t*>(p + off); off += hbytes; }
+    }
     w.done = reinterpret_cast<int*>(p + off); off += 2 * fbytes;       // two versions of n_frames ints, contiguous
     w.unsat = reinterpret_cast<int*>(p + off); off += fbytes;
     w.topbad = reinterpret_cast<int*>(p + off); off += 3 * fbytes;     // three slots of n_frames ints, contiguous
@@ -501,7 +540,22 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         const char* lp = getenv("QCLDPC_LOOP");
         tn.loop_graph = !(lp && strcmp(lp, "stream") == 0);
         tn.body_mult = std::min(16, std::max(0, env_int("QCLDPC_BODY", 0)));
+        tn.il = std::min(2, std::max(0, env_int("QCLDPC_IL", 1)));
     }
+
+    // frame-interleaved family: offsets in lines of 32 frames, runs of exactly Z lines
+    code->edge_il = code->edge;
+    for (EdgeDesc& d : code->edge_il) {
+        d.t_off = d.t_off / Zs * Z;
+        if (d.p_off >= 0) d.p_off = d.p_off / Zs * Z;
+        if (d.p2_off >= 0) d.p2_off = d.p2_off / Zs * Z;
+    }
+    code->partner_il = code->partner;
+    for (PartnerDesc& d : code->partner_il) d.off = d.off / Zs * Z;
+    code->il_ok = !exact && code->n_act_cols > 0 && (int64_t)code->n_act_edges * Z < ((int64_t)1 << 25) &&
+                  (int64_t)mb * Z < ((int64_t)1 << 25) &&
+                  il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
+    code->il_w = il_pick_w(Z, code->max_dv, max_np);
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
         const size_t bytes = std::max<size_t>(vec.size(), 1) * sizeof(vec[0]);
@@ -516,6 +570,8 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     if (e == cudaSuccess) e = upload(code->col, &code->d_col);
     if (e == cudaSuccess) e = upload(code->row, &code->d_row);
     if (e == cudaSuccess) e = upload(code->redge, &code->d_redge);
+    if (e == cudaSuccess && code->il_ok) e = upload(code->edge_il, &code->d_edge_il);
+    if (e == cudaSuccess && code->il_ok) e = upload(code->partner_il, &code->d_partner_il);
     int dev = 0;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&code->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -531,6 +587,7 @@ void qcldpc_code_destroy(qcldpc_code_t* code) {
     if (code->cap_body) cudaStreamDestroy(code->cap_body);
     cudaFree(code->d_edge); cudaFree(code->d_gen); cudaFree(code->d_partner); cudaFree(code->d_col);
     cudaFree(code->d_row); cudaFree(code->d_redge);
+    cudaFree(code->d_edge_il); cudaFree(code->d_partner_il);
     delete code;
 }
 
@@ -584,6 +641,7 @@ struct DecodePlan {
     bool merge_check, flip;
     int* ctl;
     int32_t* d_iters; uint8_t* d_pass;
+    bool il; IlLaunch ill;                               // frame-interleaved family (pass_il.cuh)
 
     int* done_ver(int t) const { return w.done + (size_t)(t & 1) * n_frames; }
     int* topbad_slot(int T) const { return w.topbad + (size_t)(((T % 3) + 3) % 3) * n_frames; }
@@ -596,6 +654,11 @@ void issue_prologue(DecodePlan& P, cudaStream_t st) {
     k_reset<<<P.fblocks, 128, 0, st>>>(P.w.done, P.w.unsat, P.w.topbad, P.w.fullbad, P.w.ticket, P.d_iters, P.d_pass,
                                        P.n_frames, P.max_iter);
     ++g_launches;
+    if (P.il) {
+        launch_il_init(P.ill.tab, P.ctab, P.ill.args, st);
+        g_launches += 2;
+        return;
+    }
     if (P.code->n_act_cols > 0) {
         k_init_cols<<<dim3(P.tiles1 * P.code->n_act_cols, P.n_frames), kThreads, 0, st>>>(P.ptab, P.ia);
         ++g_launches;
@@ -619,7 +682,8 @@ void set_check(DecodePlan& P, int T, int t, const int* t_base, const int* skip) 
 void launch_check(DecodePlan& P, cudaStream_t st, int T, int t, const int* t_base, const int* skip) {
     set_check(P, T, t, t_base, skip);
     const int pk = prof_begin(1, st);
-    launch_pdl(k_cand, dim3(P.cand_blocks), dim3(kThreads), 0, st, P.ctab, P.ca);
+    if (P.il) launch_il_cand(P.ctab, P.ca, P.ill.args, P.cand_blocks, st);
+    else launch_pdl(k_cand, dim3(P.cand_blocks), dim3(kThreads), 0, st, P.ctab, P.ca);
     prof_end(pk, st);
     ++g_launches;
 }
@@ -631,7 +695,21 @@ void issue_iteration(DecodePlan& P, cudaStream_t st, int t, const int* t_base) {
     const qcldpc_code* code = P.code;
     const bool want = t_base ? (P.early_stop != 0) : P.check_wanted(t - 2);
     const bool merged = P.merge_check && want && code->n_act_cols > 0;
-    if (code->n_act_cols > 0) {
+    if (P.il) {
+        IlLaunch& L = P.ill;
+        L.stream = st;
+        L.final_mode = false;
+        L.args.q_in = P.w.qbuf[(t - 1) % 4]; L.args.q_out = P.w.qbuf[t % 4];
+        L.args.hard_in = P.w.hardm[(t - 1) % 3]; L.args.hard_out = P.w.hardm[t % 3];
+        L.args.topbad = P.topbad_slot(t - 1);
+        L.args.done = P.done_ver(t);
+        L.check = nullptr;
+        if (merged) { set_check(P, t - 2, t, t_base, nullptr); L.check = &P.ca; }
+        const int pk = prof_begin(0, st);
+        launch_pass_il_entry(L);
+        prof_end(pk, st);
+        ++g_launches;
+    } else if (code->n_act_cols > 0) {
         PassLaunch& pl = P.pl;
         pl.stream = st;
         pl.args.in_buf = (t - 1) % 4; pl.args.out_buf = t % 4;
@@ -657,6 +735,23 @@ void issue_iteration(DecodePlan& P, cudaStream_t st, int t, const int* t_base) {
 // did not stop)
 void issue_epilogue(DecodePlan& P, cudaStream_t st, int t_last, const int* skip) {
     if (t_last >= 2 && P.check_wanted(t_last - 1)) launch_check(P, st, t_last - 1, t_last + 1, nullptr, skip);
+    if (P.il) {
+        IlLaunch& L = P.ill;
+        L.stream = st;
+        L.check = nullptr;
+        L.args.hardm_final = P.w.hardm[0];               // max_iter = 0: the decisions of k_il_init_cols
+        if (P.max_iter > 0) {
+            L.args.hardm_final = P.w.hardm[3];
+            L.final_mode = true;
+            launch_pass_il_entry(L);
+            L.final_mode = false;
+            ++g_launches;
+        }
+        launch_il_check_final(P.ctab, L.args, st);
+        k_flags_final<<<P.fblocks, 128, 0, st>>>(P.w.unsat, P.d_pass, P.n_frames);
+        g_launches += 2;
+        return;
+    }
     if (P.code->n_act_cols > 0 && P.max_iter > 0) {
         P.pl.stream = st;
         P.pl.final_mode = true;
@@ -679,7 +774,11 @@ cudaError_t build_decode_graph(DecodePlan& P, cudaGraphExec_t* exec_out) {
     if (!code->cap_main) e = cudaStreamCreateWithFlags(&code->cap_main, cudaStreamNonBlocking);
     if (e == cudaSuccess && !code->cap_body) e = cudaStreamCreateWithFlags(&code->cap_body, cudaStreamNonBlocking);
     if (e != cudaSuccess) return e;
-    if (code->n_act_cols > 0) {                                   // kernel attributes are set outside the capture
+    if (P.il) {                                                   // kernel attributes are set outside the capture
+        P.ill.prepare_only = 1;
+        launch_pass_il_entry(P.ill);
+        P.ill.prepare_only = 0;
+    } else if (code->n_act_cols > 0) {
         P.pl.prepare_only = 1;
         P.pl.final_mode = false; code->launcher(P.pl);
         P.pl.final_mode = true; code->launcher(P.pl);
@@ -825,6 +924,26 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     const int cand_per_sm = code->tune.cand_per_sm ? code->tune.cand_per_sm : (n_frames <= 8 ? 1 : 4);
     P.cand_blocks = std::max(1, std::min(code->n_sm * cand_per_sm, code->mb * P.tiles1));
     P.merge_check = code->tune.merge_check != 0;
+    P.il = w.il;
+    if (P.il) {
+        const int64_t EZ = (int64_t)code->n_act_edges * Z, mZ = (int64_t)code->mb * Z, AZ = (int64_t)code->n_act_cols * Z;
+        IlArgs ia{};
+        ia.llr = d_llr; ia.syn = d_syndrome;
+        for (int b = 0; b < 4; ++b) ia.qb[b] = w.qbuf[b];
+        ia.t = w.t; ia.qc = w.qc;
+        for (int b = 0; b < 3; ++b) ia.hardm[b] = w.hardm[b];
+        ia.hardm_final = w.hardm[3];
+        ia.d_hard = d_hard; ia.d_post = d_posterior;
+        ia.done = w.done; ia.iters = d_iters; ia.topbad = nullptr; ia.unsat = w.unsat;
+        ia.Z = Z; ia.W = code->il_w; ia.tiles = (Z + code->il_w - 1) / code->il_w;
+        ia.n_frames = n_frames; ia.n_groups = w.n_groups; ia.n_cols = code->n_act_cols; ia.mb = code->mb;
+        ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
+        ia.max_np = code->max_np;
+        ia.n = code->n; ia.m = code->m; ia.EZ = EZ; ia.mZ = mZ; ia.AZ = AZ;
+        P.ill = IlLaunch{PassTables{code->d_edge_il, code->d_gen, code->d_partner_il, code->d_col}, P.ctab, ia, st,
+                         nullptr, false, code->n_sm, 0};
+        P.cand_blocks = std::max(1, std::min(code->n_sm * 2, code->mb * Z / 8 + 1));
+    }
 
     // ---- graph path
     const int body = loop_body_len(code, n_frames);
