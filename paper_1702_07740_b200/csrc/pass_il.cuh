@@ -40,17 +40,26 @@ struct IlArgs {
     const float* q_in; float* q_out;           // regular pass: qb[(t - 1) % 4] -> qb[t % 4]
     const unsigned* hard_in; unsigned* hard_out;   // hardm[(t - 1) % 3] -> hardm[t % 3]
     int Z, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;
+    int tp, ctas_per_col;      // k_pass_il: tiles per CTA (one table load serves them all), CTAs per column
+    const uint4* blob; int blob16;   // per-column tables in shared-memory layout, blob16 16-byte words per column
     int64_t n, m, EZ, mZ, AZ;  // E*Z, mb*Z, A*Z (per group, in lines of 32)
 };
 
+// Per-column table blob, the same bytes in global and in shared memory, fixed stride, so that a CTA copies it in ONE
+// round trip without first reading where it is: header, then [max_dv] IlEdgeA, [max_dv] GenDesc, [max_dv] IlEdgeB,
+// [max_np] PartnerDesc.
+struct IlColHdr { int col, ebeg, dv, ng, ngh, np, pad0, pad1; };
 struct IlEdgeA { int shift, t_off, p_off, delta; };           // first 16 bytes of EdgeDesc (16-byte aligned copy)
 struct IlEdgeB { int p2_off, delta2; };
 __host__ __device__ inline size_t il_table_bytes(int max_dv, int max_np) {
-    return (size_t)(max_dv > 0 ? max_dv : 1) * (sizeof(IlEdgeA) + sizeof(IlEdgeB) + sizeof(GenDesc)) +
-           (size_t)(max_np > 0 ? max_np : 1) * sizeof(PartnerDesc);
+    const size_t b = sizeof(IlColHdr) + (size_t)(max_dv > 0 ? max_dv : 1) * (sizeof(IlEdgeA) + sizeof(IlEdgeB) + sizeof(GenDesc)) +
+                     (size_t)(max_np > 0 ? max_np : 1) * sizeof(PartnerDesc);
+    return (b + 15) / 16 * 16;
 }
 inline size_t il_smem_bytes(int max_dv, int max_np, int W) {
-    return (il_table_bytes(max_dv, max_np) + 127) / 128 * 128 + (size_t)W * (max_dv > 0 ? max_dv : 1) * kIlGroup * sizeof(float);
+    return (il_table_bytes(max_dv, max_np) + 127) / 128 * 128 +
+           (size_t)W * ((max_dv > 0 ? max_dv : 1) + 8) * kIlGroup * sizeof(float) +   // messages + 2 x 4 partial sums per variable
+           128;                                                                        // handshake flags of the warp pairs
 }
 
 
@@ -232,11 +241,18 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 }
 
 // ---- a1 + a2: the fused pass ------------------------------------------------------------------------------------------
-// CTA = W warps = W consecutive variables of one active column; grid = (columns * tiles [+ check workers], groups).
-// Shared memory: the column's tables, then the messages m'[W][max_dv][32].
-template <bool FINAL>
-__global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
+// CTA = W variables of one active column x H warps per variable; grid = (columns * tiles [+ check workers], groups).
+// Shared memory: the column's tables, the messages m'[W][max_dv][32], the partial sums [W][4][32].
+// The messages of a column are added as the generic pass adds them: block b = k / 8 of the column's edges belongs to
+// partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = 4 for long columns (max_dv > 16), else 1; inside a partial sum k
+// increases; the partial sums meet in the order 0 .. G-1.  H = 2 (G = 4): warp h of a variable owns the partial sums
+// 2h and 2h + 1 -- and with them the edges, their loads, their messages and their stores --, so a column of degree 60 is
+// two chains of 28 and 32 edges and twice as many warps keep loads in flight; the two warps meet once, at a named
+// barrier, to exchange their partial sums.  H = 1 (G = 1): one warp, one sum.
+template <bool FINAL, int H, int GPW>
+__global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                  const CheckArgs chk) {
+    constexpr int G = H * GPW;
     extern __shared__ __align__(128) unsigned char smem_il[];
     pdl_launch();
     if (!FINAL && a.cand_x >= 0 && (int)blockIdx.x >= a.cand_x) {
@@ -246,51 +262,60 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
         return;
     }
     const int Z = a.Z, g = blockIdx.y;
-    const int ca = blockIdx.x / a.tiles;
+    const int ca = blockIdx.x / a.ctas_per_col;
+    const int tile0 = (blockIdx.x - ca * a.ctas_per_col) * a.tp;
     const int warp = il_warp_id(), lane = threadIdx.x & 31;
-    const int i = (blockIdx.x - ca * a.tiles) * a.W + warp;
-    const ColDesc cd = tab.col[ca];                           // tables: constant, not the previous launch's output
-    const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
+    const int var = warp / H, h = warp - var * H;            // variable of the tile, warp of the variable
     const int mdv = a.max_dv;
-    IlEdgeA* const s_a = reinterpret_cast<IlEdgeA*>(smem_il);
-    IlEdgeB* const s_b = reinterpret_cast<IlEdgeB*>(s_a + mdv);
-    GenDesc* const s_g = reinterpret_cast<GenDesc*>(s_b + mdv);
-    PartnerDesc* const s_p = reinterpret_cast<PartnerDesc*>(s_g + mdv);
-    for (int k = threadIdx.x; k < dv; k += blockDim.x) {
-        const EdgeDesc d = tab.edge[cd.ebeg + k];
-        s_a[k] = IlEdgeA{d.shift, d.t_off, d.p_off, d.delta};
-        s_b[k] = IlEdgeB{d.p2_off, d.delta2};
+    // prologue: the column's tables (constant: not the previous launch's output) in one round trip
+    {
+        const uint4* __restrict__ src = a.blob + (size_t)ca * a.blob16;
+        uint4* dst = reinterpret_cast<uint4*>(smem_il);
+        for (int k = threadIdx.x; k < a.blob16; k += blockDim.x) dst[k] = __ldg(src + k);
     }
-    for (int k = threadIdx.x; k < ng; k += blockDim.x) s_g[k] = tab.gen[cd.gbeg + k];
-    for (int k = threadIdx.x; k < cd.np; k += blockDim.x) s_p[k] = tab.partner[cd.pbeg + k];
+    float* const msg_base = reinterpret_cast<float*>(smem_il + (il_table_bytes(mdv, a.max_np) + 127) / 128 * 128);
+    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdv + 8) * kIlGroup);
+    if (threadIdx.x < 32) s_flag[threadIdx.x] = 0;
     const int f = g * kIlGroup + lane;
     const bool in_range = f < a.n_frames;
     const int fc = in_range ? f : a.n_frames - 1;
     pdl_wait();                                               // from here on: memory the previous launch wrote
     const int flag = FINAL ? a.iters[fc] : a.done[fc];
     __syncthreads();
-    if (i >= Z) return;
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
-    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped
-    const unsigned line_v = (unsigned)(ca * Z + i);
-    const unsigned xb = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v] >> lane) & 1u;
-    const float Q = a.qc[((int64_t)g * a.AZ + line_v) * kIlGroup + lane];
+    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped (both warps of a
+                                                              // variable see the same frames and leave together)
+    const IlColHdr cd = *reinterpret_cast<const IlColHdr*>(smem_il);
+    const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
+    const IlEdgeA* const s_a = reinterpret_cast<const IlEdgeA*>(smem_il + sizeof(IlColHdr));
+    const GenDesc* const s_g = reinterpret_cast<const GenDesc*>(s_a + mdv);
+    const IlEdgeB* const s_b = reinterpret_cast<const IlEdgeB*>(s_g + mdv);
+    const PartnerDesc* const s_p = reinterpret_cast<const PartnerDesc*>(s_b + mdv);
     // FINAL: every frame reads the state of its own last iteration, w^(T-1) in buffer (T - 1) mod 4
     const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup;
     const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup;
-    float* const mm = reinterpret_cast<float*>(smem_il + (il_table_bytes(mdv, a.max_np) + 127) / 128 * 128) +
-                      (size_t)warp * mdv * kIlGroup + lane;
+    float* const mm = msg_base + (size_t)var * mdv * kIlGroup + lane;
+    float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)var * 8 * kIlGroup + lane;   // partial sums, 2 buffers
     const unsigned ulane = (unsigned)lane;
+    const unsigned step = (unsigned)Z * kIlGroup * 4u;
+    const bool single = dv == 1;                              // a single edge sends Q itself (P:330)
+
+#pragma unroll 1
+    for (int tt = 0; tt < a.tp; ++tt) {
+    const int i = (tile0 + tt) * a.W + var;
+    if (tile0 + tt >= a.tiles || i >= Z) break;               // both warps of a variable leave together
+    const unsigned line_v = (unsigned)(ca * Z + i);
+    const unsigned xb = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v] >> lane) & 1u;
+    const float Q = a.qc[((int64_t)g * a.AZ + line_v) * kIlGroup + lane];
+    float* const xch = xch0 + (tt & 1) * 4 * kIlGroup;
     unsigned bad = 0;
 
     auto t_line = [&](const IlEdgeA& d) { int r = i - d.shift; r += r < 0 ? Z : 0; return (unsigned)(d.t_off + r); };
     auto p_line = [&](int off, int delta) { return (unsigned)(off + il_wrap(i + delta, Z)); };
 
-    int k = 0;
-    // gen edges [0, ngh): fold every other edge of the row (the rule is associative); bit 0 of a gen edge's state is its
+    // gen edge: fold every other edge of the row (the rule is associative); bit 0 of a gen edge's state is its
     // variable's hard decision: the XOR of the raw words carries sign AND parity
-#pragma unroll 1
-    for (; k < ngh; ++k) {
+    auto gen_edge = [&](int k, float& acc) {
         const IlEdgeA d = s_a[k];
         const GenDesc gd = s_g[k];
         const float tv = __ldg(il_line(tP, t_line(d), ulane));
@@ -315,10 +340,12 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
         if (!FINAL && gd.counter)            // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
             bad |= (xa ^ xb ^ (__float_as_uint(tv) >> 31)) & 1u;
         boxplus_acc(fabsf(tv), num, den);
-        mm[k * kIlGroup] = with_sign(mag_of(num, den), (xa ^ __float_as_uint(tv)) & 0x80000000u);
-    }
-    // edges of triple rows [ngh, ng): two partners and an absorbed variable, one fraction, no reciprocal in between
-    auto triple = [&](auto CHc, int k0) {
+        const float mk = with_sign(mag_of(num, den), (xa ^ __float_as_uint(tv)) & 0x80000000u);
+        mm[k * kIlGroup] = mk;
+        acc += mk;
+    };
+    // edges of triple rows: two partners and an absorbed variable, one fraction, no reciprocal in between
+    auto triple = [&](auto CHc, int k0, float& acc) {
         constexpr int CH = decltype(CHc)::value;
         float tv[CH], pa[CH], pb[CH];
 #pragma unroll
@@ -335,15 +362,13 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
             const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
             float num = qa + qb, den = fmaf(qa, qb, 1.0f);
             boxplus_acc(fabsf(tv[j]), num, den);
-            mm[(k0 + j) * kIlGroup] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j])) & 0x80000000u);
+            const float mk = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j])) & 0x80000000u);
+            mm[(k0 + j) * kIlGroup] = mk;
+            acc += mk;
         }
     };
-#pragma unroll 1
-    for (; k + 4 <= ng; k += 4) triple(std::integral_constant<int, 4>{}, k);
-#pragma unroll 1
-    for (; k < ng; ++k) triple(std::integral_constant<int, 1>{}, k);
-    // pair edges [ng, dv): one partner and an absorbed variable
-    auto pair = [&](auto CHc, int k0) {
+    // pair edges: one partner and an absorbed variable
+    auto pair = [&](auto CHc, int k0, float& acc) {
         constexpr int CH = decltype(CHc)::value;
         float tv[CH], wv[CH];
 #pragma unroll
@@ -353,33 +378,72 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
             wv[j] = __ldg(il_line(qP, p_line(d.p_off, d.delta), ulane));
         }
 #pragma unroll
-        for (int j = 0; j < CH; ++j) mm[(k0 + j) * kIlGroup] = cn_rule(wv[j], tv[j]);
-    };
-#pragma unroll 1
-    for (; k + 8 <= dv; k += 8) pair(std::integral_constant<int, 8>{}, k);
-    if (k + 4 <= dv) { pair(std::integral_constant<int, 4>{}, k); k += 4; }
-#pragma unroll 1
-    for (; k < dv; ++k) pair(std::integral_constant<int, 1>{}, k);
-
-    // variable-node rule.  The messages are added in the order of the generic pass: block b = k / 8 belongs
-    // to partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = a.split; inside a partial sum k increases; the partial
-    // sums meet in the order 0 .. G-1.
-    float sum = 0.0f;
-    const int G = a.split;
-#pragma unroll 1
-    for (int grp = 0; grp < G; ++grp) {
-        float acc = 0.0f;
-#pragma unroll 1
-        for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
-            const int kb = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk;
-            const int ke = min(kb + kIlChunk, dv);
-            for (int kk = kb; kk < ke; ++kk) acc += mm[kk * kIlGroup];
+        for (int j = 0; j < CH; ++j) {
+            const float mk = cn_rule(wv[j], tv[j]);
+            mm[(k0 + j) * kIlGroup] = mk;
+            acc += mk;
         }
-        sum = (G == 1) ? acc : sum + acc;
+    };
+    using I1 = std::integral_constant<int, 1>;
+    using I4 = std::integral_constant<int, 4>;
+    using I8 = std::integral_constant<int, 8>;
+    // block kb .. ke of this warp's partial sum `gi`: class-pure segments (gen, triple, pair), the largest chunks first
+    auto block_of = [&](int rnd, int gi, int& kb, int& ke) {
+        const int grp = h * GPW + gi;
+        kb = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk;
+        ke = min(kb + kIlChunk, dv);
+    };
+    float part[GPW];
+#pragma unroll
+    for (int gi = 0; gi < GPW; ++gi) part[gi] = 0.0f;
+#pragma unroll 1
+    for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
+#pragma unroll
+        for (int gi = 0; gi < GPW; ++gi) {
+            int k, ke;
+            block_of(rnd, gi, k, ke);
+            float acc = part[gi];
+            const int e1 = min(ke, ngh), e3 = min(ke, ng);
+            for (; k < e1; ++k) gen_edge(k, acc);
+            if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
+            if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
+            for (; k < e3; ++k) triple(I1{}, k, acc);
+            if (k + 8 <= ke) { pair(I8{}, k, acc); k += 8; }
+            if (k + 4 <= ke) { pair(I4{}, k, acc); k += 4; }
+            for (; k < ke; ++k) pair(I1{}, k, acc);
+            part[gi] = acc;
+        }
+    }
+
+    // variable-node rule: the partial sums meet in the order 0 .. G-1
+    float sum;
+    if (H == 1) {
+        sum = part[0];
+        if (GPW > 1) {
+            sum = 0.0f;
+#pragma unroll
+            for (int gi = 0; gi < GPW; ++gi) sum += part[gi];
+        }
+    } else {
+#pragma unroll
+        for (int gi = 0; gi < GPW; ++gi) xch[(h * GPW + gi) * kIlGroup] = part[gi];
+        // the two warps of this variable meet here: release / acquire on a counter in shared memory (a named barrier
+        // per variable would pin all 16 hardware barriers of the CTA); tile tt + 1 uses the other buffer of partial
+        // sums, and a warp cannot be more than one exchange ahead of its partner
+        __syncwarp();
+        if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + var * 2 + h), "r"(tt + 1) : "memory");
+        int seen;
+        do {
+            asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + var * 2 + (1 - h)) : "memory");
+        } while (seen < tt + 1);
+        sum = 0.0f;
+#pragma unroll
+        for (int gg = 0; gg < G; ++gg) sum += xch[gg * kIlGroup];
     }
     const float L = Q + sum;                                  // L'_v
     unsigned xh = __float_as_uint(L) >> 31;                   // 0 iff L_v >= 0
     if (FINAL) {
+        if (h != 0) continue;
         if (live) {
             const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + i;
             a.d_hard[vv] = (uint8_t)xh;
@@ -389,22 +453,42 @@ __global__ void __launch_bounds__(512) k_pass_il(const PassTables tab, const IlA
         }
         const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
         if (lane == 0) a.hardm_final[(int64_t)g * a.AZ + line_v] = mask;
-        return;
+        continue;
     }
-    const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
-    if (lane == 0) a.hard_out[(int64_t)g * a.AZ + line_v] = mask;
+    if (h == 0) {
+        const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
+        if (lane == 0) a.hard_out[(int64_t)g * a.AZ + line_v] = mask;
+    }
     if (ng > 0 && bad != 0 && live) a.topbad[f] = 1;
 
-    const bool single = dv == 1;                              // a single edge sends Q itself (P:330)
+    // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'
     float* const sp = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * Z + i) * kIlGroup + lane;
-    const unsigned step = (unsigned)Z * kIlGroup * 4u;
-#pragma unroll 4
-    for (int kk = 0; kk < dv; ++kk) {
-        const float Lvc = single ? Q : L - mm[kk * kIlGroup];   // Q + sum_{k' != k} m_k'
-        unsigned wb = __float_as_uint(w_of(Lvc));
-        if (kk < ng) wb = (wb & 0xfffffffeu) | xh;            // gen edge: tag with the hard decision
-        if (live) *byte_ptr(sp, (unsigned)kk * step) = __uint_as_float(wb);
+#pragma unroll 1
+    for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
+#pragma unroll
+        for (int gi = 0; gi < GPW; ++gi) {
+            int k, ke;
+            block_of(rnd, gi, k, ke);
+            const int e3 = min(ke, ng);
+            for (; k < e3; ++k) {                             // gen edges: tagged with the hard decision
+                const float Lvc = single ? Q : L - mm[k * kIlGroup];
+                if (live) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((__float_as_uint(w_of(Lvc)) & 0xfffffffeu) | xh);
+            }
+            if (k + 8 <= ke) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float wn = w_of(L - mm[(k + j) * kIlGroup]);
+                    if (live) *byte_ptr(sp, (unsigned)(k + j) * step) = wn;       // nothing of a stopped frame is stored
+                }
+                k += 8;
+            }
+            for (; k < ke; ++k) {
+                const float wn = w_of(single ? Q : L - mm[k * kIlGroup]);
+                if (live) *byte_ptr(sp, (unsigned)k * step) = wn;
+            }
+        }
     }
+    }   // tiles of this CTA
 }
 
 // ---- a4: every check of every frame on the frame's frozen state (iteration d_iters[f]) -------------------------------
@@ -491,45 +575,60 @@ struct IlLaunch {
     bool final_mode; int n_sm, prepare_only;
 };
 
-// warps per CTA: the width whose last tile idles the fewest warps, near 8, within the shared-memory budget
+// variables per CTA: the width whose last tile idles the fewest warps, as wide as 512 threads and the shared-memory
+// budget allow (the table load of a CTA serves all of them); H warps per variable
 inline int il_pick_w(int Z, int max_dv, int max_np) {
+    const int H = max_dv > 2 * kIlChunk ? 2 : 1, wmax = 16 / H;
     int best = 1;
     double best_cost = 1e30;
-    for (int w = 2; w <= 16; ++w) {
+    for (int w = 1; w <= wmax; ++w) {
         if (il_smem_bytes(max_dv, max_np, w) > 200 * 1024) break;
         const int tiles = (Z + w - 1) / w;
         const double waste = (double)(tiles * w - Z) / (double)(tiles * w);
-        const double cost = waste + 0.01 * (w > 8 ? w - 8 : 8 - w);   // ties: close to 8 warps
+        const double cost = waste + 0.002 * (wmax - w);
         if (cost < best_cost - 1e-12) { best_cost = cost; best = w; }
     }
     return best;
 }
+// tiles per CTA: as many as still leave about 24 CTAs per multiprocessor
+inline int il_pick_tp(int n_cols, int tiles, int n_groups, int n_sm) {
+    const long long total = (long long)n_cols * tiles * n_groups;
+    const long long tp = total / (24LL * n_sm);
+    return (int)(tp < 1 ? 1 : tp > tiles ? tiles : tp);
+}
 
 #ifdef QC_IL_IMPL
-inline void launch_pass_il(const IlLaunch& L) {
+template <int H, int GPW>
+inline void launch_pass_il_h(const IlLaunch& L) {
     IlArgs args = L.args;
     const size_t smem = il_smem_bytes(args.max_dv, args.max_np, args.W);
     static thread_local int attr_dev = -1;                  // the attribute is per device
     int dev = 0;
     cudaGetDevice(&dev);
     if (attr_dev != dev) {
-        cudaFuncSetAttribute(k_pass_il<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
-        cudaFuncSetAttribute(k_pass_il<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<true, H, GPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<false, H, GPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
         attr_dev = dev;
     }
     if (L.prepare_only) return;
     const bool with_check = !L.final_mode && L.check != nullptr;
-    const int work = args.n_cols * args.tiles;
+    const int work = args.n_cols * args.ctas_per_col;
     const int extra = with_check ? (2 * L.n_sm + args.n_groups - 1) / args.n_groups : 0;
     args.cand_x = with_check ? work : -1;
     static const CheckTables no_tab{nullptr, nullptr};
     static const CheckArgs no_args{};
-    const dim3 grid(work + extra, args.n_groups), block(32 * args.W);
+    const dim3 grid(work + extra, args.n_groups), block(32 * H * args.W);
     if (L.final_mode)
-        k_pass_il<true><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
+        k_pass_il<true, H, GPW><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
     else
-        launch_pdl(k_pass_il<false>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
+        launch_pdl(k_pass_il<false, H, GPW>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
                    with_check ? *L.check : no_args);
+}
+
+// long columns (four partial sums): two warps per variable; short ones: one warp, one sum
+inline void launch_pass_il(const IlLaunch& L) {
+    if (L.args.split == 4) launch_pass_il_h<2, 2>(L);
+    else launch_pass_il_h<1, 1>(L);
 }
 #endif
 

@@ -114,6 +114,7 @@ struct qcldpc_code {
     // frame-interleaved family (pass_il.cuh): the same tables with run length Z (a run is Z lines of 32 frames)
     std::vector<EdgeDesc> edge_il; std::vector<PartnerDesc> partner_il;
     EdgeDesc* d_edge_il = nullptr; PartnerDesc* d_partner_il = nullptr;
+    std::vector<uint4> il_blob; uint4* d_il_blob = nullptr; int il_blob16 = 0;   // per-column tables of k_pass_il
     bool il_ok = false;                   // the code fits the family's 32-bit byte offsets
     int il_w = 8;                         // warps per CTA of k_pass_il
     PassLauncher launcher = nullptr;
@@ -556,6 +557,29 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
                   (int64_t)mb * Z < ((int64_t)1 << 25) &&
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
+    if (code->il_ok) {                                     // one fixed-stride blob per column, in shared-memory layout
+        const int mdv = std::max(code->max_dv, 1);
+        const size_t stride = il_table_bytes(mdv, max_np);
+        code->il_blob16 = (int)(stride / 16);
+        code->il_blob.assign((size_t)code->n_act_cols * code->il_blob16, uint4{0, 0, 0, 0});
+        for (int c = 0; c < code->n_act_cols; ++c) {
+            const ColDesc& cd = code->col[c];
+            char* base = reinterpret_cast<char*>(code->il_blob.data()) + (size_t)c * stride;
+            IlColHdr hdr{cd.col, cd.ebeg, cd.dv, cd.ng, cd.ngh, cd.np, 0, 0};
+            memcpy(base, &hdr, sizeof(hdr));
+            IlEdgeA* ea = reinterpret_cast<IlEdgeA*>(base + sizeof(IlColHdr));
+            GenDesc* eg = reinterpret_cast<GenDesc*>(ea + mdv);
+            IlEdgeB* eb = reinterpret_cast<IlEdgeB*>(eg + mdv);
+            PartnerDesc* ep = reinterpret_cast<PartnerDesc*>(eb + mdv);
+            for (int k = 0; k < cd.dv; ++k) {
+                const EdgeDesc& d = code->edge_il[cd.ebeg + k];
+                ea[k] = IlEdgeA{d.shift, d.t_off, d.p_off, d.delta};
+                eb[k] = IlEdgeB{d.p2_off, d.delta2};
+            }
+            for (int k = 0; k < cd.ng; ++k) eg[k] = code->gen[cd.gbeg + k];
+            for (int k = 0; k < cd.np; ++k) ep[k] = code->partner_il[cd.pbeg + k];
+        }
+    }
 
     auto upload = [](auto& vec, auto** dptr) -> cudaError_t {
         const size_t bytes = std::max<size_t>(vec.size(), 1) * sizeof(vec[0]);
@@ -572,6 +596,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     if (e == cudaSuccess) e = upload(code->redge, &code->d_redge);
     if (e == cudaSuccess && code->il_ok) e = upload(code->edge_il, &code->d_edge_il);
     if (e == cudaSuccess && code->il_ok) e = upload(code->partner_il, &code->d_partner_il);
+    if (e == cudaSuccess && code->il_ok) e = upload(code->il_blob, &code->d_il_blob);
     int dev = 0;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&code->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -587,7 +612,7 @@ void qcldpc_code_destroy(qcldpc_code_t* code) {
     if (code->cap_body) cudaStreamDestroy(code->cap_body);
     cudaFree(code->d_edge); cudaFree(code->d_gen); cudaFree(code->d_partner); cudaFree(code->d_col);
     cudaFree(code->d_row); cudaFree(code->d_redge);
-    cudaFree(code->d_edge_il); cudaFree(code->d_partner_il);
+    cudaFree(code->d_edge_il); cudaFree(code->d_partner_il); cudaFree(code->d_il_blob);
     delete code;
 }
 
@@ -939,6 +964,9 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         ia.n_frames = n_frames; ia.n_groups = w.n_groups; ia.n_cols = code->n_act_cols; ia.mb = code->mb;
         ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
         ia.max_np = code->max_np;
+        ia.tp = il_pick_tp(code->n_act_cols, ia.tiles, w.n_groups, code->n_sm);
+        ia.ctas_per_col = (ia.tiles + ia.tp - 1) / ia.tp;
+        ia.blob = code->d_il_blob; ia.blob16 = code->il_blob16;
         ia.n = code->n; ia.m = code->m; ia.EZ = EZ; ia.mZ = mZ; ia.AZ = AZ;
         P.ill = IlLaunch{PassTables{code->d_edge_il, code->d_gen, code->d_partner_il, code->d_col}, P.ctab, ia, st,
                          nullptr, false, code->n_sm, 0};
