@@ -241,18 +241,22 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 }
 
 // ---- a1 + a2: the fused pass ------------------------------------------------------------------------------------------
-// CTA = W variables of one active column x H warps per variable; grid = (columns * tiles [+ check workers], groups).
-// Shared memory: the column's tables, the messages m'[W][max_dv][32], the partial sums [W][4][32].
+// CTA = S slots x H warps; a slot = V = 2 consecutive variables of one active column, carried by the same threads (the
+// table lookups, window indices and loop control -- most of this kernel's instructions -- serve both); a tile = W = 2 S
+// variables; grid = (columns * CTAs per column [+ check workers], groups).
+// Shared memory: the column's tables, the messages m'[W][max_dv][32], the partial sums, the handshake counters.
 // The messages of a column are added as the generic pass adds them: block b = k / 8 of the column's edges belongs to
 // partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = 4 for long columns (max_dv > 16), else 1; inside a partial sum k
-// increases; the partial sums meet in the order 0 .. G-1.  H = 2 (G = 4): warp h of a variable owns the partial sums
-// 2h and 2h + 1 -- and with them the edges, their loads, their messages and their stores --, so a column of degree 60 is
-// two chains of 28 and 32 edges and twice as many warps keep loads in flight; the two warps meet once, at a named
-// barrier, to exchange their partial sums.  H = 1 (G = 1): one warp, one sum.
+// increases; the partial sums meet in the order 0 .. G-1.  H = 2 (G = 4): warp h of a slot owns the partial sums 2h and
+// 2h + 1 -- and with them the edges, their loads, their messages and their stores --, so a column of degree 60 is two
+// chains of 28 and 32 edges; the two warps meet once per tile to exchange their partial sums.  H = 1 (G = 1): one warp.
+constexpr int kIlV = 2;
+
 template <bool FINAL, int H, int GPW>
-__global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
-                                                 const CheckArgs chk) {
+__global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
+                                                    const CheckArgs chk) {
     constexpr int G = H * GPW;
+    constexpr int V = kIlV;
     extern __shared__ __align__(128) unsigned char smem_il[];
     pdl_launch();
     if (!FINAL && a.cand_x >= 0 && (int)blockIdx.x >= a.cand_x) {
@@ -265,7 +269,7 @@ __global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const 
     const int ca = blockIdx.x / a.ctas_per_col;
     const int tile0 = (blockIdx.x - ca * a.ctas_per_col) * a.tp;
     const int warp = il_warp_id(), lane = threadIdx.x & 31;
-    const int var = warp / H, h = warp - var * H;            // variable of the tile, warp of the variable
+    const int slot = warp / H, h = warp - slot * H;
     const int mdv = a.max_dv;
     // prologue: the column's tables (constant: not the previous launch's output) in one round trip
     {
@@ -284,7 +288,7 @@ __global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const 
     __syncthreads();
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
     if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped (both warps of a
-                                                              // variable see the same frames and leave together)
+                                                              // slot see the same frames and leave together)
     const IlColHdr cd = *reinterpret_cast<const IlColHdr*>(smem_il);
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
     const IlEdgeA* const s_a = reinterpret_cast<const IlEdgeA*>(smem_il + sizeof(IlColHdr));
@@ -294,95 +298,138 @@ __global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const 
     // FINAL: every frame reads the state of its own last iteration, w^(T-1) in buffer (T - 1) mod 4
     const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup;
     const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup;
-    float* const mm = msg_base + (size_t)var * mdv * kIlGroup + lane;
-    float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)var * 8 * kIlGroup + lane;   // partial sums, 2 buffers
+    float* const mm = msg_base + (size_t)slot * V * mdv * kIlGroup + lane;            // m'[v][k][lane] of this slot
+    const int vstride = mdv * kIlGroup;
+    float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 8 * V * kIlGroup + lane;   // 2 buffers
     const unsigned ulane = (unsigned)lane;
     const unsigned step = (unsigned)Z * kIlGroup * 4u;
     const bool single = dv == 1;                              // a single edge sends Q itself
 
 #pragma unroll 1
     for (int tt = 0; tt < a.tp; ++tt) {
-    const int i = (tile0 + tt) * a.W + var;
-    if (tile0 + tt >= a.tiles || i >= Z) break;               // both warps of a variable leave together
-    const unsigned line_v = (unsigned)(ca * Z + i);
-    const unsigned xb = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v] >> lane) & 1u;
-    const float Q = a.qc[((int64_t)g * a.AZ + line_v) * kIlGroup + lane];
-    float* const xch = xch0 + (tt & 1) * 4 * kIlGroup;
+    const int i0 = (tile0 + tt) * a.W + slot * V;
+    if (tile0 + tt >= a.tiles || i0 >= Z) break;              // both warps of a slot leave together
+    const bool val1 = i0 + 1 < Z;                             // the slot's second variable exists (else: computed on the
+    const int i1 = val1 ? i0 + 1 : i0;                        // first one's data, nothing of it is stored)
+    const unsigned line_v[V] = {(unsigned)(ca * Z + i0), (unsigned)(ca * Z + i1)};
+    unsigned xb[V];
+    float Q[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        xb[v] = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v[v]] >> lane) & 1u;
+        Q[v] = a.qc[((int64_t)g * a.AZ + line_v[v]) * kIlGroup + lane];
+    }
+    float* const xch = xch0 + (tt & 1) * 4 * V * kIlGroup;
     unsigned bad = 0;
 
-    auto t_line = [&](const IlEdgeA& d) { int r = i - d.shift; r += r < 0 ? Z : 0; return (unsigned)(d.t_off + r); };
-    auto p_line = [&](int off, int delta) { return (unsigned)(off + il_wrap(i + delta, Z)); };
+    // lines of the two variables in a run: index (i + d) mod Z and its successor
+    auto two_lines = [&](int off, int x, unsigned (&ln)[V]) {
+        int x1 = x + (i1 - i0);
+        x1 = x1 >= Z ? x1 - Z : x1;
+        ln[0] = (unsigned)(off + x);
+        ln[1] = (unsigned)(off + x1);
+    };
+    auto t_lines = [&](const IlEdgeA& d, unsigned (&ln)[V]) { int r = i0 - d.shift; r += r < 0 ? Z : 0; two_lines(d.t_off, r, ln); };
+    auto p_lines = [&](int off, int delta, unsigned (&ln)[V]) { two_lines(off, il_wrap(i0 + delta, Z), ln); };
 
     // gen edge: fold every other edge of the row (the rule is associative); bit 0 of a gen edge's state is its
     // variable's hard decision: the XOR of the raw words carries sign AND parity
-    auto gen_edge = [&](int k, float& acc) {
+    auto gen_edge = [&](int k, float (&acc)[V]) {
         const IlEdgeA d = s_a[k];
         const GenDesc gd = s_g[k];
-        const float tv = __ldg(il_line(tP, t_line(d), ulane));
-        float num = 0.0f, den = 1.0f;
-        unsigned xa = 0u;
-#pragma unroll 1
-        for (int jb = 0; jb < gd.np; jb += 4) {
-            float pm[4];
+        unsigned tl[V];
+        t_lines(d, tl);
+        float tv[V], num[V], den[V];
+        unsigned xa[V];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+        for (int v = 0; v < V; ++v) { tv[v] = __ldg(il_line(tP, tl[v], ulane)); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
+#pragma unroll 1
+        for (int jb = 0; jb < gd.np; jb += 2) {
+            float pm[2][V];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
                 const bool have = jb + u < gd.np;
                 const PartnerDesc p = s_p[gd.pbeg + (have ? jb + u : 0)];
-                pm[u] = have ? __ldg(il_line(qP, p_line(p.off, p.delta), ulane)) : 0.0f;   // +0.0: the identity
+                unsigned pl[V];
+                p_lines(p.off, p.delta, pl);
+#pragma unroll
+                for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(il_line(qP, pl[v], ulane)) : 0.0f;   // +0.0: the identity
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const unsigned wb = __float_as_uint(pm[u]);
-                xa ^= wb;
-                boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num, den);
-            }
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const unsigned wb = __float_as_uint(pm[u][v]);
+                    xa[v] ^= wb;
+                    boxplus_acc(__uint_as_float(wb & 0x7ffffffeu), num[v], den[v]);
+                }
         }
-        if (!FINAL && gd.counter)            // parity of the row at the input iteration (t = (-1)^{s_c} 0 there)
-            bad |= (xa ^ xb ^ (__float_as_uint(tv) >> 31)) & 1u;
-        boxplus_acc(fabsf(tv), num, den);
-        const float mk = with_sign(mag_of(num, den), (xa ^ __float_as_uint(tv)) & 0x80000000u);
-        mm[k * kIlGroup] = mk;
-        acc += mk;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            if (!FINAL && gd.counter && (v == 0 || val1))   // parity of the row at the input iteration (t = (-1)^{s_c} 0)
+                bad |= ((xa[v] ^ xb[v] ^ (__float_as_uint(tv[v]) >> 31)) & 1u) << v;
+            boxplus_acc(fabsf(tv[v]), num[v], den[v]);
+            const float mk = with_sign(mag_of(num[v], den[v]), (xa[v] ^ __float_as_uint(tv[v])) & 0x80000000u);
+            mm[v * vstride + k * kIlGroup] = mk;
+            acc[v] += mk;
+        }
     };
     // edges of triple rows: two partners and an absorbed variable, one fraction, no reciprocal in between
-    auto triple = [&](auto CHc, int k0, float& acc) {
+    auto triple = [&](auto CHc, int k0, float (&acc)[V]) {
         constexpr int CH = decltype(CHc)::value;
-        float tv[CH], pa[CH], pb[CH];
+        float tv[CH][V], pa[CH][V], pb[CH][V];
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
             const IlEdgeA d = s_a[k0 + j];
             const IlEdgeB e = s_b[k0 + j];
-            tv[j] = __ldg(il_line(tP, t_line(d), ulane));
-            pa[j] = __ldg(il_line(qP, p_line(d.p_off, d.delta), ulane));
-            pb[j] = __ldg(il_line(qP, p_line(e.p2_off, e.delta2), ulane));
+            unsigned tl[V], al[V], bl[V];
+            t_lines(d, tl);
+            p_lines(d.p_off, d.delta, al);
+            p_lines(e.p2_off, e.delta2, bl);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                tv[j][v] = __ldg(il_line(tP, tl[v], ulane));
+                pa[j][v] = __ldg(il_line(qP, al[v], ulane));
+                pb[j][v] = __ldg(il_line(qP, bl[v], ulane));
+            }
         }
 #pragma unroll
-        for (int j = 0; j < CH; ++j) {
-            const unsigned ua = __float_as_uint(pa[j]), ub = __float_as_uint(pb[j]);
-            const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
-            float num = qa + qb, den = fmaf(qa, qb, 1.0f);
-            boxplus_acc(fabsf(tv[j]), num, den);
-            const float mk = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j])) & 0x80000000u);
-            mm[(k0 + j) * kIlGroup] = mk;
-            acc += mk;
-        }
+        for (int j = 0; j < CH; ++j)
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const unsigned ua = __float_as_uint(pa[j][v]), ub = __float_as_uint(pb[j][v]);
+                const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
+                float num = qa + qb, den = fmaf(qa, qb, 1.0f);
+                boxplus_acc(fabsf(tv[j][v]), num, den);
+                const float mk = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j][v])) & 0x80000000u);
+                mm[v * vstride + (k0 + j) * kIlGroup] = mk;
+                acc[v] += mk;
+            }
     };
     // pair edges: one partner and an absorbed variable
-    auto pair = [&](auto CHc, int k0, float& acc) {
+    auto pair = [&](auto CHc, int k0, float (&acc)[V]) {
         constexpr int CH = decltype(CHc)::value;
-        float tv[CH], wv[CH];
+        float tv[CH][V], wv[CH][V];
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
             const IlEdgeA d = s_a[k0 + j];
-            tv[j] = __ldg(il_line(tP, t_line(d), ulane));
-            wv[j] = __ldg(il_line(qP, p_line(d.p_off, d.delta), ulane));
+            unsigned tl[V], pl[V];
+            t_lines(d, tl);
+            p_lines(d.p_off, d.delta, pl);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                tv[j][v] = __ldg(il_line(tP, tl[v], ulane));
+                wv[j][v] = __ldg(il_line(qP, pl[v], ulane));
+            }
         }
 #pragma unroll
-        for (int j = 0; j < CH; ++j) {
-            const float mk = cn_rule(wv[j], tv[j]);
-            mm[(k0 + j) * kIlGroup] = mk;
-            acc += mk;
-        }
+        for (int j = 0; j < CH; ++j)
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const float mk = cn_rule(wv[j][v], tv[j][v]);
+                mm[v * vstride + (k0 + j) * kIlGroup] = mk;
+                acc[v] += mk;
+            }
     };
     using I1 = std::integral_constant<int, 1>;
     using I4 = std::integral_constant<int, 4>;
@@ -393,16 +440,20 @@ __global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const 
         kb = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk;
         ke = min(kb + kIlChunk, dv);
     };
-    float part[GPW];
+    float part[GPW][V];
 #pragma unroll
-    for (int gi = 0; gi < GPW; ++gi) part[gi] = 0.0f;
+    for (int gi = 0; gi < GPW; ++gi)
+#pragma unroll
+        for (int v = 0; v < V; ++v) part[gi][v] = 0.0f;
 #pragma unroll 1
     for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
 #pragma unroll
         for (int gi = 0; gi < GPW; ++gi) {
             int k, ke;
             block_of(rnd, gi, k, ke);
-            float acc = part[gi];
+            float acc[V];
+#pragma unroll
+            for (int v = 0; v < V; ++v) acc[v] = part[gi][v];
             const int e1 = min(ke, ngh), e3 = min(ke, ng);
             for (; k < e1; ++k) gen_edge(k, acc);
             if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
@@ -411,80 +462,107 @@ __global__ void __launch_bounds__(512, 3) k_pass_il(const PassTables tab, const 
             if (k + 8 <= ke) { pair(I8{}, k, acc); k += 8; }
             if (k + 4 <= ke) { pair(I4{}, k, acc); k += 4; }
             for (; k < ke; ++k) pair(I1{}, k, acc);
-            part[gi] = acc;
+#pragma unroll
+            for (int v = 0; v < V; ++v) part[gi][v] = acc[v];
         }
     }
 
     // variable-node rule: the partial sums meet in the order 0 .. G-1
-    float sum;
+    float sum[V];
     if (H == 1) {
-        sum = part[0];
-        if (GPW > 1) {
-            sum = 0.0f;
 #pragma unroll
-            for (int gi = 0; gi < GPW; ++gi) sum += part[gi];
+        for (int v = 0; v < V; ++v) {
+            sum[v] = part[0][v];
+            if (GPW > 1) {
+                sum[v] = 0.0f;
+#pragma unroll
+                for (int gi = 0; gi < GPW; ++gi) sum[v] += part[gi][v];
+            }
         }
     } else {
 #pragma unroll
-        for (int gi = 0; gi < GPW; ++gi) xch[(h * GPW + gi) * kIlGroup] = part[gi];
-        // the two warps of this variable meet here: release / acquire on a counter in shared memory (a named barrier
-        // per variable would pin all 16 hardware barriers of the CTA); tile tt + 1 uses the other buffer of partial
-        // sums, and a warp cannot be more than one exchange ahead of its partner
+        for (int gi = 0; gi < GPW; ++gi)
+#pragma unroll
+            for (int v = 0; v < V; ++v) xch[((h * GPW + gi) * V + v) * kIlGroup] = part[gi][v];
+        // the two warps of this slot meet here: release / acquire on a counter in shared memory (a named barrier per
+        // slot would pin all 16 hardware barriers of the CTA); tile tt + 1 uses the other buffer of partial sums, and a
+        // warp cannot be more than one exchange ahead of its partner
         __syncwarp();
-        if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + var * 2 + h), "r"(tt + 1) : "memory");
+        if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + slot * 2 + h), "r"(tt + 1) : "memory");
         int seen;
         do {
-            asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + var * 2 + (1 - h)) : "memory");
+            asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + slot * 2 + (1 - h)) : "memory");
         } while (seen < tt + 1);
-        sum = 0.0f;
 #pragma unroll
-        for (int gg = 0; gg < G; ++gg) sum += xch[gg * kIlGroup];
+        for (int v = 0; v < V; ++v) {
+            sum[v] = 0.0f;
+#pragma unroll
+            for (int gg = 0; gg < G; ++gg) sum[v] += xch[(gg * V + v) * kIlGroup];
+        }
     }
-    const float L = Q + sum;                                  // L'_v
-    unsigned xh = __float_as_uint(L) >> 31;                   // 0 iff L_v >= 0
+    float L[V];
+    unsigned xh[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        L[v] = Q[v] + sum[v];                                 // L'_v
+        xh[v] = __float_as_uint(L[v]) >> 31;                  // 0 iff L_v >= 0
+    }
     if (FINAL) {
         if (h != 0) continue;
-        if (live) {
-            const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + i;
-            a.d_hard[vv] = (uint8_t)xh;
-            if (a.d_post) a.d_post[vv] = L * kLn2;
-        } else {
-            xh = (a.hardm[0][(int64_t)g * a.AZ + line_v] >> lane) & 1u;   // t = 0: the decisions of the channel values
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            if (live) {
+                if (v == 0 || val1) {
+                    const int64_t vv = (int64_t)f * a.n + (int64_t)cd.col * Z + (v ? i1 : i0);
+                    a.d_hard[vv] = (uint8_t)xh[v];
+                    if (a.d_post) a.d_post[vv] = L[v] * kLn2;
+                }
+            } else {
+                xh[v] = (a.hardm[0][(int64_t)g * a.AZ + line_v[v]] >> lane) & 1u;   // t = 0: decisions of the channel values
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, xh[v] != 0);
+            if (lane == 0 && (v == 0 || val1)) a.hardm_final[(int64_t)g * a.AZ + line_v[v]] = mask;
         }
-        const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
-        if (lane == 0) a.hardm_final[(int64_t)g * a.AZ + line_v] = mask;
         continue;
     }
     if (h == 0) {
-        const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
-        if (lane == 0) a.hard_out[(int64_t)g * a.AZ + line_v] = mask;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const unsigned mask = __ballot_sync(0xffffffffu, xh[v] != 0);
+            if (lane == 0 && (v == 0 || val1)) a.hard_out[(int64_t)g * a.AZ + line_v[v]] = mask;
+        }
     }
     if (ng > 0 && bad != 0 && live) a.topbad[f] = 1;
 
     // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'
-    float* const sp = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * Z + i) * kIlGroup + lane;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        const bool st = live && (v == 0 || val1);             // nothing of a stopped frame is stored
+        float* const sp = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * Z + (v ? i1 : i0)) * kIlGroup + lane;
+        const float* const mv = mm + v * vstride;
 #pragma unroll 1
-    for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
+        for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
 #pragma unroll
-        for (int gi = 0; gi < GPW; ++gi) {
-            int k, ke;
-            block_of(rnd, gi, k, ke);
-            const int e3 = min(ke, ng);
-            for (; k < e3; ++k) {                             // gen edges: tagged with the hard decision
-                const float Lvc = single ? Q : L - mm[k * kIlGroup];
-                if (live) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((__float_as_uint(w_of(Lvc)) & 0xfffffffeu) | xh);
-            }
-            if (k + 8 <= ke) {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float wn = w_of(L - mm[(k + j) * kIlGroup]);
-                    if (live) *byte_ptr(sp, (unsigned)(k + j) * step) = wn;       // nothing of a stopped frame is stored
+            for (int gi = 0; gi < GPW; ++gi) {
+                int k, ke;
+                block_of(rnd, gi, k, ke);
+                const int e3 = min(ke, ng);
+                for (; k < e3; ++k) {                         // gen edges: tagged with the hard decision
+                    const float Lvc = single ? Q[v] : L[v] - mv[k * kIlGroup];
+                    if (st) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((__float_as_uint(w_of(Lvc)) & 0xfffffffeu) | xh[v]);
                 }
-                k += 8;
-            }
-            for (; k < ke; ++k) {
-                const float wn = w_of(single ? Q : L - mm[k * kIlGroup]);
-                if (live) *byte_ptr(sp, (unsigned)k * step) = wn;
+                if (k + 8 <= ke) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const float wn = w_of(L[v] - mv[(k + j) * kIlGroup]);
+                        if (st) *byte_ptr(sp, (unsigned)(k + j) * step) = wn;
+                    }
+                    k += 8;
+                }
+                for (; k < ke; ++k) {
+                    const float wn = w_of(single ? Q[v] : L[v] - mv[k * kIlGroup]);
+                    if (st) *byte_ptr(sp, (unsigned)k * step) = wn;
+                }
             }
         }
     }
@@ -575,17 +653,18 @@ struct IlLaunch {
     bool final_mode; int n_sm, prepare_only;
 };
 
-// variables per CTA: the width whose last tile idles the fewest warps, as wide as 512 threads and the shared-memory
-// budget allow (the table load of a CTA serves all of them); H warps per variable
+// variables per tile (an even number: slots of two): the width whose last tile idles the fewest warps, as wide as 12
+// warps and the shared-memory budget allow (the table load of a CTA serves all of them); H warps per slot
 inline int il_pick_w(int Z, int max_dv, int max_np) {
-    const int H = max_dv > 2 * kIlChunk ? 2 : 1, wmax = 16 / H;
-    int best = 1;
+    const int H = max_dv > 2 * kIlChunk ? 2 : 1, smax = 12 / H;
+    int best = 2;
     double best_cost = 1e30;
-    for (int w = 1; w <= wmax; ++w) {
-        if (il_smem_bytes(max_dv, max_np, w) > 200 * 1024) break;
+    for (int sl = 1; sl <= smax; ++sl) {
+        const int w = 2 * sl;
+        if (il_smem_bytes(max_dv, max_np, w) > 100 * 1024) break;       // two CTAs per multiprocessor
         const int tiles = (Z + w - 1) / w;
         const double waste = (double)(tiles * w - Z) / (double)(tiles * w);
-        const double cost = waste + 0.002 * (wmax - w);
+        const double cost = waste + 0.03 * (smax - sl);        // a narrow CTA pays its table load for few variables
         if (cost < best_cost - 1e-12) { best_cost = cost; best = w; }
     }
     return best;
@@ -617,7 +696,7 @@ inline void launch_pass_il_h(const IlLaunch& L) {
     args.cand_x = with_check ? work : -1;
     static const CheckTables no_tab{nullptr, nullptr};
     static const CheckArgs no_args{};
-    const dim3 grid(work + extra, args.n_groups), block(32 * H * args.W);
+    const dim3 grid(work + extra, args.n_groups), block(32 * H * (args.W / 2));
     if (L.final_mode)
         k_pass_il<true, H, GPW><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
     else
