@@ -343,11 +343,14 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
         unsigned xa[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) { tv[v] = __ldg(il_line(tP, tl[v], ulane)); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
+        // partners in batches of kGenBatch, all loads of a batch in flight (a check of degree 7, the largest of the
+        // paper's ensemble, is one round trip)
+        constexpr int kGenBatch = 6;
 #pragma unroll 1
-        for (int jb = 0; jb < gd.np; jb += 2) {
-            float pm[2][V];
+        for (int jb = 0; jb < gd.np; jb += kGenBatch) {
+            float pm[kGenBatch][V];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < kGenBatch; ++u) {
                 const bool have = jb + u < gd.np;
                 const PartnerDesc p = s_p[gd.pbeg + (have ? jb + u : 0)];
                 unsigned pl[V];
@@ -356,7 +359,7 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
                 for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(il_line(qP, pl[v], ulane)) : 0.0f;   // +0.0: the identity
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
+            for (int u = 0; u < kGenBatch; ++u)
 #pragma unroll
                 for (int v = 0; v < V; ++v) {
                     const unsigned wb = __float_as_uint(pm[u][v]);
