@@ -72,6 +72,8 @@ template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[4], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : idx == 2 ? p[2] : p[3]; }
 template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : p[2]; }
+// line index -> pointer, lane already in the base
+__device__ __forceinline__ const float* il_row(const float* base_lane, unsigned line) { return byte_ptr(base_lane, line << 7); }
 // line index -> pointer to this lane's float
 __device__ __forceinline__ const float* il_line(const float* base, unsigned line, unsigned lane) {
     return byte_ptr(base, (line * kIlGroup + lane) * 4u);
@@ -296,8 +298,9 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     const IlEdgeB* const s_b = reinterpret_cast<const IlEdgeB*>(s_g + mdv);
     const PartnerDesc* const s_p = reinterpret_cast<const PartnerDesc*>(s_b + mdv);
     // FINAL: every frame reads the state of its own last iteration, w^(T-1) in buffer (T - 1) mod 4
-    const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup;
-    const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup;
+    // (the lane is folded into the base pointers: a load address is base + 128 * line)
+    const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup + lane;
+    const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup + lane;
     float* const mm = msg_base + (size_t)slot * V * mdv * kIlGroup + lane;            // m'[v][k][lane] of this slot
     const int vstride = mdv * kIlGroup;
     float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 8 * V * kIlGroup + lane;   // 2 buffers
@@ -342,7 +345,7 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
         float tv[V], num[V], den[V];
         unsigned xa[V];
 #pragma unroll
-        for (int v = 0; v < V; ++v) { tv[v] = __ldg(il_line(tP, tl[v], ulane)); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
+        for (int v = 0; v < V; ++v) { tv[v] = __ldg(il_row(tP, tl[v])); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
         // partners in batches of kGenBatch, all loads of a batch in flight (a check of degree 7, the largest of the
         // paper's ensemble, is one round trip)
         constexpr int kGenBatch = 6;
@@ -356,7 +359,7 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
                 unsigned pl[V];
                 p_lines(p.off, p.delta, pl);
 #pragma unroll
-                for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(il_line(qP, pl[v], ulane)) : 0.0f;   // +0.0: the identity
+                for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(il_row(qP, pl[v])) : 0.0f;   // +0.0: the identity
             }
 #pragma unroll
             for (int u = 0; u < kGenBatch; ++u)
@@ -391,9 +394,9 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
             p_lines(e.p2_off, e.delta2, bl);
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                tv[j][v] = __ldg(il_line(tP, tl[v], ulane));
-                pa[j][v] = __ldg(il_line(qP, al[v], ulane));
-                pb[j][v] = __ldg(il_line(qP, bl[v], ulane));
+                tv[j][v] = __ldg(il_row(tP, tl[v]));
+                pa[j][v] = __ldg(il_row(qP, al[v]));
+                pb[j][v] = __ldg(il_row(qP, bl[v]));
             }
         }
 #pragma unroll
@@ -421,8 +424,8 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
             p_lines(d.p_off, d.delta, pl);
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                tv[j][v] = __ldg(il_line(tP, tl[v], ulane));
-                wv[j][v] = __ldg(il_line(qP, pl[v], ulane));
+                tv[j][v] = __ldg(il_row(tP, tl[v]));
+                wv[j][v] = __ldg(il_row(qP, pl[v]));
             }
         }
 #pragma unroll
@@ -549,22 +552,19 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
             for (int gi = 0; gi < GPW; ++gi) {
                 int k, ke;
                 block_of(rnd, gi, k, ke);
-                const int e3 = min(ke, ng);
-                for (; k < e3; ++k) {                         // gen edges: tagged with the hard decision
-                    const float Lvc = single ? Q[v] : L[v] - mv[k * kIlGroup];
-                    if (st) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((__float_as_uint(w_of(Lvc)) & 0xfffffffeu) | xh[v]);
-                }
-                if (k + 8 <= ke) {
+                if (ke - k == kIlChunk) {                     // a whole block: unrolled, the tag of the gen edges branch-free
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const float wn = w_of(L[v] - mv[(k + j) * kIlGroup]);
-                        if (st) *byte_ptr(sp, (unsigned)(k + j) * step) = wn;
+                    for (int j = 0; j < kIlChunk; ++j) {
+                        const unsigned tagbit = (k + j < ng) ? 1u : 0u;   // gen edge: bit 0 carries the hard decision
+                        const unsigned wb = __float_as_uint(w_of(L[v] - mv[(k + j) * kIlGroup]));
+                        if (st) *byte_ptr(sp, (unsigned)(k + j) * step) = __uint_as_float((wb & ~tagbit) | (xh[v] & tagbit));
                     }
-                    k += 8;
-                }
-                for (; k < ke; ++k) {
-                    const float wn = w_of(single ? Q[v] : L[v] - mv[k * kIlGroup]);
-                    if (st) *byte_ptr(sp, (unsigned)k * step) = wn;
+                } else {
+                    for (; k < ke; ++k) {
+                        const unsigned tagbit = (k < ng) ? 1u : 0u;
+                        const unsigned wb = __float_as_uint(w_of(single ? Q[v] : L[v] - mv[k * kIlGroup]));
+                        if (st) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((wb & ~tagbit) | (xh[v] & tagbit));
+                    }
                 }
             }
         }
@@ -664,7 +664,7 @@ inline int il_pick_w(int Z, int max_dv, int max_np) {
     double best_cost = 1e30;
     for (int sl = 1; sl <= smax; ++sl) {
         const int w = 2 * sl;
-        if (il_smem_bytes(max_dv, max_np, w) > 100 * 1024) break;       // two CTAs per multiprocessor
+        if (il_smem_bytes(max_dv, max_np, w) > 110 * 1024) break;       // two CTAs per multiprocessor
         const int tiles = (Z + w - 1) / w;
         const double waste = (double)(tiles * w - Z) / (double)(tiles * w);
         const double cost = waste + 0.03 * (smax - sl);        // a narrow CTA pays its table load for few variables
@@ -672,12 +672,9 @@ inline int il_pick_w(int Z, int max_dv, int max_np) {
     }
     return best;
 }
-// tiles per CTA: as many as still leave about 24 CTAs per multiprocessor
-inline int il_pick_tp(int n_cols, int tiles, int n_groups, int n_sm) {
-    const long long total = (long long)n_cols * tiles * n_groups;
-    const long long tp = total / (24LL * n_sm);
-    return (int)(tp < 1 ? 1 : tp > tiles ? tiles : tp);
-}
+// tiles per CTA: one.  Measured (q = 50, 32 frames, ms per launch): 1 tile 0.273, 2 tiles 0.284, 3 tiles 0.294, 5 tiles
+// (a whole column) 0.300 -- fewer, longer CTAs balance worse than the table load they save; QCLDPC_ILTP overrides.
+inline int il_pick_tp(int, int, int, int) { return 1; }
 
 #ifdef QC_IL_IMPL
 template <int H, int GPW>

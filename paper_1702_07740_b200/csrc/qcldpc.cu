@@ -83,6 +83,7 @@ struct Tuning {
     int loop_graph = 1;                   // QCLDPC_LOOP=stream: one launch per iteration from the host, no graph
     int body_mult = 0;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations (0: by batch size)
     int il = 1;                           // QCLDPC_IL=0: never the frame-interleaved family; 2: for every batch size
+    int il_tp = 0;                        // QCLDPC_ILTP=k: tiles per CTA of k_pass_il (0: by grid size)
 };
 
 // One instantiated decode graph per argument tuple (the kernel parameters are baked into the graph's nodes).
@@ -545,6 +546,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         tn.loop_graph = !(lp && strcmp(lp, "stream") == 0);
         tn.body_mult = std::min(16, std::max(0, env_int("QCLDPC_BODY", 0)));
         tn.il = std::min(2, std::max(0, env_int("QCLDPC_IL", 1)));
+        tn.il_tp = std::max(0, env_int("QCLDPC_ILTP", 0));
     }
 
     // frame-interleaved family: offsets in lines of 32 frames, runs of exactly Z lines
@@ -560,6 +562,11 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
                   (int64_t)mb * Z < ((int64_t)1 << 25) &&
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
+    if (const int wf = env_int("QCLDPC_ILW", 0)) {         // tuning knob: variables per tile of k_pass_il (even, <= 12)
+        if (wf >= 2 && wf <= (code->max_dv > 2 * kIlChunk ? 12 : 24) && wf % 2 == 0 &&
+            il_smem_bytes(code->max_dv, max_np, wf) <= (size_t)200 * 1024)
+            code->il_w = wf;
+    }
     if (code->il_ok) {                                     // one fixed-stride blob per column, in shared-memory layout
         const int mdv = std::max(code->max_dv, 1);
         const size_t stride = il_table_bytes(mdv, max_np);
@@ -968,6 +975,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
         ia.max_np = code->max_np;
         ia.tp = il_pick_tp(code->n_act_cols, ia.tiles, w.n_groups, code->n_sm);
+        if (code->tune.il_tp > 0) ia.tp = std::min(code->tune.il_tp, ia.tiles);
         ia.ctas_per_col = (ia.tiles + ia.tp - 1) / ia.tp;
         ia.blob = code->d_il_blob; ia.blob16 = code->il_blob16;
         ia.n = code->n; ia.m = code->m; ia.EZ = EZ; ia.mZ = mZ; ia.AZ = AZ;
