@@ -197,19 +197,6 @@ int qcldpc_iterations_issued(const qcldpc_code_t* code, int n_frames, const void
                              int* h_iterations);
 int qcldpc_last_loop_mode(void);
 
-/*
- * Optional launch timing for roofline reports (bench.py).  qcldpc_profile_enable(stride) with stride > 0 makes the
- * following qcldpc_decode calls of this thread record a CUDA event pair, on the decode stream, around every
- * stride-th launch of the two per-iteration kernels (kind 0 = fused check/variable update k_pass, kind 1 =
- * early-exit check k_cand); stride = 0 switches it off.  qcldpc_profile_collect waits for the recorded events (host
- * blocks until they have completed), returns for each kind the summed duration in ms of the timed launches, how many
- * were timed and how many were launched since enable/collect, and clears the record.  ms_sum, timed, launched:
- * HOST arrays of 2 entries.  The events live in a per-thread pool that grows on demand while profiling is on (the one
- * place where a decode call creates CUDA objects) and is destroyed by qcldpc_profile_enable(0).
- */
-int qcldpc_profile_enable(int stride);
-int qcldpc_profile_collect(double* ms_sum, int64_t* timed, int64_t* launched);
-
 const char* qcldpc_status_string(int status);
 const char* qcldpc_last_cuda_error(void); /* thread-local text of the last CUDA failure ("" if none) */
 

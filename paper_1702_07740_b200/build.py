@@ -16,7 +16,8 @@ CSRC = os.path.join(_HERE, "csrc")
 OBJDIR = os.path.join(CSRC, "build")
 SO_PATH = os.path.join(CSRC, "libqcldpc.so")
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "pass_kernel.cuh"), os.path.join(CSRC, "pass_exact.cuh"), os.path.join(CSRC, "check.cuh"), os.path.join(CSRC, "pass_il.cuh"),
-           os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h")]
+           os.path.join(os.path.dirname(_HERE), "include", "qcldpc.h"),
+           os.path.join(os.path.dirname(_HERE), "include", "qcldpc_profile.h")]
 # (symbol, DV, NG, PCAP): exact families = every active column has degree DV with NG gen edges (the BASELINE.json codes:
 # 11 or 21 edges, 3 of them into the top rows); pass_generic.cu takes any column of degree <= 64
 # partner slots per gen edge held in registers, per family (measured: config 2's top rows reach degree 9, configs

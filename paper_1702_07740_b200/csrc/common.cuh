@@ -7,6 +7,7 @@
 #include <cstdint>
 
 #include "../../include/qcldpc.h"
+#include "../../include/qcldpc_profile.h"
 
 namespace qc {
 

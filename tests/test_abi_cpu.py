@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-HEADER = os.path.join(ROOT, "include", "qcldpc.h")
+HEADERS = [os.path.join(ROOT, "include", "qcldpc.h"), os.path.join(ROOT, "include", "qcldpc_profile.h")]
 
 
 @pytest.fixture(scope="module")
@@ -19,7 +19,7 @@ def lib():
 
 
 def declared_functions():
-    text = open(HEADER).read()
+    text = "\n".join(open(h).read() for h in HEADERS)
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(qcldpc_[a-z0-9_]+)\s*\(", text)))
 
@@ -28,7 +28,7 @@ def test_header_symbols_are_exported(lib):
     names = declared_functions()
     assert len(names) >= 10 and "qcldpc_code_create" in names and "qcldpc_decode" in names
     for name in names:
-        assert hasattr(lib, name), f"{name} declared in include/qcldpc.h but not exported"
+        assert hasattr(lib, name), f"{name} declared in include/*.h but not exported"
     from paper_1702_07740_b200 import binding
     assert sorted(binding.EXPORTED_SYMBOLS) == names
 
