@@ -72,8 +72,8 @@ template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[4], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : idx == 2 ? p[2] : p[3]; }
 template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : p[2]; }
-// line index -> pointer, lane already in the base
-__device__ __forceinline__ const float* il_row(const float* base_lane, unsigned line) { return byte_ptr(base_lane, line << 7); }
+// byte offset of a line -> pointer, lane already in the base
+__device__ __forceinline__ const float* il_row(const float* base_lane, unsigned byte_off) { return byte_ptr(base_lane, byte_off); }
 // line index -> pointer to this lane's float
 __device__ __forceinline__ const float* il_line(const float* base, unsigned line, unsigned lane) {
     return byte_ptr(base, (line * kIlGroup + lane) * 4u);
@@ -325,12 +325,12 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     float* const xch = xch0 + (tt & 1) * 4 * V * kIlGroup;
     unsigned bad = 0;
 
-    // lines of the two variables in a run: index (i + d) mod Z and its successor
+    // BYTE offsets of the two variables' lines in a run (the blob's offsets are in bytes: line << 7): index x = (i + d)
+    // mod Z and its successor, which is the run's first line when x is the last one
+    const unsigned step1 = val1 ? 128u : 0u, step_wrap = val1 ? 128u - (unsigned)Z * 128u : 0u;
     auto two_lines = [&](int off, int x, unsigned (&ln)[V]) {
-        int x1 = x + (i1 - i0);
-        x1 = x1 >= Z ? x1 - Z : x1;
-        ln[0] = (unsigned)(off + x);
-        ln[1] = (unsigned)(off + x1);
+        ln[0] = (unsigned)off + ((unsigned)x << 7);
+        ln[1] = ln[0] + (x == Z - 1 ? step_wrap : step1);
     };
     auto t_lines = [&](const IlEdgeA& d, unsigned (&ln)[V]) { int r = i0 - d.shift; r += r < 0 ? Z : 0; two_lines(d.t_off, r, ln); };
     auto p_lines = [&](int off, int delta, unsigned (&ln)[V]) { two_lines(off, il_wrap(i0 + delta, Z), ln); };

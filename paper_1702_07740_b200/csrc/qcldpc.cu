@@ -583,11 +583,15 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
             PartnerDesc* ep = reinterpret_cast<PartnerDesc*>(eb + mdv);
             for (int k = 0; k < cd.dv; ++k) {
                 const EdgeDesc& d = code->edge_il[cd.ebeg + k];
-                ea[k] = IlEdgeA{d.shift, d.t_off, d.p_off, d.delta};
-                eb[k] = IlEdgeB{d.p2_off, d.delta2};
+                // offsets of the blob are BYTE offsets of lines (line << 7; below 2^32 by il_ok)
+                ea[k] = IlEdgeA{d.shift, (int)((unsigned)d.t_off << 7), d.p_off >= 0 ? (int)((unsigned)d.p_off << 7) : -1, d.delta};
+                eb[k] = IlEdgeB{d.p2_off >= 0 ? (int)((unsigned)d.p2_off << 7) : -1, d.delta2};
             }
             for (int k = 0; k < cd.ng; ++k) eg[k] = code->gen[cd.gbeg + k];
-            for (int k = 0; k < cd.np; ++k) ep[k] = code->partner_il[cd.pbeg + k];
+            for (int k = 0; k < cd.np; ++k) {
+                ep[k] = code->partner_il[cd.pbeg + k];
+                ep[k].off = (int)((unsigned)ep[k].off << 7);
+            }
         }
     }
 
