@@ -2,8 +2,9 @@
 // ensemble (NEXT-1: circulants of q = 21 or 50, columns of degree 59/60) above all.
 //
 // Layout.  Frames are taken in groups of 32 and interleaved innermost: element (run e, index i, frame f of the group)
-// of any per-edge / per-check / per-variable array lives at ((e * Z + i) * 32 + f).  One WARP = one variable (or one
-// check) of all 32 frames of a group, lane = frame.  Consequences:
+// of any per-edge / per-check / per-variable array lives at ((e * Z + i) * 32 + f).  A warp works on one variable (or
+// one check; in the pass: a slot of two consecutive variables, shared by two warps) of all 32 frames of a group,
+// lane = frame.  Consequences:
 //   * every access of a warp is one aligned 128-byte line, whatever the circulant size and shift (a cyclic shift by p
 //     is a shift by p whole lines): no partial sectors, no idle lanes for q = 21 or 50, no halo, and the wrap of the
 //     index is one warp-uniform compare-subtract instead of one per element;

@@ -24,6 +24,10 @@
 //               returns at once when there is no candidate; freezes d_iters / d_pass / done per frame.  Runs in an
 //               extra grid row of k_pass_exact, or as the stand-alone k_cand (generic family, last iteration).
 //   the FINAL instantiations of the pass, k_check_final, k_flags_final   a4  outputs from each frame's frozen state
+//   k_pass_il, k_il_*, k_cand_il   the same steps on the frame-interleaved layout (pass_il.cuh): batches of codes with
+//               long columns, the paper's own ensemble above all
+//   k_loop_ctl  the iteration loop itself: one CUDA graph per decode with a conditional WHILE node (decode_impl)
+//   (the steps either side of the decoder -- LLR front end, bit packing, CRC-32 -- are in frontend.cu)
 // Edge state lives in four buffers (iteration t in buffer t mod 4); the early-exit check of iteration t-2 runs next to
 // pass t and touches nothing that pass writes: check.cuh has the timeline.
 #include "check.cuh"
