@@ -188,7 +188,8 @@ int64_t qcldpc_last_launch_count(void);
  * of empty launches although the call never waits.  Instantiated graphs are cached in the handle, keyed by all pointer
  * and scalar arguments (the one place where the handle changes after creation; guarded by a mutex; building a graph
  * allocates driver memory).  QCLDPC_LOOP=stream (read by qcldpc_code_create) keeps one launch per iteration from the
- * host; so do decodes of fewer than 14 iterations and calls made while qcldpc_profile_enable is on.
+ * host; so do decodes of fewer than 14 iterations, calls made while qcldpc_profile_enable is on, and calls on a stream
+ * that the caller is capturing into a graph of its own (the launches then become nodes of that graph).
  *   qcldpc_iterations_issued  how many iterations' launches the last decode in d_workspace actually issued (reads one
  *                             int back from the workspace on `stream` and WAITS for it; h_iterations: HOST pointer)
  *   qcldpc_last_loop_mode     1 if the last decode call of this thread ran as a graph, 0 if as stream launches

@@ -994,7 +994,11 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
 
     // ---- graph path
     const int body = loop_body_len(code, n_frames);
-    if (code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2) {
+    // (a caller that is itself capturing `stream` into a graph gets the plain launches: they become nodes of ITS graph)
+    cudaStreamCaptureStatus caller_capture = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &caller_capture) != cudaSuccess) { cudaGetLastError(); caller_capture = cudaStreamCaptureStatusNone; }
+    if (code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2 &&
+        caller_capture == cudaStreamCaptureStatusNone) {
         int dev = 0;
         CUDA_TRY(cudaGetDevice(&dev));
         const GraphKey key{d_llr, d_syndrome, d_hard, d_iters, d_pass, d_posterior, d_workspace,

@@ -451,6 +451,28 @@ def test_device_loop_stops_issuing_when_the_batch_has_stopped(B):
     assert code.iterations_issued(len(stuck), ws2) == 77
 
 
+def test_decode_inside_a_callers_graph_capture(B):
+    """A caller that captures its stream into a CUDA graph of its own gets the per-iteration launches as nodes of that
+    graph (no graph launched inside a capture); replaying the captured graph reproduces the plain decode."""
+    cfg, base, Z, fr = W.make_config(1)
+    code = B.QCLDPCCode(base, Z)
+    d_llr = torch.from_numpy(fr.llr).cuda()
+    d_syn = torch.from_numpy(fr.syndrome).cuda()
+    ws = torch.empty(code.workspace_bytes(len(fr.llr)), dtype=torch.uint8, device="cuda")
+    ref = code.decode(d_llr, d_syn, 30, 1, want_posterior=True)
+    torch.cuda.synchronize()
+    out = B.DecodeResult(torch.zeros_like(ref.hard), torch.zeros_like(ref.iters), torch.zeros_like(ref.passed),
+                         torch.zeros_like(ref.posterior))
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        code.decode(d_llr, d_syn, 30, 1, want_posterior=True, workspace=ws, out=out)
+        assert B.qcldpc_last_loop_mode() == 0
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out.hard, ref.hard) and torch.equal(out.iters, ref.iters)
+    assert torch.equal(out.passed, ref.passed) and torch.equal(out.posterior, ref.posterior)
+
+
 def test_gpu_argument_errors(B):
     cfg, base, Z, fr = W.make_config(1, n_frames=2)
     code = B.QCLDPCCode(base, Z)
