@@ -2,7 +2,9 @@
 // ensemble (NEXT-1: circulants of q = 21 or 50, columns of degree 59/60) above all.
 //
 // Layout.  Frames are taken in groups of 32 and interleaved innermost: element (run e, index i, frame f of the group)
-// of any per-edge / per-check / per-variable array lives at ((e * Z + i) * 32 + f).  A warp works on one variable (or
+// of the per-edge and per-check arrays lives at ((e * (Z + 1) + i) * 32 + f): a run is Z lines of 128 bytes plus one
+// HALO line, a copy of the run's line 0 kept by whoever writes line 0, so that the successor of ANY index -- the second
+// variable of a slot -- is the next line, wrap or not.  Per-variable arrays are [A * Z] lines.  A warp works on one variable (or
 // one check; in the pass: a slot of two consecutive variables, shared by two warps) of all 32 frames of a group,
 // lane = frame.  Consequences:
 //   * every access of a warp is one aligned 128-byte line, whatever the circulant size and shift (a cyclic shift by p
@@ -40,21 +42,25 @@ struct IlArgs {
     const int* done; const int32_t* iters; int* topbad; int* unsat;
     const float* q_in; float* q_out;           // regular pass: qb[(t - 1) % 4] -> qb[t % 4]
     const unsigned* hard_in; unsigned* hard_out;   // hardm[(t - 1) % 3] -> hardm[t % 3]
-    int Z, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;
+    int Z, Zp, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;   // Zp = Z + 1: lines per run
     int tp, ctas_per_col;      // k_pass_il: tiles per CTA (one table load serves them all), CTAs per column
     const uint4* blob; int blob16;   // per-column tables in shared-memory layout, blob16 16-byte words per column
-    int64_t n, m, EZ, mZ, AZ;  // E*Z, mb*Z, A*Z (per group, in lines of 32)
+    int64_t n, m, EZ, mZ, AZ;  // E*Zp, mb*Zp, A*Z (per group, in lines of 32)
 };
 
 // Per-column table blob, the same bytes in global and in shared memory, fixed stride, so that a CTA copies it in ONE
 // round trip without first reading where it is: header, then [max_dv] IlEdgeA, [max_dv] GenDesc, [max_dv] IlEdgeB,
-// [max_np] PartnerDesc.
+// [max_np] IlRef.
+// A reference to "line (i + d) mod Z of run e" as the pass wants it: the variable's own line offset 128 i is in the base
+// pointer, so the line is at byte  pre - (128 i >= thr ? 128 Z : 0),  pre = 128 (e (Z + 1) + d),  thr = 128 (Z - d).
+struct IlRef { int pre, thr; };
+inline IlRef il_ref(int64_t run_line0, int d, int Z) { return IlRef{(int)((run_line0 + d) << 7), (Z - d) << 7}; }
 struct IlColHdr { int col, ebeg, dv, ng, ngh, np, pad0, pad1; };
-struct IlEdgeA { int shift, t_off, p_off, delta; };           // first 16 bytes of EdgeDesc (16-byte aligned copy)
-struct IlEdgeB { int p2_off, delta2; };
+struct IlEdgeA { IlRef t, p; };                               // t_c (d = -shift mod Z) and the first partner
+struct IlEdgeB { IlRef p2; };                                 // a triple edge's second partner
 __host__ __device__ inline size_t il_table_bytes(int max_dv, int max_np) {
     const size_t b = sizeof(IlColHdr) + (size_t)(max_dv > 0 ? max_dv : 1) * (sizeof(IlEdgeA) + sizeof(IlEdgeB) + sizeof(GenDesc)) +
-                     (size_t)(max_np > 0 ? max_np : 1) * sizeof(PartnerDesc);
+                     (size_t)(max_np > 0 ? max_np : 1) * sizeof(IlRef);
     return (b + 15) / 16 * 16;
 }
 inline size_t il_smem_bytes(int max_dv, int max_np, int W) {
@@ -73,8 +79,11 @@ template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[4], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : idx == 2 ? p[2] : p[3]; }
 template <class T>
 __device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0 ? p[0] : idx == 1 ? p[1] : p[2]; }
-// byte offset of a line -> pointer, lane already in the base
-__device__ __forceinline__ const float* il_row(const float* base_lane, unsigned byte_off) { return byte_ptr(base_lane, byte_off); }
+// base + a signed byte offset
+__device__ __forceinline__ const float* il_at(const float* base, int byte_off) {
+    return reinterpret_cast<const float*>(reinterpret_cast<const char*>(base) + byte_off);
+}
+__device__ __forceinline__ void il_stg(float* p, unsigned bits) { asm volatile("st.global.b32 [%0], %1;" ::"l"(p), "r"(bits) : "memory"); }
 // line index -> pointer to this lane's float
 __device__ __forceinline__ const float* il_line(const float* base, unsigned line, unsigned lane) {
     return byte_ptr(base, (line * kIlGroup + lane) * 4u);
@@ -111,9 +120,12 @@ __global__ void __launch_bounds__(256) k_il_init_cols(const PassTables tab, cons
         a.qc[((int64_t)g * a.AZ + line) * kIlGroup + lane] = Q2;
         const unsigned mask = __ballot_sync(0xffffffffu, xh != 0);
         if (lane == 0) a.hardm[0][(int64_t)g * a.AZ + line] = mask;
-        float* q0 = a.qb[0] + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * a.Z + i) * kIlGroup + lane;
-        for (int k = 0; k < cd.dv; ++k)
-            q0[(int64_t)k * a.Z * kIlGroup] = __uint_as_float(k < cd.ng ? ((wb & 0xfffffffeu) | xh) : wb);
+        float* q0 = a.qb[0] + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * a.Zp + i) * kIlGroup + lane;
+        for (int k = 0; k < cd.dv; ++k) {
+            const float w0 = __uint_as_float(k < cd.ng ? ((wb & 0xfffffffeu) | xh) : wb);
+            q0[(int64_t)k * a.Zp * kIlGroup] = w0;
+            if (i == 0) q0[((int64_t)k * a.Zp + a.Z) * kIlGroup] = w0;                 // the run's halo line
+        }
     }
 }
 
@@ -142,7 +154,8 @@ __global__ void __launch_bounds__(256) k_il_init_rows(const CheckTables tab, con
     for (int rl = w; rl < 32; rl += 8) {
         const int r = r0 + rl;
         if (r >= a.Z) break;
-        a.t[((int64_t)g * a.mZ + (int64_t)R * a.Z + r) * kIlGroup + lane] = s_t[lane][rl];
+        a.t[((int64_t)g * a.mZ + (int64_t)R * a.Zp + r) * kIlGroup + lane] = s_t[lane][rl];
+        if (r == 0) a.t[((int64_t)g * a.mZ + (int64_t)R * a.Zp + a.Z) * kIlGroup + lane] = s_t[lane][rl];   // halo
     }
 }
 
@@ -164,7 +177,7 @@ __device__ __forceinline__ unsigned il_check_one(const CheckTables& tab, const C
         const int iv = il_wrap(r + re.shift, Z);
         par ^= (hm[re.ca * Z + iv] >> lane) & 1u;
         if (rd.abs_col >= 0 && T > 0) {
-            unsigned wb = __float_as_uint(__ldg(il_line(qprev, (unsigned)(re.edge * Z + iv), lane)));
+            unsigned wb = __float_as_uint(__ldg(il_line(qprev, (unsigned)(re.edge * a.Zp + iv), lane)));
             sg ^= wb & 0x80000000u;
             wb &= rd.gen ? 0x7ffffffeu : 0x7fffffffu;
             boxplus_acc(__uint_as_float(wb), num, den);
@@ -297,7 +310,7 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     const IlEdgeA* const s_a = reinterpret_cast<const IlEdgeA*>(smem_il + sizeof(IlColHdr));
     const GenDesc* const s_g = reinterpret_cast<const GenDesc*>(s_a + mdv);
     const IlEdgeB* const s_b = reinterpret_cast<const IlEdgeB*>(s_g + mdv);
-    const PartnerDesc* const s_p = reinterpret_cast<const PartnerDesc*>(s_b + mdv);
+    const IlRef* const s_p = reinterpret_cast<const IlRef*>(s_b + mdv);
     // FINAL: every frame reads the state of its own last iteration, w^(T-1) in buffer (T - 1) mod 4
     // (the lane is folded into the base pointers: a load address is base + 128 * line)
     const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup + lane;
@@ -305,8 +318,8 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     float* const mm = msg_base + (size_t)slot * V * mdv * kIlGroup + lane;            // m'[v][k][lane] of this slot
     const int vstride = mdv * kIlGroup;
     float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 8 * V * kIlGroup + lane;   // 2 buffers
-    const unsigned ulane = (unsigned)lane;
-    const unsigned step = (unsigned)Z * kIlGroup * 4u;
+    const int Zb = Z << 7;                                    // bytes of the Z lines of a run
+    const unsigned step = (unsigned)a.Zp << 7;                // bytes from a run to the next
     const bool single = dv == 1;                              // a single edge sends Q itself
 
 #pragma unroll 1
@@ -326,27 +339,22 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     float* const xch = xch0 + (tt & 1) * 4 * V * kIlGroup;
     unsigned bad = 0;
 
-    // BYTE offsets of the two variables' lines in a run (the blob's offsets are in bytes: line << 7): index x = (i + d)
-    // mod Z and its successor, which is the run's first line when x is the last one
-    const unsigned step1 = val1 ? 128u : 0u, step_wrap = val1 ? 128u - (unsigned)Z * 128u : 0u;
-    auto two_lines = [&](int off, int x, unsigned (&ln)[V]) {
-        ln[0] = (unsigned)off + ((unsigned)x << 7);
-        ln[1] = ln[0] + (x == Z - 1 ? step_wrap : step1);
-    };
-    auto t_lines = [&](const IlEdgeA& d, unsigned (&ln)[V]) { int r = i0 - d.shift; r += r < 0 ? Z : 0; two_lines(d.t_off, r, ln); };
-    auto p_lines = [&](int off, int delta, unsigned (&ln)[V]) { two_lines(off, il_wrap(i0 + delta, Z), ln); };
+    // the slot's first variable's line in a run comes from an IlRef (its own offset 128 i0 sits in the base pointers);
+    // the second variable's line is the next one (the halo line where the index wraps)
+    const int i0b = i0 << 7;
+    const float* const qT = qP + i0 * kIlGroup;
+    const float* const tT = tP + i0 * kIlGroup;
+    auto at = [&](const float* base, const IlRef r) { return il_at(base, r.pre - (i0b >= r.thr ? Zb : 0)); };
 
     // gen edge: fold every other edge of the row (the rule is associative); bit 0 of a gen edge's state is its
     // variable's hard decision: the XOR of the raw words carries sign AND parity
     auto gen_edge = [&](int k, float (&acc)[V]) {
-        const IlEdgeA d = s_a[k];
         const GenDesc gd = s_g[k];
-        unsigned tl[V];
-        t_lines(d, tl);
+        const float* const tl = at(tT, s_a[k].t);
         float tv[V], num[V], den[V];
         unsigned xa[V];
 #pragma unroll
-        for (int v = 0; v < V; ++v) { tv[v] = __ldg(il_row(tP, tl[v])); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
+        for (int v = 0; v < V; ++v) { tv[v] = __ldg(tl + v * kIlGroup); num[v] = 0.0f; den[v] = 1.0f; xa[v] = 0u; }
         // partners in batches of kGenBatch, all loads of a batch in flight (a check of degree 7, the largest of the
         // paper's ensemble, is one round trip)
         constexpr int kGenBatch = 6;
@@ -356,11 +364,9 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
 #pragma unroll
             for (int u = 0; u < kGenBatch; ++u) {
                 const bool have = jb + u < gd.np;
-                const PartnerDesc p = s_p[gd.pbeg + (have ? jb + u : 0)];
-                unsigned pl[V];
-                p_lines(p.off, p.delta, pl);
+                const float* const pl = at(qT, s_p[gd.pbeg + (have ? jb + u : 0)]);
 #pragma unroll
-                for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(il_row(qP, pl[v])) : 0.0f;   // +0.0: the identity
+                for (int v = 0; v < V; ++v) pm[u][v] = have ? __ldg(pl + v * kIlGroup) : 0.0f;   // +0.0: the identity
             }
 #pragma unroll
             for (int u = 0; u < kGenBatch; ++u)
@@ -388,16 +394,14 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
             const IlEdgeA d = s_a[k0 + j];
-            const IlEdgeB e = s_b[k0 + j];
-            unsigned tl[V], al[V], bl[V];
-            t_lines(d, tl);
-            p_lines(d.p_off, d.delta, al);
-            p_lines(e.p2_off, e.delta2, bl);
+            const float* const tl = at(tT, d.t);
+            const float* const al = at(qT, d.p);
+            const float* const bl = at(qT, s_b[k0 + j].p2);
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                tv[j][v] = __ldg(il_row(tP, tl[v]));
-                pa[j][v] = __ldg(il_row(qP, al[v]));
-                pb[j][v] = __ldg(il_row(qP, bl[v]));
+                tv[j][v] = __ldg(tl + v * kIlGroup);
+                pa[j][v] = __ldg(al + v * kIlGroup);
+                pb[j][v] = __ldg(bl + v * kIlGroup);
             }
         }
 #pragma unroll
@@ -420,13 +424,12 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
             const IlEdgeA d = s_a[k0 + j];
-            unsigned tl[V], pl[V];
-            t_lines(d, tl);
-            p_lines(d.p_off, d.delta, pl);
+            const float* const tl = at(tT, d.t);
+            const float* const pl = at(qT, d.p);
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                tv[j][v] = __ldg(il_row(tP, tl[v]));
-                wv[j][v] = __ldg(il_row(qP, pl[v]));
+                tv[j][v] = __ldg(tl + v * kIlGroup);
+                wv[j][v] = __ldg(pl + v * kIlGroup);
             }
         }
 #pragma unroll
@@ -541,30 +544,41 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     }
     if (ng > 0 && bad != 0 && live) a.topbad[f] = 1;
 
-    // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'
-#pragma unroll
-    for (int v = 0; v < V; ++v) {
-        const bool st = live && (v == 0 || val1);             // nothing of a stopped frame is stored
-        float* const sp = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * Z + (v ? i1 : i0)) * kIlGroup + lane;
-        const float* const mv = mm + v * vstride;
+    // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'; nothing of a
+    // stopped frame is stored.  The slot that holds a run's line 0 also writes the run's halo line (second round).
+    float* const sp0 = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * a.Zp + i0) * kIlGroup + lane;
+#pragma unroll 1
+    for (int round = 0; round < (i0 == 0 ? 2 : 1); ++round) {
+        float* const sp = round ? sp0 + (int64_t)Z * kIlGroup : sp0;
+        const bool st[V] = {live, live && val1 && round == 0};
 #pragma unroll 1
         for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
 #pragma unroll
             for (int gi = 0; gi < GPW; ++gi) {
                 int k, ke;
                 block_of(rnd, gi, k, ke);
-                if (ke - k == kIlChunk) {                     // a whole block: unrolled, the tag of the gen edges branch-free
+                float* pk = byte_ptr(sp, (unsigned)k * step);          // edge k, the slot's first variable
+                const float* mk = mm + k * kIlGroup;
+                if (ke - k == kIlChunk && k >= ng) {          // a whole block without gen edges (no tag): unrolled
 #pragma unroll
                     for (int j = 0; j < kIlChunk; ++j) {
-                        const unsigned tagbit = (k + j < ng) ? 1u : 0u;   // gen edge: bit 0 carries the hard decision
-                        const unsigned wb = __float_as_uint(w_of(L[v] - mv[(k + j) * kIlGroup]));
-                        if (st) *byte_ptr(sp, (unsigned)(k + j) * step) = __uint_as_float((wb & ~tagbit) | (xh[v] & tagbit));
+#pragma unroll
+                        for (int v = 0; v < V; ++v) {
+                            const float wv = w_of(L[v] - mk[v * vstride + j * kIlGroup]);
+                            if (st[v]) il_stg(pk + v * kIlGroup, __float_as_uint(wv));
+                        }
+                        pk = byte_ptr(pk, step);
                     }
                 } else {
                     for (; k < ke; ++k) {
-                        const unsigned tagbit = (k < ng) ? 1u : 0u;
-                        const unsigned wb = __float_as_uint(w_of(single ? Q[v] : L[v] - mv[k * kIlGroup]));
-                        if (st) *byte_ptr(sp, (unsigned)k * step) = __uint_as_float((wb & ~tagbit) | (xh[v] & tagbit));
+                        const unsigned tagbit = (k < ng) ? 1u : 0u;   // gen edge: bit 0 carries the hard decision
+#pragma unroll
+                        for (int v = 0; v < V; ++v) {
+                            const unsigned wb = __float_as_uint(w_of(single ? Q[v] : L[v] - mk[v * vstride]));
+                            if (st[v]) il_stg(pk + v * kIlGroup, (wb & ~tagbit) | (xh[v] & tagbit));
+                        }
+                        pk = byte_ptr(pk, step);
+                        mk += kIlGroup;
                     }
                 }
             }
@@ -618,7 +632,7 @@ __global__ void __launch_bounds__(256) k_il_check_final(const CheckTables tab, c
                 const int iv = il_wrap(r + re.shift, Z);
                 par ^= (hm[re.ca * Z + iv] >> lane) & 1u;
                 if (rd.abs_col >= 0) {
-                    unsigned wb = __float_as_uint(__ldg(il_line(qprev, (unsigned)(re.edge * Z + iv), (unsigned)lane)));
+                    unsigned wb = __float_as_uint(__ldg(il_line(qprev, (unsigned)(re.edge * a.Zp + iv), (unsigned)lane)));
                     sg ^= wb & 0x80000000u;
                     wb &= rd.gen ? 0x7ffffffeu : 0x7fffffffu;         // gen edges carry a tag in bit 0
                     boxplus_acc(__uint_as_float(wb), num, den);

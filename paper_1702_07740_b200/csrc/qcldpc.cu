@@ -322,8 +322,8 @@ Workspace carve(const qcldpc_code* code, int n_frames, void* base) {
     const size_t fbytes = align_up((size_t)n_frames * sizeof(int), 256);
     if (w.il) {
         const size_t lines = (size_t)w.n_groups * kIlGroup * sizeof(float);            // bytes per line index
-        const size_t qbytes = align_up(lines * code->n_act_edges * code->Z, 256);
-        const size_t tbytes = align_up(lines * code->mb * code->Z, 256);
+        const size_t qbytes = align_up(lines * code->n_act_edges * (code->Z + 1), 256);    // runs of Z lines + the halo line
+        const size_t tbytes = align_up(lines * code->mb * (code->Z + 1), 256);
         const size_t cbytes = align_up(lines * code->n_act_cols * code->Z, 256);
         const size_t hbytes = align_up((size_t)w.n_groups * code->n_act_cols * code->Z * sizeof(unsigned), 256);
         for (int b = 0; b < 4; ++b) { w.qbuf[b] = reinterpret_cast<float*>(p + off); off += qbytes; }
@@ -553,17 +553,19 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         tn.il_tp = std::max(0, env_int("QCLDPC_ILTP", 0));
     }
 
-    // frame-interleaved family: offsets in lines of 32 frames, runs of exactly Z lines
+    // frame-interleaved family: offsets in lines of 32 frames, runs of Z lines + one halo line (pass_il.cuh)
+    const int Zp = Z + 1;
     code->edge_il = code->edge;
     for (EdgeDesc& d : code->edge_il) {
-        d.t_off = d.t_off / Zs * Z;
-        if (d.p_off >= 0) d.p_off = d.p_off / Zs * Z;
-        if (d.p2_off >= 0) d.p2_off = d.p2_off / Zs * Z;
+        d.t_off = d.t_off / Zs * Zp;
+        if (d.p_off >= 0) d.p_off = d.p_off / Zs * Zp;
+        if (d.p2_off >= 0) d.p2_off = d.p2_off / Zs * Zp;
     }
     code->partner_il = code->partner;
-    for (PartnerDesc& d : code->partner_il) d.off = d.off / Zs * Z;
-    code->il_ok = !exact && code->n_act_cols > 0 && (int64_t)code->n_act_edges * Z < ((int64_t)1 << 25) &&
-                  (int64_t)mb * Z < ((int64_t)1 << 25) &&
+    for (PartnerDesc& d : code->partner_il) d.off = d.off / Zs * Zp;
+    // byte offsets of lines within a group are signed 32-bit in the pass
+    code->il_ok = !exact && code->n_act_cols > 0 && (int64_t)code->n_act_edges * Zp < ((int64_t)1 << 24) &&
+                  (int64_t)mb * Zp < ((int64_t)1 << 24) &&
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
     if (const int wf = env_int("QCLDPC_ILW", 0)) {         // tuning knob: variables per tile of k_pass_il (even, <= 12)
@@ -584,17 +586,18 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
             IlEdgeA* ea = reinterpret_cast<IlEdgeA*>(base + sizeof(IlColHdr));
             GenDesc* eg = reinterpret_cast<GenDesc*>(ea + mdv);
             IlEdgeB* eb = reinterpret_cast<IlEdgeB*>(eg + mdv);
-            PartnerDesc* ep = reinterpret_cast<PartnerDesc*>(eb + mdv);
+            IlRef* ep = reinterpret_cast<IlRef*>(eb + mdv);
+            const IlRef none{0, 0};
             for (int k = 0; k < cd.dv; ++k) {
                 const EdgeDesc& d = code->edge_il[cd.ebeg + k];
-                // offsets of the blob are BYTE offsets of lines (line << 7; below 2^32 by il_ok)
-                ea[k] = IlEdgeA{d.shift, (int)((unsigned)d.t_off << 7), d.p_off >= 0 ? (int)((unsigned)d.p_off << 7) : -1, d.delta};
-                eb[k] = IlEdgeB{d.p2_off >= 0 ? (int)((unsigned)d.p2_off << 7) : -1, d.delta2};
+                // t_c of variable i is check (i - shift) mod Z; byte offsets of lines stay below 2^31 by il_ok
+                ea[k] = IlEdgeA{il_ref(d.t_off, (Z - d.shift) % Z, Z), d.p_off >= 0 ? il_ref(d.p_off, d.delta, Z) : none};
+                eb[k] = IlEdgeB{d.p2_off >= 0 ? il_ref(d.p2_off, d.delta2, Z) : none};
             }
             for (int k = 0; k < cd.ng; ++k) eg[k] = code->gen[cd.gbeg + k];
             for (int k = 0; k < cd.np; ++k) {
-                ep[k] = code->partner_il[cd.pbeg + k];
-                ep[k].off = (int)((unsigned)ep[k].off << 7);
+                const PartnerDesc& pd = code->partner_il[cd.pbeg + k];
+                ep[k] = il_ref(pd.off, pd.delta, Z);
             }
         }
     }
@@ -969,7 +972,8 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     P.merge_check = code->tune.merge_check != 0;
     P.il = w.il;
     if (P.il) {
-        const int64_t EZ = (int64_t)code->n_act_edges * Z, mZ = (int64_t)code->mb * Z, AZ = (int64_t)code->n_act_cols * Z;
+        const int64_t EZ = (int64_t)code->n_act_edges * (Z + 1), mZ = (int64_t)code->mb * (Z + 1),
+                      AZ = (int64_t)code->n_act_cols * Z;
         IlArgs ia{};
         ia.llr = d_llr; ia.syn = d_syndrome;
         for (int b = 0; b < 4; ++b) ia.qb[b] = w.qbuf[b];
@@ -978,7 +982,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         ia.hardm_final = w.hardm[3];
         ia.d_hard = d_hard; ia.d_post = d_posterior;
         ia.done = w.done; ia.iters = d_iters; ia.topbad = nullptr; ia.unsat = w.unsat;
-        ia.Z = Z; ia.W = code->il_w; ia.tiles = (Z + code->il_w - 1) / code->il_w;
+        ia.Z = Z; ia.Zp = Z + 1; ia.W = code->il_w; ia.tiles = (Z + code->il_w - 1) / code->il_w;
         ia.n_frames = n_frames; ia.n_groups = w.n_groups; ia.n_cols = code->n_act_cols; ia.mb = code->mb;
         ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
         ia.max_np = code->max_np;
