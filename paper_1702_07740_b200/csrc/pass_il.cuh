@@ -268,8 +268,10 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 // chains of 28 and 32 edges; the two warps meet once per tile to exchange their partial sums.  H = 1 (G = 1): one warp.
 constexpr int kIlV = 2;
 
-template <bool FINAL, int H, int GPW>
-__global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
+// MAXT: threads per CTA the instance is compiled for; 320 (tiles of up to 10 variables with H = 2) leaves 102 registers
+// per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time
+template <bool FINAL, int H, int GPW, int MAXT>
+__global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                     const CheckArgs chk) {
     constexpr int G = H * GPW;
     constexpr int V = kIlV;
@@ -287,12 +289,13 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     const int warp = il_warp_id(), lane = threadIdx.x & 31;
     const int slot = warp / H, h = warp - slot * H;
     const int mdv = a.max_dv;
-    // prologue: the column's tables (constant: not the previous launch's output) in one round trip
-    {
-        const uint4* __restrict__ src = a.blob + (size_t)ca * a.blob16;
-        uint4* dst = reinterpret_cast<uint4*>(smem_il);
-        for (int k = threadIdx.x; k < a.blob16; k += blockDim.x) dst[k] = __ldg(src + k);
-    }
+    // prologue: the column's tables (constant: not the previous launch's output) in one round trip; their first loads
+    // are issued before, and land in shared memory after, the loads of the stop flags
+    const uint4* __restrict__ blob_src = a.blob + (size_t)ca * a.blob16;
+    uint4* const blob_dst = reinterpret_cast<uint4*>(smem_il);
+    const bool blob_first = (int)threadIdx.x < a.blob16;
+    uint4 blob0 = uint4{0u, 0u, 0u, 0u};
+    if (blob_first) blob0 = __ldg(blob_src + threadIdx.x);
     float* const msg_base = reinterpret_cast<float*>(smem_il + (il_table_bytes(mdv, a.max_np) + 127) / 128 * 128);
     int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdv + 8) * kIlGroup);
     if (threadIdx.x < 32) s_flag[threadIdx.x] = 0;
@@ -301,6 +304,8 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     const int fc = in_range ? f : a.n_frames - 1;
     pdl_wait();                                               // from here on: memory the previous launch wrote
     const int flag = FINAL ? a.iters[fc] : a.done[fc];
+    if (blob_first) blob_dst[threadIdx.x] = blob0;
+    for (int k = threadIdx.x + blockDim.x; k < a.blob16; k += blockDim.x) blob_dst[k] = __ldg(blob_src + k);
     __syncthreads();
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
     if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped (both warps of a
@@ -329,15 +334,18 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
     const bool val1 = i0 + 1 < Z;                             // the slot's second variable exists (else: computed on the
     const int i1 = val1 ? i0 + 1 : i0;                        // first one's data, nothing of it is stored)
     const unsigned line_v[V] = {(unsigned)(ca * Z + i0), (unsigned)(ca * Z + i1)};
-    unsigned xb[V];
+    // the variables' own values: loaded here, first used after the edges (no load of the edge loop waits for them)
+    unsigned hin[V];
     float Q[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-        xb[v] = FINAL ? 0u : (a.hard_in[(int64_t)g * a.AZ + line_v[v]] >> lane) & 1u;
+        hin[v] = FINAL ? 0u : a.hard_in[(int64_t)g * a.AZ + line_v[v]];
         Q[v] = a.qc[((int64_t)g * a.AZ + line_v[v]) * kIlGroup + lane];
     }
     float* const xch = xch0 + (tt & 1) * 4 * V * kIlGroup;
-    unsigned bad = 0;
+    // parities of the reporting gen rows without the variable's own decision x: bit v of odd / even = some row of
+    // variable v has odd / even parity of the others; the row fails iff its parity differs from ... x (joined below)
+    unsigned odd = 0, even = 0;
 
     // the slot's first variable's line in a run comes from an IlRef (its own offset 128 i0 sits in the base pointers);
     // the second variable's line is the next one (the halo line where the index wraps)
@@ -379,8 +387,11 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
         }
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            if (!FINAL && gd.counter && (v == 0 || val1))   // parity of the row at the input iteration (t = (-1)^{s_c} 0)
-                bad |= ((xa[v] ^ xb[v] ^ (__float_as_uint(tv[v]) >> 31)) & 1u) << v;
+            if (!FINAL && gd.counter && (v == 0 || val1)) {   // parity of the row at the input iteration (t = (-1)^{s_c} 0)
+                const unsigned par = (xa[v] ^ (__float_as_uint(tv[v]) >> 31)) & 1u;
+                odd |= par << v;
+                even |= (par ^ 1u) << v;
+            }
             boxplus_acc(fabsf(tv[v]), num[v], den[v]);
             const float mk = with_sign(mag_of(num[v], den[v]), (xa[v] ^ __float_as_uint(tv[v])) & 0x80000000u);
             mm[v * vstride + k * kIlGroup] = mk;
@@ -466,7 +477,11 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
             for (int v = 0; v < V; ++v) acc[v] = part[gi][v];
             const int e1 = min(ke, ngh), e3 = min(ke, ng);
             for (; k < e1; ++k) gen_edge(k, acc);
-            if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
+            if (MAXT <= 320) {
+                if (k + 8 <= e3) { triple(I8{}, k, acc); k += 8; }
+            } else {
+                if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
+            }
             if (k + 4 <= e3) { triple(I4{}, k, acc); k += 4; }
             for (; k < e3; ++k) triple(I1{}, k, acc);
             if (k + 8 <= ke) { pair(I8{}, k, acc); k += 8; }
@@ -500,9 +515,11 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
         __syncwarp();
         if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + slot * 2 + h), "r"(tt + 1) : "memory");
         int seen;
-        do {
+        for (;;) {
             asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + slot * 2 + (1 - h)) : "memory");
-        } while (seen < tt + 1);
+            if (seen >= tt + 1) break;
+            __nanosleep(40);                                  // leave the issue slots to the partner
+        }
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             sum[v] = 0.0f;
@@ -542,7 +559,12 @@ __global__ void __launch_bounds__(384, 2) k_pass_il(const PassTables tab, const 
             if (lane == 0 && (v == 0 || val1)) a.hard_out[(int64_t)g * a.AZ + line_v[v]] = mask;
         }
     }
-    if (ng > 0 && bad != 0 && live) a.topbad[f] = 1;
+    if (ng > 0 && live) {                                     // a reporting row fails iff (parity of the others) ^ x = 1
+        unsigned bad = 0;
+#pragma unroll
+        for (int v = 0; v < V; ++v) bad |= ((hin[v] >> lane) & 1u) ? (even >> v) & 1u : (odd >> v) & 1u;
+        if (bad) a.topbad[f] = 1;
+    }
 
     // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'; nothing of a
     // stopped frame is stored.  The slot that holds a run's line 0 also writes the run's halo line (second round).
@@ -692,7 +714,7 @@ inline int il_pick_w(int Z, int max_dv, int max_np) {
 inline int il_pick_tp(int, int, int, int) { return 1; }
 
 #ifdef QC_IL_IMPL
-template <int H, int GPW>
+template <int H, int GPW, int MAXT>
 inline void launch_pass_il_h(const IlLaunch& L) {
     IlArgs args = L.args;
     const size_t smem = il_smem_bytes(args.max_dv, args.max_np, args.W);
@@ -700,8 +722,8 @@ inline void launch_pass_il_h(const IlLaunch& L) {
     int dev = 0;
     cudaGetDevice(&dev);
     if (attr_dev != dev) {
-        cudaFuncSetAttribute(k_pass_il<true, H, GPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
-        cudaFuncSetAttribute(k_pass_il<false, H, GPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<true, H, GPW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<false, H, GPW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
         attr_dev = dev;
     }
     if (L.prepare_only) return;
@@ -713,16 +735,20 @@ inline void launch_pass_il_h(const IlLaunch& L) {
     static const CheckArgs no_args{};
     const dim3 grid(work + extra, args.n_groups), block(32 * H * (args.W / 2));
     if (L.final_mode)
-        k_pass_il<true, H, GPW><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
+        k_pass_il<true, H, GPW, MAXT><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
     else
-        launch_pdl(k_pass_il<false, H, GPW>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
+        launch_pdl(k_pass_il<false, H, GPW, MAXT>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
                    with_check ? *L.check : no_args);
 }
 
 // long columns (four partial sums): two warps per variable; short ones: one warp, one sum
 inline void launch_pass_il(const IlLaunch& L) {
-    if (L.args.split == 4) launch_pass_il_h<2, 2>(L);
-    else launch_pass_il_h<1, 1>(L);
+    if (L.args.split == 4) {
+        if (32 * 2 * (L.args.W / 2) <= 320) launch_pass_il_h<2, 2, 320>(L);
+        else launch_pass_il_h<2, 2, 384>(L);
+    } else {
+        launch_pass_il_h<1, 1, 384>(L);
+    }
 }
 #endif
 
