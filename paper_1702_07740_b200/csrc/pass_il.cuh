@@ -42,8 +42,8 @@ struct IlArgs {
     const int* done; const int32_t* iters; int* topbad; int* unsat;
     const float* q_in; float* q_out;           // regular pass: qb[(t - 1) % 4] -> qb[t % 4]
     const unsigned* hard_in; unsigned* hard_out;   // hardm[(t - 1) % 3] -> hardm[t % 3]
-    int Z, Zp, W, tiles, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;   // Zp = Z + 1: lines per run
-    int tp, ctas_per_col;      // k_pass_il: tiles per CTA (one table load serves them all), CTAs per column
+    int Z, Zp, W, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;   // Zp = Z + 1: lines per run
+    int spc, ipc;              // k_pass_il: slots (pairs of variables) per column, slots per CTA (<= spc, <= W / 2)
     const uint4* blob; int blob16;   // per-column tables in shared-memory layout, blob16 16-byte words per column
     int64_t n, m, EZ, mZ, AZ;  // E*Zp, mb*Zp, A*Z (per group, in lines of 32)
 };
@@ -63,9 +63,12 @@ __host__ __device__ inline size_t il_table_bytes(int max_dv, int max_np) {
                      (size_t)(max_np > 0 ? max_np : 1) * sizeof(IlRef);
     return (b + 15) / 16 * 16;
 }
+__host__ __device__ inline size_t il_tables_bytes(int max_dv, int max_np) {           // a CTA's slots lie in at most two columns
+    return (2 * il_table_bytes(max_dv, max_np) + 127) / 128 * 128;
+}
 inline size_t il_smem_bytes(int max_dv, int max_np, int W) {
-    return (il_table_bytes(max_dv, max_np) + 127) / 128 * 128 +
-           (size_t)W * ((max_dv > 0 ? max_dv : 1) + 8) * kIlGroup * sizeof(float) +   // messages + 2 x 4 partial sums per variable
+    return il_tables_bytes(max_dv, max_np) +
+           (size_t)W * ((max_dv > 0 ? max_dv : 1) + 4) * kIlGroup * sizeof(float) +   // messages + 4 partial sums per variable
            128;                                                                        // handshake flags of the warp pairs
 }
 
@@ -258,17 +261,20 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 
 // ---- a1 + a2: the fused pass ------------------------------------------------------------------------------------------
 // CTA = S slots x H warps; a slot = V = 2 consecutive variables of one active column, carried by the same threads (the
-// table lookups, window indices and loop control -- most of this kernel's instructions -- serve both); a tile = W = 2 S
-// variables; grid = (columns * CTAs per column [+ check workers], groups).
-// Shared memory: the column's tables, the messages m'[W][max_dv][32], the partial sums, the handshake counters.
+// table lookups, window indices and loop control -- most of this kernel's instructions -- serve both).  The slots of all
+// active columns are numbered through (spc = ceil(Z / 2) per column) and CTA b takes the slots [b ipc, (b + 1) ipc),
+// ipc = min(S, spc): no slot of a CTA idles because Z is not a multiple of the CTA's width (q = 21: 11 slots per column,
+// 5 per CTA), and the slots of a CTA lie in at most two columns, whose tables it loads; grid = (ceil(columns * spc / ipc)
+// [+ check workers], groups).
+// Shared memory: the tables of two columns, the messages m'[2 S][max_dv][32], the partial sums, the handshake counters.
 // The messages of a column are added as the generic pass adds them: block b = k / 8 of the column's edges belongs to
 // partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = 4 for long columns (max_dv > 16), else 1; inside a partial sum k
 // increases; the partial sums meet in the order 0 .. G-1.  H = 2 (G = 4): warp h of a slot owns the partial sums 2h and
 // 2h + 1 -- and with them the edges, their loads, their messages and their stores --, so a column of degree 60 is two
-// chains of 28 and 32 edges; the two warps meet once per tile to exchange their partial sums.  H = 1 (G = 1): one warp.
+// chains of 28 and 32 edges; the two warps meet once to exchange their partial sums.  H = 1 (G = 1): one warp.
 constexpr int kIlV = 2;
 
-// MAXT: threads per CTA the instance is compiled for; 320 (tiles of up to 10 variables with H = 2) leaves 102 registers
+// MAXT: threads per CTA the instance is compiled for; 320 (up to five slots with H = 2) leaves 102 registers
 // per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time
 template <bool FINAL, int H, int GPW, int MAXT>
 __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
@@ -284,35 +290,37 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
         return;
     }
     const int Z = a.Z, g = blockIdx.y;
-    const int ca = blockIdx.x / a.ctas_per_col;
-    const int tile0 = (blockIdx.x - ca * a.ctas_per_col) * a.tp;
     const int warp = il_warp_id(), lane = threadIdx.x & 31;
     const int slot = warp / H, h = warp - slot * H;
     const int mdv = a.max_dv;
-    // prologue: the column's tables (constant: not the previous launch's output) in one round trip; their first loads
-    // are issued before, and land in shared memory after, the loads of the stop flags
-    const uint4* __restrict__ blob_src = a.blob + (size_t)ca * a.blob16;
-    uint4* const blob_dst = reinterpret_cast<uint4*>(smem_il);
-    const bool blob_first = (int)threadIdx.x < a.blob16;
-    uint4 blob0 = uint4{0u, 0u, 0u, 0u};
-    if (blob_first) blob0 = __ldg(blob_src + threadIdx.x);
-    float* const msg_base = reinterpret_cast<float*>(smem_il + (il_table_bytes(mdv, a.max_np) + 127) / 128 * 128);
-    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdv + 8) * kIlGroup);
+    const int item0 = blockIdx.x * a.ipc, item = item0 + slot;            // slots of all columns, numbered through
+    const int ca0 = item0 / a.spc;                                         // the CTA's first column
+    const bool has = slot < a.ipc && item < a.n_cols * a.spc;
+    const int ca = has ? item / a.spc : ca0;
+    const int i0 = (item - ca * a.spc) * kIlV;
+    // prologue: the tables of the CTA's (at most two) columns, constant data, in one round trip
+    {
+        const int n16 = (ca0 + 1 < a.n_cols ? 2 : 1) * a.blob16;
+        const uint4* __restrict__ src = a.blob + (size_t)ca0 * a.blob16;
+        uint4* const dst = reinterpret_cast<uint4*>(smem_il);
+        for (int k = threadIdx.x; k < n16; k += blockDim.x) dst[k] = __ldg(src + k);
+    }
+    float* const msg_base = reinterpret_cast<float*>(smem_il + il_tables_bytes(mdv, a.max_np));
+    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdv + 4) * kIlGroup);
     if (threadIdx.x < 32) s_flag[threadIdx.x] = 0;
     const int f = g * kIlGroup + lane;
     const bool in_range = f < a.n_frames;
     const int fc = in_range ? f : a.n_frames - 1;
     pdl_wait();                                               // from here on: memory the previous launch wrote
     const int flag = FINAL ? a.iters[fc] : a.done[fc];
-    if (blob_first) blob_dst[threadIdx.x] = blob0;
-    for (int k = threadIdx.x + blockDim.x; k < a.blob16; k += blockDim.x) blob_dst[k] = __ldg(blob_src + k);
     __syncthreads();
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
-    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped (both warps of a
-                                                              // slot see the same frames and leave together)
-    const IlColHdr cd = *reinterpret_cast<const IlColHdr*>(smem_il);
+    if (!has) return;                                         // (both warps of a slot leave together)
+    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped
+    const unsigned char* const tbl = smem_il + (size_t)(ca - ca0) * il_table_bytes(mdv, a.max_np);
+    const IlColHdr cd = *reinterpret_cast<const IlColHdr*>(tbl);
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
-    const IlEdgeA* const s_a = reinterpret_cast<const IlEdgeA*>(smem_il + sizeof(IlColHdr));
+    const IlEdgeA* const s_a = reinterpret_cast<const IlEdgeA*>(tbl + sizeof(IlColHdr));
     const GenDesc* const s_g = reinterpret_cast<const GenDesc*>(s_a + mdv);
     const IlEdgeB* const s_b = reinterpret_cast<const IlEdgeB*>(s_g + mdv);
     const IlRef* const s_p = reinterpret_cast<const IlRef*>(s_b + mdv);
@@ -322,15 +330,11 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
     const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup + lane;
     float* const mm = msg_base + (size_t)slot * V * mdv * kIlGroup + lane;            // m'[v][k][lane] of this slot
     const int vstride = mdv * kIlGroup;
-    float* const xch0 = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 8 * V * kIlGroup + lane;   // 2 buffers
+    float* const xch = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 4 * V * kIlGroup + lane;
     const int Zb = Z << 7;                                    // bytes of the Z lines of a run
     const unsigned step = (unsigned)a.Zp << 7;                // bytes from a run to the next
     const bool single = dv == 1;                              // a single edge sends Q itself
 
-#pragma unroll 1
-    for (int tt = 0; tt < a.tp; ++tt) {
-    const int i0 = (tile0 + tt) * a.W + slot * V;
-    if (tile0 + tt >= a.tiles || i0 >= Z) break;              // both warps of a slot leave together
     const bool val1 = i0 + 1 < Z;                             // the slot's second variable exists (else: computed on the
     const int i1 = val1 ? i0 + 1 : i0;                        // first one's data, nothing of it is stored)
     const unsigned line_v[V] = {(unsigned)(ca * Z + i0), (unsigned)(ca * Z + i1)};
@@ -342,7 +346,6 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
         hin[v] = FINAL ? 0u : a.hard_in[(int64_t)g * a.AZ + line_v[v]];
         Q[v] = a.qc[((int64_t)g * a.AZ + line_v[v]) * kIlGroup + lane];
     }
-    float* const xch = xch0 + (tt & 1) * 4 * V * kIlGroup;
     // parities of the reporting gen rows without the variable's own decision x: bit v of odd / even = some row of
     // variable v has odd / even parity of the others; the row fails iff its parity differs from ... x (joined below)
     unsigned odd = 0, even = 0;
@@ -510,14 +513,13 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
 #pragma unroll
             for (int v = 0; v < V; ++v) xch[((h * GPW + gi) * V + v) * kIlGroup] = part[gi][v];
         // the two warps of this slot meet here: release / acquire on a counter in shared memory (a named barrier per
-        // slot would pin all 16 hardware barriers of the CTA); tile tt + 1 uses the other buffer of partial sums, and a
-        // warp cannot be more than one exchange ahead of its partner
+        // slot would pin all 16 hardware barriers of the CTA)
         __syncwarp();
-        if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + slot * 2 + h), "r"(tt + 1) : "memory");
+        if (lane == 0) asm volatile("st.release.cta.s32 [%0], %1;" ::"l"(s_flag + slot * 2 + h), "r"(1) : "memory");
         int seen;
         for (;;) {
             asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + slot * 2 + (1 - h)) : "memory");
-            if (seen >= tt + 1) break;
+            if (seen >= 1) break;
             __nanosleep(40);                                  // leave the issue slots to the partner
         }
 #pragma unroll
@@ -535,7 +537,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
         xh[v] = __float_as_uint(L[v]) >> 31;                  // 0 iff L_v >= 0
     }
     if (FINAL) {
-        if (h != 0) continue;
+        if (h != 0) return;
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             if (live) {
@@ -550,7 +552,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
             const unsigned mask = __ballot_sync(0xffffffffu, xh[v] != 0);
             if (lane == 0 && (v == 0 || val1)) a.hardm_final[(int64_t)g * a.AZ + line_v[v]] = mask;
         }
-        continue;
+        return;
     }
     if (h == 0) {
 #pragma unroll
@@ -606,7 +608,6 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
             }
         }
     }
-    }   // tiles of this CTA
 }
 
 // ---- a4: every check of every frame on the frame's frozen state (iteration d_iters[f]) -------------------------------
@@ -693,25 +694,15 @@ struct IlLaunch {
     bool final_mode; int n_sm, prepare_only;
 };
 
-// variables per tile (an even number: slots of two): the width whose last tile idles the fewest warps, as wide as 12
-// warps and the shared-memory budget allow (the table load of a CTA serves all of them); H warps per slot
+// variables per CTA (an even number: slots of two): H warps per slot; long columns (H = 2) take five slots -- the
+// 320-thread instance, two CTAs of 10 warps per multiprocessor --, short ones up to twelve; never more slots than a
+// column has, and two CTAs per multiprocessor must fit the shared memory
 inline int il_pick_w(int Z, int max_dv, int max_np) {
-    const int H = max_dv > 2 * kIlChunk ? 2 : 1, smax = 12 / H;
-    int best = 2;
-    double best_cost = 1e30;
-    for (int sl = 1; sl <= smax; ++sl) {
-        const int w = 2 * sl;
-        if (il_smem_bytes(max_dv, max_np, w) > 110 * 1024) break;       // two CTAs per multiprocessor
-        const int tiles = (Z + w - 1) / w;
-        const double waste = (double)(tiles * w - Z) / (double)(tiles * w);
-        const double cost = waste + 0.03 * (smax - sl);        // a narrow CTA pays its table load for few variables
-        if (cost < best_cost - 1e-12) { best_cost = cost; best = w; }
-    }
-    return best;
+    const int H = max_dv > 2 * kIlChunk ? 2 : 1, spc = (Z + 1) / 2;
+    int sl = std::min(spc, H == 2 ? 5 : 12);
+    while (sl > 1 && il_smem_bytes(max_dv, max_np, 2 * sl) > 110 * 1024) --sl;
+    return 2 * sl;
 }
-// tiles per CTA: one.  Measured (q = 50, 32 frames, ms per launch): 1 tile 0.273, 2 tiles 0.284, 3 tiles 0.294, 5 tiles
-// (a whole column) 0.300 -- fewer, longer CTAs balance worse than the table load they save; QCLDPC_ILTP overrides.
-inline int il_pick_tp(int, int, int, int) { return 1; }
 
 #ifdef QC_IL_IMPL
 template <int H, int GPW, int MAXT>
@@ -728,7 +719,7 @@ inline void launch_pass_il_h(const IlLaunch& L) {
     }
     if (L.prepare_only) return;
     const bool with_check = !L.final_mode && L.check != nullptr;
-    const int work = args.n_cols * args.ctas_per_col;
+    const int work = (args.n_cols * args.spc + args.ipc - 1) / args.ipc;
     const int extra = with_check ? (2 * L.n_sm + args.n_groups - 1) / args.n_groups : 0;
     args.cand_x = with_check ? work : -1;
     static const CheckTables no_tab{nullptr, nullptr};

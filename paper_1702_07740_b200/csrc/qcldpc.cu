@@ -87,7 +87,6 @@ struct Tuning {
     int loop_graph = 1;                   // QCLDPC_LOOP=stream: one launch per iteration from the host, no graph
     int body_mult = 0;                    // QCLDPC_BODY=k: the graph loop's body is 12 k iterations (0: by batch size)
     int il = 1;                           // QCLDPC_IL=0: never the frame-interleaved family; 2: for every batch size
-    int il_tp = 0;                        // QCLDPC_ILTP=k: tiles per CTA of k_pass_il (0: by grid size)
 };
 
 // One instantiated decode graph per argument tuple (the kernel parameters are baked into the graph's nodes).
@@ -550,7 +549,6 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
         tn.loop_graph = !(lp && strcmp(lp, "stream") == 0);
         tn.body_mult = std::min(16, std::max(0, env_int("QCLDPC_BODY", 0)));
         tn.il = std::min(2, std::max(0, env_int("QCLDPC_IL", 1)));
-        tn.il_tp = std::max(0, env_int("QCLDPC_ILTP", 0));
     }
 
     // frame-interleaved family: offsets in lines of 32 frames, runs of Z lines + one halo line (pass_il.cuh)
@@ -568,7 +566,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
                   (int64_t)mb * Zp < ((int64_t)1 << 24) &&
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
-    if (const int wf = env_int("QCLDPC_ILW", 0)) {         // tuning knob: variables per tile of k_pass_il (even, <= 12)
+    if (const int wf = env_int("QCLDPC_ILW", 0)) {         // tuning knob: variables per CTA of k_pass_il (even, <= 12)
         if (wf >= 2 && wf <= (code->max_dv > 2 * kIlChunk ? 12 : 24) && wf % 2 == 0 &&
             il_smem_bytes(code->max_dv, max_np, wf) <= (size_t)200 * 1024)
             code->il_w = wf;
@@ -982,13 +980,11 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         ia.hardm_final = w.hardm[3];
         ia.d_hard = d_hard; ia.d_post = d_posterior;
         ia.done = w.done; ia.iters = d_iters; ia.topbad = nullptr; ia.unsat = w.unsat;
-        ia.Z = Z; ia.Zp = Z + 1; ia.W = code->il_w; ia.tiles = (Z + code->il_w - 1) / code->il_w;
+        ia.Z = Z; ia.Zp = Z + 1; ia.W = code->il_w;
+        ia.spc = (Z + 1) / 2; ia.ipc = std::min(code->il_w / 2, ia.spc);
         ia.n_frames = n_frames; ia.n_groups = w.n_groups; ia.n_cols = code->n_act_cols; ia.mb = code->mb;
         ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
         ia.max_np = code->max_np;
-        ia.tp = il_pick_tp(code->n_act_cols, ia.tiles, w.n_groups, code->n_sm);
-        if (code->tune.il_tp > 0) ia.tp = std::min(code->tune.il_tp, ia.tiles);
-        ia.ctas_per_col = (ia.tiles + ia.tp - 1) / ia.tp;
         ia.blob = code->d_il_blob; ia.blob16 = code->il_blob16;
         ia.n = code->n; ia.m = code->m; ia.EZ = EZ; ia.mZ = mZ; ia.AZ = AZ;
         P.ill = IlLaunch{PassTables{code->d_edge_il, code->d_gen, code->d_partner_il, code->d_col}, P.ctab, ia, st,
