@@ -619,6 +619,7 @@ __global__ void __launch_bounds__(256) k_il_check_final(const CheckTables tab, c
     __shared__ float s_post[kIlGroup][33];
     __shared__ unsigned char s_syn[kIlGroup][36];
     __shared__ unsigned char s_xj[kIlGroup][36];
+    __shared__ int s_bad[8][kIlGroup];
     const int g = blockIdx.y, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int Z = a.Z;
     const int tiles32 = (Z + 31) / 32;
@@ -650,6 +651,7 @@ __global__ void __launch_bounds__(256) k_il_check_final(const CheckTables tab, c
             unsigned par = s_syn[lane][rl];
             unsigned sg = par << 31;
             float num = 0.0f, den = 1.0f;
+#pragma unroll 4
             for (int k = 0; k < rd.ne; ++k) {
                 const RowEdge re = tab.redge[rd.ebeg + k];
                 const int iv = il_wrap(r + re.shift, Z);
@@ -672,10 +674,16 @@ __global__ void __launch_bounds__(256) k_il_check_final(const CheckTables tab, c
             }
             nbad += in_range ? (int)par : 0;
         }
-        if (nbad) atomicAdd(a.unsat + f, nbad);
+        s_bad[w][lane] = nbad;
+    }
+    __syncthreads();
+    if (w == 0) {                                             // one atomic per frame and CTA (thousands of CTAs, 32 addresses)
+        int nbad = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) nbad += s_bad[k][lane];
+        if (nbad) atomicAdd(a.unsat + g * kIlGroup + lane, nbad);
     }
     if (rd.abs_col < 0) return;                               // block-uniform
-    __syncthreads();
     for (int fl = w; fl < kIlGroup; fl += 8) {
         const int f = g * kIlGroup + fl, r = r0 + lane;
         if (f < a.n_frames && r < Z) {
