@@ -26,6 +26,7 @@ extern "C" {
 
 #define QCLDPC_MSG_MAX 30.0f /* clamp on |m_cv| (reading S2); part of the definition of the result */
 #define QCLDPC_MAX_FRAMES 65535 /* frames per decode call (one grid dimension of the kernels); more: split the batch */
+#define QCLDPC_STATIC_WORKSPACE_BYTES (16u << 20) /* the library's own workspace of qcldpc_decode_static: 16 MiB per GPU */
 
 enum {
     QCLDPC_OK = 0,
@@ -197,6 +198,31 @@ int64_t qcldpc_last_launch_count(void);
 int qcldpc_iterations_issued(const qcldpc_code_t* code, int n_frames, const void* d_workspace, void* stream,
                              int* h_iterations);
 int qcldpc_last_loop_mode(void);
+
+/*
+ * qcldpc_decode_static: qcldpc_decode_ex for callers that cannot allocate device memory (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc).  Same operation (Algorithm 1, syndrome form), same
+ * arguments, layouts and outputs as qcldpc_decode_ex, but NO workspace argument: the decoder's scratch memory (four
+ * buffers of edge state, the static check terms, the decisions, the per-frame flags) lives in a device array of
+ * QCLDPC_STATIC_WORKSPACE_BYTES = 16 MiB that is part of the library image: every GPU that loads the library holds it
+ * until the process exits.  The call itself calls no cudaMalloc / cudaFree and no allocating library routine: it only
+ * enqueues plain kernel launches on `stream`, one pass per iteration for all max_iter iterations (no device-side graph
+ * loop -- building a graph allocates --, no host polling, never waits); on a stream the caller is capturing the
+ * launches become nodes of the caller's graph.  The code handle (whose tables qcldpc_code_create allocates) must exist.
+ *   Limit: qcldpc_workspace_bytes(code, n_frames) <= qcldpc_static_workspace_bytes(), else QCLDPC_ERR_WORKSPACE with
+ *   the two sizes in qcldpc_last_cuda_error() (BASELINE.json's config 1 fits with up to about 90 frames; the n = 10^6
+ *   codes do not: they take qcldpc_decode with a workspace of the caller's).  QCLDPC_ERR_BAD_ARGUMENT while
+ *   qcldpc_profile_enable is on (the profile allocates events), other errors as qcldpc_decode_ex.
+ *   Sharing: every call on a GPU uses the SAME array, which keeps the previous call's contents; each call first clears
+ *   and rewrites all of it that it reads.  Two calls that overlap on the GPU (different streams, or replays of two
+ *   captured graphs at once) race on it: serialise them on one stream or with events.  One array per GPU: calls on
+ *   different GPUs are independent.
+ * qcldpc_static_workspace_bytes: the size of that array.
+ */
+int qcldpc_decode_static(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                         int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                         uint8_t* d_pass, float* d_posterior, void* stream);
+size_t qcldpc_static_workspace_bytes(void);
 
 const char* qcldpc_status_string(int status);
 const char* qcldpc_last_cuda_error(void); /* thread-local text of the last CUDA failure ("" if none) */

@@ -21,6 +21,7 @@ EXPORTED_SYMBOLS = (
     "qcldpc_host_workspace_bytes", "qcldpc_decode_host", "qcldpc_decode_host_ex", "qcldpc_last_launch_count", "qcldpc_status_string",
     "qcldpc_last_cuda_error", "qcldpc_profile_enable", "qcldpc_profile_collect",
     "qcldpc_llr_init", "qcldpc_pack_bits", "qcldpc_crc32_check", "qcldpc_iterations_issued", "qcldpc_last_loop_mode",
+    "qcldpc_decode_static", "qcldpc_static_workspace_bytes",
 )
 
 if not os.path.exists(SO_PATH):
@@ -68,6 +69,10 @@ _lib.qcldpc_iterations_issued.restype = _i
 _lib.qcldpc_iterations_issued.argtypes = [_vp, _i, _vp, _vp, ctypes.POINTER(_i)]
 _lib.qcldpc_last_loop_mode.restype = _i
 _lib.qcldpc_last_loop_mode.argtypes = []
+_lib.qcldpc_decode_static.restype = _i
+_lib.qcldpc_decode_static.argtypes = [_vp, _vp, _vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]
+_lib.qcldpc_static_workspace_bytes.restype = _sz
+_lib.qcldpc_static_workspace_bytes.argtypes = []
 _lib.qcldpc_status_string.restype = ctypes.c_char_p
 _lib.qcldpc_status_string.argtypes = [_i]
 _lib.qcldpc_last_cuda_error.restype = ctypes.c_char_p
@@ -75,11 +80,12 @@ _lib.qcldpc_last_cuda_error.argtypes = []
 
 
 class QCLDPCError(RuntimeError):
-    def __init__(self, status: int, where: str):
+    def __init__(self, status: int, where: str, with_detail: bool = False):
         self.status = status
         text = _lib.qcldpc_status_string(status).decode()
         detail = _lib.qcldpc_last_cuda_error().decode()
-        super().__init__(f"{where}: {text} ({status})" + (f": {detail}" if detail and status == -4 else ""))
+        super().__init__(f"{where}: {text} ({status})" +
+                         (f": {detail}" if detail and (status == -4 or with_detail) else ""))
 
 
 def _check(status: int, where: str) -> None:
@@ -98,6 +104,11 @@ def qcldpc_last_launch_count() -> int:
 def qcldpc_last_loop_mode() -> int:
     """1: the last decode of this thread ran as one graph with the loop on the device; 0: one launch per iteration."""
     return int(_lib.qcldpc_last_loop_mode())
+
+
+def qcldpc_static_workspace_bytes() -> int:
+    """Bytes of the library's own device workspace (per GPU), the limit of QCLDPCCode.decode_static."""
+    return int(_lib.qcldpc_static_workspace_bytes())
 
 
 def qcldpc_profile_enable(stride: int) -> None:
@@ -273,6 +284,35 @@ class QCLDPCCode:
                                        out.posterior.data_ptr() if out.posterior is not None else None,
                                        workspace.data_ptr(), workspace.numel(), st.cuda_stream)
         _check(rc, "qcldpc_decode_ex")
+        return out
+
+    def decode_static(self, llr, syndrome, max_iter: int, early_stop: int, out: DecodeResult, stream=None,
+                      check_from_iter: int = 1) -> DecodeResult:
+        """qcldpc_decode_static: the decode without any allocation, here or in the library.  The caller passes the
+        inputs AND the outputs (`out`, torch CUDA tensors, contiguous; out.posterior may be None); the workspace is the
+        library's own device array (qcldpc_static_workspace_bytes() per GPU, shared by every call on that GPU: calls
+        that overlap on the GPU race on it).  Raises QCLDPCError (QCLDPC_ERR_WORKSPACE) if this code and batch need more
+        than that.  Only enqueues plain launches on `stream` (default: torch's current stream)."""
+        import torch
+        _cuda_tensor(llr, "llr", torch.float32, torch)
+        _cuda_tensor(syndrome, "syndrome", torch.uint8, torch)
+        if llr.dim() != 2 or llr.shape[1] != self.n or tuple(syndrome.shape) != (llr.shape[0], self.m):
+            raise ValueError(f"shapes {tuple(llr.shape)} / {tuple(syndrome.shape)} do not match n={self.n}, m={self.m}")
+        F = llr.shape[0]
+        dev = llr.device
+        self._require_device(dev)
+        if syndrome.device != dev:
+            raise ValueError("llr and syndrome must live on one device")
+        _check_outputs(out, F, self.n, torch, cuda=True)
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        with torch.cuda.device(dev):
+            rc = _lib.qcldpc_decode_static(self._handle, llr.data_ptr(), syndrome.data_ptr(), F, int(max_iter),
+                                           int(early_stop), int(check_from_iter), out.hard.data_ptr(),
+                                           out.iters.data_ptr(), out.passed.data_ptr(),
+                                           out.posterior.data_ptr() if out.posterior is not None else None,
+                                           st.cuda_stream)
+        if rc != 0:
+            raise QCLDPCError(rc, "qcldpc_decode_static", with_detail=True)   # (the sizes, for QCLDPC_ERR_WORKSPACE)
         return out
 
     def decode_host(self, llr: np.ndarray, syndrome: np.ndarray, max_iter: int, early_stop: int,

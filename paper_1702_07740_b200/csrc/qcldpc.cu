@@ -903,7 +903,7 @@ bool same_key(const GraphKey& a, const GraphKey& b) {
 static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                        int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
                        uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream,
-                       bool host_poll);
+                       bool host_poll, bool allow_graph = true);
 
 int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                      int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
@@ -915,7 +915,7 @@ int qcldpc_decode_ex(const qcldpc_code_t* code, const float* d_llr, const uint8_
 static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
                        int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
                        uint8_t* d_pass, float* d_posterior, void* d_workspace, size_t workspace_bytes, void* stream,
-                       bool host_poll) {
+                       bool host_poll, bool allow_graph) {
     constexpr int kPollEvery = 32;
     g_launches = 0;
     if (check_from_iter < 1) return QCLDPC_ERR_BAD_ARGUMENT;
@@ -997,7 +997,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
     // (a caller that is itself capturing `stream` into a graph gets the plain launches: they become nodes of ITS graph)
     cudaStreamCaptureStatus caller_capture = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &caller_capture) != cudaSuccess) { cudaGetLastError(); caller_capture = cudaStreamCaptureStatusNone; }
-    if (code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2 &&
+    if (allow_graph && code->tune.loop_graph && g_prof.stride == 0 && max_iter >= body + 2 &&
         caller_capture == cudaStreamCaptureStatusNone) {
         int dev = 0;
         CUDA_TRY(cudaGetDevice(&dev));
@@ -1069,6 +1069,66 @@ int qcldpc_iterations_issued(const qcldpc_code_t* code, int n_frames, const void
 }
 
 int qcldpc_last_loop_mode(void) { return g_loop_mode; }
+
+// ---- decode without any allocation: the workspace is a file-scope device array ------------------------------------
+// (every GPU that loads the library holds QCLDPC_STATIC_WORKSPACE_BYTES of it until the process exits)
+static __device__ __align__(256) unsigned char g_static_workspace[QCLDPC_STATIC_WORKSPACE_BYTES];
+
+namespace {
+// In host code `g_static_workspace` is a host-side stand-in, not a device address: the address a kernel may use comes
+// from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kMaxStaticDevices = 64;
+void* g_static_ws_ptr[kMaxStaticDevices] = {};
+std::mutex g_static_ws_mu;
+
+int static_workspace_ptr(void** out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxStaticDevices) {
+        snprintf(g_cuda_error, sizeof(g_cuda_error), "qcldpc_decode_static: device ordinal %d beyond %d", dev,
+                 kMaxStaticDevices - 1);
+        return QCLDPC_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_static_ws_mu);
+    if (!g_static_ws_ptr[dev]) {
+        void* ptr = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_workspace));
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255)) {
+            snprintf(g_cuda_error, sizeof(g_cuda_error), "qcldpc_decode_static: bad address of the static workspace");
+            return QCLDPC_ERR_CUDA;
+        }
+        g_static_ws_ptr[dev] = ptr;
+    }
+    *out = g_static_ws_ptr[dev];
+    return QCLDPC_OK;
+}
+}  // namespace
+
+size_t qcldpc_static_workspace_bytes(void) { return (size_t)QCLDPC_STATIC_WORKSPACE_BYTES; }
+
+int qcldpc_decode_static(const qcldpc_code_t* code, const float* d_llr, const uint8_t* d_syndrome, int n_frames,
+                         int max_iter, int early_stop, int check_from_iter, uint8_t* d_hard, int32_t* d_iters,
+                         uint8_t* d_pass, float* d_posterior, void* stream) {
+    if (!code || n_frames <= 0 || n_frames > QCLDPC_MAX_FRAMES) return QCLDPC_ERR_BAD_ARGUMENT;
+    const size_t need = qcldpc_workspace_bytes(code, n_frames);
+    if (need == 0 || need > (size_t)QCLDPC_STATIC_WORKSPACE_BYTES) {
+        snprintf(g_cuda_error, sizeof(g_cuda_error),
+                 "qcldpc_decode_static: this code and batch need %zu bytes of workspace, the static workspace holds %zu: "
+                 "use qcldpc_decode with a workspace of the caller's", need, (size_t)QCLDPC_STATIC_WORKSPACE_BYTES);
+        return QCLDPC_ERR_WORKSPACE;
+    }
+    if (g_prof.stride != 0) {                                 // the profile's event pool grows by cudaEventCreate
+        snprintf(g_cuda_error, sizeof(g_cuda_error), "qcldpc_decode_static: not while qcldpc_profile_enable is on");
+        return QCLDPC_ERR_BAD_ARGUMENT;
+    }
+    void* ws = nullptr;
+    const int rc = static_workspace_ptr(&ws);
+    if (rc != QCLDPC_OK) return rc;
+    // plain launches, one pass per iteration, no graph (building one allocates), no host polling; the prologue
+    // (k_reset and the init kernels) clears and rewrites everything of the workspace that a decode reads
+    return decode_impl(code, d_llr, d_syndrome, n_frames, max_iter, early_stop, check_from_iter, d_hard, d_iters, d_pass,
+                       d_posterior, ws, (size_t)QCLDPC_STATIC_WORKSPACE_BYTES, stream, false, false);
+}
 
 size_t qcldpc_host_workspace_bytes(const qcldpc_code_t* code, int n_frames, int want_posterior) {
     if (!code || n_frames <= 0) return 0;
