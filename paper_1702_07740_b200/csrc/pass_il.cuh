@@ -44,6 +44,7 @@ struct IlArgs {
     const unsigned* hard_in; unsigned* hard_out;   // hardm[(t - 1) % 3] -> hardm[t % 3]
     int Z, Zp, W, n_frames, n_groups, n_cols, mb, cand_x, split, max_dv, max_np;   // Zp = Z + 1: lines per run
     int spc, ipc;              // k_pass_il: slots (pairs of variables) per column, slots per CTA (<= spc, <= W / 2)
+    int as_depth;              // k_pass_il: chunks of two edges a warp keeps in flight by asynchronous copies (0: register loads)
     const uint4* blob; int blob16;   // per-column tables in shared-memory layout, blob16 16-byte words per column
     int64_t n, m, EZ, mZ, AZ;  // E*Zp, mb*Zp, A*Z (per group, in lines of 32)
 };
@@ -66,10 +67,16 @@ __host__ __device__ inline size_t il_table_bytes(int max_dv, int max_np) {
 __host__ __device__ inline size_t il_tables_bytes(int max_dv, int max_np) {           // a CTA's slots lie in at most two columns
     return (2 * il_table_bytes(max_dv, max_np) + 127) / 128 * 128;
 }
-inline size_t il_smem_bytes(int max_dv, int max_np, int W) {
+constexpr int kIlAsEdges = 4;                                 // edges per chunk of the asynchronous pipeline
+constexpr int kIlAsEdgeBytes = 768;                           // ring bytes per edge: the pairs of t, partner and second-partner lines
+// tensor-memory columns a CTA of the asynchronous variant holds: 64 per warp of a lane quarter (512 per multiprocessor)
+__host__ __device__ constexpr int il_tmem_cols(int max_threads) { return max_threads <= 256 ? 128 : 256; }
+inline size_t il_smem_bytes(int max_dv, int max_np, int W, int as_depth = 0, int warps = 0) {
     return il_tables_bytes(max_dv, max_np) +
-           (size_t)W * ((max_dv > 0 ? max_dv : 1) + 4) * kIlGroup * sizeof(float) +   // messages + 4 partial sums per variable
-           128;                                                                        // handshake flags of the warp pairs
+           (size_t)W * ((as_depth ? 0 : (max_dv > 0 ? max_dv : 1)) + 4) * kIlGroup * sizeof(float) +   // messages (as_depth: in
+                                                                        // tensor memory instead) + 4 partial sums per variable
+           128 +                                                                       // handshake flags of the warp pairs
+           (size_t)warps * as_depth * kIlAsEdges * kIlAsEdgeBytes;                     // rings of the asynchronous pipeline
 }
 
 
@@ -85,6 +92,28 @@ __device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0
 // base + a signed byte offset
 __device__ __forceinline__ const float* il_at(const float* base, int byte_off) {
     return reinterpret_cast<const float*>(reinterpret_cast<const char*>(base) + byte_off);
+}
+// asynchronous 16-byte copy global -> shared; groups of copies; wait until at most N groups of this thread are pending
+__device__ __forceinline__ void il_cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void il_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void il_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// tensor memory as per-thread scratch: a warp reaches lanes 32 (warp % 4) .. + 31 of it, thread = lane, 32-bit columns
+__device__ __forceinline__ void il_tmem_st8(unsigned taddr, const float (&r)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+                 "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]), "f"(r[4]), "f"(r[5]), "f"(r[6]), "f"(r[7]) : "memory");
+}
+__device__ __forceinline__ void il_tmem_st2(unsigned taddr, float r0, float r1) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "f"(r0), "f"(r1) : "memory");
+}
+__device__ __forceinline__ void il_tmem_ld16(unsigned taddr, float (&r)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]), "=f"(r[8]),
+                   "=f"(r[9]), "=f"(r[10]), "=f"(r[11]), "=f"(r[12]), "=f"(r[13]), "=f"(r[14]), "=f"(r[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void il_stg(float* p, unsigned bits) { asm volatile("st.global.b32 [%0], %1;" ::"l"(p), "r"(bits) : "memory"); }
 // line index -> pointer to this lane's float
@@ -276,8 +305,13 @@ constexpr int kIlV = 2;
 
 // MAXT: threads per CTA the instance is compiled for; 320 (up to five slots with H = 2) leaves 102 registers
 // per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time
-template <bool FINAL, int H, int GPW, int MAXT>
-__global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
+// AS > 0 (H = 2 only): the pair, triple-row and static-term loads do not go through registers: a warp keeps AS chunks of
+// two edges in flight as asynchronous 16-byte copies (lanes 0-15: the edge's pair of t lines into a ring, lanes 16-31: its
+// pair of partner lines straight into the edge's message slot; one more copy per chunk for the second partners of
+// triple-row edges) and consumes them in order, so it never waits for a whole chunk's round trip.  Messages are then
+// stored edge-major (m'[k][v][32]) so that an edge's two lines are contiguous.
+template <bool FINAL, int H, int GPW, int MAXT, int AS>
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                     const CheckArgs chk) {
     constexpr int G = H * GPW;
     constexpr int V = kIlV;
@@ -306,8 +340,17 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
         for (int k = threadIdx.x; k < n16; k += blockDim.x) dst[k] = __ldg(src + k);
     }
     float* const msg_base = reinterpret_cast<float*>(smem_il + il_tables_bytes(mdv, a.max_np));
-    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdv + 4) * kIlGroup);
-    if (threadIdx.x < 32) s_flag[threadIdx.x] = 0;
+    const int mdm = AS ? 0 : mdv;                             // message lines per variable in shared memory
+    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdm + 4) * kIlGroup);
+    if (threadIdx.x < 31) s_flag[threadIdx.x] = 0;
+    if constexpr (AS > 0) {                                   // the messages of this CTA live in tensor memory: warp 0 allocates
+        if (warp == 0) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                             (unsigned)__cvta_generic_to_shared(s_flag + 31)), "n"(il_tmem_cols(MAXT)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
     const int f = g * kIlGroup + lane;
     const bool in_range = f < a.n_frames;
     const int fc = in_range ? f : a.n_frames - 1;
@@ -315,8 +358,24 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
     const int flag = FINAL ? a.iters[fc] : a.done[fc];
     __syncthreads();
     const bool live = in_range && (FINAL ? flag > 0 : !flag);
-    if (!has) return;                                         // (both warps of a slot leave together)
-    if (!FINAL && !__any_sync(0xffffffffu, live)) return;     // every frame of the group has stopped
+    unsigned tmem0 = 0;
+    auto tmem_release = [&]() {                               // every warp of the CTA comes here once, at its end
+        if constexpr (AS > 0) {
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
+            if (warp == 0)
+                asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem0), "n"(il_tmem_cols(MAXT)) : "memory");
+        }
+    };
+    if constexpr (AS > 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tmem0 = *reinterpret_cast<volatile unsigned*>(s_flag + 31);
+    }
+    // a slot beyond the last one, or one whose frames have all stopped, has nothing to do (both its warps leave together)
+    if (!has || (!FINAL && !__any_sync(0xffffffffu, live))) {
+        tmem_release();
+        return;
+    }
     const unsigned char* const tbl = smem_il + (size_t)(ca - ca0) * il_table_bytes(mdv, a.max_np);
     const IlColHdr cd = *reinterpret_cast<const IlColHdr*>(tbl);
     const int dv = cd.dv, ng = cd.ng, ngh = cd.ngh;
@@ -328,9 +387,18 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
     // (the lane is folded into the base pointers: a load address is base + 128 * line)
     const float* __restrict__ qP = (FINAL ? il_pick(a.qb, ((flag > 0 ? flag : 1) + 3) % 4) : a.q_in) + (int64_t)g * a.EZ * kIlGroup + lane;
     const float* __restrict__ tP = a.t + (int64_t)g * a.mZ * kIlGroup + lane;
-    float* const mm = msg_base + (size_t)slot * V * mdv * kIlGroup + lane;            // m'[v][k][lane] of this slot
+    float* const mm = msg_base + (size_t)slot * V * mdm * kIlGroup + lane;            // m'[v][k][lane] of this slot (AS: none)
+    constexpr int kstride = kIlGroup;
     const int vstride = mdv * kIlGroup;
-    float* const xch = msg_base + (size_t)a.W * mdv * kIlGroup + (size_t)slot * 4 * V * kIlGroup + lane;
+    float* const xch = msg_base + (size_t)a.W * mdm * kIlGroup + (size_t)slot * 4 * V * kIlGroup + lane;
+    // AS: message (block bi of this warp, edge j of the block, variable v) is column (bi * 8 + j) * 2 + v of this warp's
+    // 64 columns of tensor memory
+    const unsigned tm_warp = tmem0 + ((unsigned)(warp & 3) << 21) + (unsigned)(warp >> 2) * (8 * kIlChunk);
+    auto tm_col = [&](int k) {                                // column of edge k's message (an edge of this warp)
+        const int b = k / kIlChunk, rnd = b / G, pos = b - rnd * G;
+        const int gi = ((rnd & 1) ? G - 1 - pos : pos) - h * GPW;
+        return (unsigned)(((rnd * GPW + gi) * kIlChunk + (k - b * kIlChunk)) * V);
+    };
     const int Zb = Z << 7;                                    // bytes of the Z lines of a run
     const unsigned step = (unsigned)a.Zp << 7;                // bytes from a run to the next
     const bool single = dv == 1;                              // a single edge sends Q itself
@@ -397,9 +465,11 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
             }
             boxplus_acc(fabsf(tv[v]), num[v], den[v]);
             const float mk = with_sign(mag_of(num[v], den[v]), (xa[v] ^ __float_as_uint(tv[v])) & 0x80000000u);
-            mm[v * vstride + k * kIlGroup] = mk;
+            if constexpr (AS > 0) num[v] = mk;
+            else mm[v * vstride + k * kstride] = mk;
             acc[v] += mk;
         }
+        if constexpr (AS > 0) il_tmem_st2(tm_warp + tm_col(k), num[0], num[1]);
     };
     // edges of triple rows: two partners and an absorbed variable, one fraction, no reciprocal in between
     auto triple = [&](auto CHc, int k0, float (&acc)[V]) {
@@ -427,7 +497,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
                 float num = qa + qb, den = fmaf(qa, qb, 1.0f);
                 boxplus_acc(fabsf(tv[j][v]), num, den);
                 const float mk = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv[j][v])) & 0x80000000u);
-                mm[v * vstride + (k0 + j) * kIlGroup] = mk;
+                mm[v * vstride + (k0 + j) * kstride] = mk;
                 acc[v] += mk;
             }
     };
@@ -451,7 +521,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
 #pragma unroll
             for (int v = 0; v < V; ++v) {
                 const float mk = cn_rule(wv[j][v], tv[j][v]);
-                mm[v * vstride + (k0 + j) * kIlGroup] = mk;
+                mm[v * vstride + (k0 + j) * kstride] = mk;
                 acc[v] += mk;
             }
     };
@@ -469,6 +539,138 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
     for (int gi = 0; gi < GPW; ++gi)
 #pragma unroll
         for (int v = 0; v < V; ++v) part[gi][v] = 0.0f;
+    if constexpr (AS > 0) {
+        // ---- asynchronous pipeline.  Chunk c of this warp = edges k0 .. k0 + 3 of its block c / 2 (blocks in the order
+        // (rnd, gi) as below), k0 = block start + 4 (c % 2); edges outside [ngh, dv) are skipped: gen edges of other gen
+        // rows (k < ngh) keep their register loads (gen_edge), in order, while the copies of later chunks are in flight.
+        static_assert(H == 2 && GPW == 2 && !FINAL, "built for two warps per slot; FINAL reads a buffer per lane");
+        constexpr int CE = kIlAsEdges, kPer = kIlChunk / CE;  // edges per chunk, chunks per block
+        unsigned char* const ring = smem_il + il_tables_bytes(mdv, a.max_np) + (size_t)a.W * (mdm + 4) * kIlGroup * sizeof(float) +
+                                    128 + (size_t)warp * AS * CE * kIlAsEdgeBytes;   // this warp's: AS chunks x CE edges x (t | p | p2)
+        const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
+        const int half = lane >> 4;
+        const unsigned l16 = (unsigned)(lane & 15) * 16u;
+        const char* const qB = reinterpret_cast<const char*>(qT - lane) + l16;      // lane-free bases + this lane's 16 bytes
+        const char* const tB = reinterpret_cast<const char*>(tT - lane) + l16;
+        const char* const hB = half ? qB : tB;                // lanes 0-15 copy the t pair, lanes 16-31 the partner pair
+        const int n_chunks = ((dv + G * kIlChunk - 1) / (G * kIlChunk)) * GPW * kPer;
+        auto off_of = [&](const int pre, const int thr) { return pre - (i0b >= thr ? Zb : 0); };
+        auto cp16 = [&](unsigned dst_s, const char* src) {
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_s), "l"(src) : "memory");
+        };
+        auto issue = [&](int c) {
+            if (c < n_chunks) {
+                const int blk = c / kPer, rnd = blk / GPW, grp = h * GPW + (blk - rnd * GPW);
+                const int k0 = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk + (c - blk * kPer) * CE;
+                const unsigned e_s = ring_s + (unsigned)(c % AS) * (CE * kIlAsEdgeBytes) + l16;
+#pragma unroll
+                for (int j = 0; j < CE; ++j) {
+                    const int k = k0 + j;
+                    if (k >= ngh && k < dv) {
+                        const int4 d = *reinterpret_cast<const int4*>(s_a + k);     // {t.pre, t.thr, p.pre, p.thr}
+                        cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB + off_of(half ? d.z : d.x, half ? d.w : d.y));
+                    }
+                }
+                if (k0 < ng) {                                // second partners: lanes 0-15 edge 2u, lanes 16-31 edge 2u + 1
+#pragma unroll
+                    for (int u = 0; u < CE / 2; ++u) {
+                        const int k2 = k0 + 2 * u + half;
+                        if (k2 >= ngh && k2 < ng) {
+                            const IlRef r = s_b[k2].p2;
+                            cp16(e_s + (2 * u + half) * kIlAsEdgeBytes + 512, qB + off_of(r.pre, r.thr));
+                        }
+                    }
+                }
+            }
+            il_cp_async_commit();
+        };
+#pragma unroll 1
+        for (int c = 0; c < AS; ++c) issue(c);
+        // one rolled loop over the warp's chunks (the body is large; unrolled, the kernel outgrows the instruction caches)
+#pragma unroll 1
+        for (int c = 0; c < n_chunks; ++c) {
+            {
+                {
+                    const int blk = c / kPer, r2 = c - blk * kPer, rnd = blk / GPW, gi = blk - rnd * GPW;
+                    int kb, ke;
+                    block_of(rnd, gi, kb, ke);
+                    const int k0 = kb + r2 * CE;
+                    float acc[V];
+#pragma unroll
+                    for (int v = 0; v < V; ++v) acc[v] = gi ? part[1][v] : part[0][v];
+                    if (r2 == 0) {
+#pragma unroll 1
+                        for (int k = kb; k < min(ke, ngh); ++k) gen_edge(k, acc);
+                    }
+                    il_cp_async_wait<AS - 1>();               // this thread's copies of chunk c have landed ...
+                    __syncwarp();                             // ... and so have the other lanes'
+                    const float* const e = reinterpret_cast<const float*>(ring + (size_t)(c % AS) * CE * kIlAsEdgeBytes) + lane;
+                    constexpr int kE = kIlAsEdgeBytes / 4;    // floats per edge of a ring entry: t at 0, p at 64, p2 at 128
+                    float mk[CE * V];
+                    if (k0 >= ng && k0 + CE <= dv) {          // pair edges only
+#pragma unroll
+                        for (int j = 0; j < CE; ++j)
+#pragma unroll
+                            for (int v = 0; v < V; ++v) {
+                                mk[j * V + v] = cn_rule(e[j * kE + 64 + v * kIlGroup], e[j * kE + v * kIlGroup]);
+                                acc[v] += mk[j * V + v];
+                            }
+                        il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
+                    } else if (k0 >= ngh && k0 + CE <= ng) {  // edges of triple rows only
+#pragma unroll
+                        for (int j = 0; j < CE; ++j)
+#pragma unroll
+                            for (int v = 0; v < V; ++v) {
+                                const float tv = e[j * kE + v * kIlGroup];
+                                const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
+                                const unsigned ub = __float_as_uint(e[j * kE + 128 + v * kIlGroup]);
+                                const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
+                                float num = qa + qb, den = fmaf(qa, qb, 1.0f);
+                                boxplus_acc(fabsf(tv), num, den);
+                                mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
+                                acc[v] += mk[j * V + v];
+                            }
+                        il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
+                    } else if (k0 + CE > ngh && k0 < dv) {
+#pragma unroll
+                        for (int j = 0; j < CE; ++j) {
+                            const int k = k0 + j;
+                            const bool have = k >= ngh && k < dv;
+                            const bool tri = k < ng;
+                            const unsigned msk = tri ? 0x7ffffffeu : 0x7fffffffu;   // partners of a triple row carry a tag in bit 0
+#pragma unroll
+                            for (int v = 0; v < V; ++v) {
+                                mk[j * V + v] = 0.0f;
+                                if (have) {
+                                    const float tv = e[j * kE + v * kIlGroup];
+                                    const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
+                                    const unsigned ub = tri ? __float_as_uint(e[j * kE + 128 + v * kIlGroup]) : 0u;
+                                    const float qa = __uint_as_float(ua & msk), qb = __uint_as_float(ub & msk);
+                                    float num = qa + qb, den = fmaf(qa, qb, 1.0f);   // (+0.0 is the identity: a pair edge)
+                                    boxplus_acc(fabsf(tv), num, den);
+                                    mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
+                                    acc[v] += mk[j * V + v];
+                                }
+                            }
+                        }
+                        // (the chunk may hold gen edges, whose messages gen_edge has stored: write only the others)
+#pragma unroll
+                        for (int j = 0; j < CE; ++j)
+                            if (k0 + j >= ngh && k0 + j < dv)
+                                il_tmem_st2(tm_warp + (unsigned)((c * CE + j) * V), mk[j * V], mk[j * V + 1]);
+                    }
+                    __syncwarp();                             // every lane has read the ring entry: refill it
+                    issue(c + AS);
+#pragma unroll
+                    for (int v = 0; v < V; ++v) {
+                        if (gi) part[1][v] = acc[v];
+                        else part[0][v] = acc[v];
+                    }
+                }
+            }
+        }
+        il_cp_async_wait<0>();
+    } else {
 #pragma unroll 1
     for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
 #pragma unroll
@@ -493,6 +695,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
 #pragma unroll
             for (int v = 0; v < V; ++v) part[gi][v] = acc[v];
         }
+    }
     }
 
     // variable-node rule: the partial sums meet in the order 0 .. G-1
@@ -570,6 +773,7 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
 
     // every warp stores the new state of its own edges: w(L_vc), L_vc = L_v - m_cv = Q + sum_{k' != k} m_k'; nothing of a
     // stopped frame is stored.  The slot that holds a run's line 0 also writes the run's halo line (second round).
+    if constexpr (AS > 0) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     float* const sp0 = a.q_out + ((int64_t)g * a.EZ + (int64_t)cd.ebeg * a.Zp + i0) * kIlGroup + lane;
 #pragma unroll 1
     for (int round = 0; round < (i0 == 0 ? 2 : 1); ++round) {
@@ -582,13 +786,43 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
                 int k, ke;
                 block_of(rnd, gi, k, ke);
                 float* pk = byte_ptr(sp, (unsigned)k * step);          // edge k, the slot's first variable
-                const float* mk = mm + k * kIlGroup;
+                if constexpr (AS > 0) {                       // the block's 16 messages come from tensor memory at once
+                    if (k >= ke) continue;
+                    float m16[kIlChunk * V];
+                    il_tmem_ld16(tm_warp + (unsigned)((rnd * GPW + gi) * kIlChunk * V), m16);
+                    if (ke - k == kIlChunk && k >= ng) {      // a whole block without gen edges (no tag)
+#pragma unroll
+                        for (int j = 0; j < kIlChunk; ++j) {
+#pragma unroll
+                            for (int v = 0; v < V; ++v) {
+                                const float wv = w_of(L[v] - m16[j * V + v]);
+                                if (st[v]) il_stg(pk + v * kIlGroup, __float_as_uint(wv));
+                            }
+                            pk = byte_ptr(pk, step);
+                        }
+                        continue;
+                    }
+#pragma unroll
+                    for (int j = 0; j < kIlChunk; ++j) {
+                        if (k + j < ke) {
+                            const unsigned tagbit = (k + j < ng) ? 1u : 0u;   // gen edge: bit 0 carries the hard decision
+#pragma unroll
+                            for (int v = 0; v < V; ++v) {
+                                const unsigned wb = __float_as_uint(w_of(single ? Q[v] : L[v] - m16[j * V + v]));
+                                if (st[v]) il_stg(pk + v * kIlGroup, (wb & ~tagbit) | (xh[v] & tagbit));
+                            }
+                            pk = byte_ptr(pk, step);
+                        }
+                    }
+                    continue;
+                }
+                const float* mk = mm + k * kstride;
                 if (ke - k == kIlChunk && k >= ng) {          // a whole block without gen edges (no tag): unrolled
 #pragma unroll
                     for (int j = 0; j < kIlChunk; ++j) {
 #pragma unroll
                         for (int v = 0; v < V; ++v) {
-                            const float wv = w_of(L[v] - mk[v * vstride + j * kIlGroup]);
+                            const float wv = w_of(L[v] - mk[v * vstride + j * kstride]);
                             if (st[v]) il_stg(pk + v * kIlGroup, __float_as_uint(wv));
                         }
                         pk = byte_ptr(pk, step);
@@ -602,12 +836,13 @@ __global__ void __launch_bounds__(MAXT, 2) k_pass_il(const PassTables tab, const
                             if (st[v]) il_stg(pk + v * kIlGroup, (wb & ~tagbit) | (xh[v] & tagbit));
                         }
                         pk = byte_ptr(pk, step);
-                        mk += kIlGroup;
+                        mk += kstride;
                     }
                 }
             }
         }
     }
+    tmem_release();
 }
 
 // ---- a4: every check of every frame on the frame's frozen state (iteration d_iters[f]) -------------------------------
@@ -713,16 +948,17 @@ inline int il_pick_w(int Z, int max_dv, int max_np) {
 }
 
 #ifdef QC_IL_IMPL
-template <int H, int GPW, int MAXT>
+template <int H, int GPW, int MAXT, int AS>
 inline void launch_pass_il_h(const IlLaunch& L) {
     IlArgs args = L.args;
-    const size_t smem = il_smem_bytes(args.max_dv, args.max_np, args.W);
+    const int threads = 32 * H * (args.W / 2);
+    const size_t smem = il_smem_bytes(args.max_dv, args.max_np, args.W, AS, threads / 32);
     static thread_local int attr_dev = -1;                  // the attribute is per device
     int dev = 0;
     cudaGetDevice(&dev);
     if (attr_dev != dev) {
-        cudaFuncSetAttribute(k_pass_il<true, H, GPW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
-        cudaFuncSetAttribute(k_pass_il<false, H, GPW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<true, H, GPW, MAXT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
+        cudaFuncSetAttribute(k_pass_il<false, H, GPW, MAXT, AS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 208 * 1024);
         attr_dev = dev;
     }
     if (L.prepare_only) return;
@@ -732,21 +968,39 @@ inline void launch_pass_il_h(const IlLaunch& L) {
     args.cand_x = with_check ? work : -1;
     static const CheckTables no_tab{nullptr, nullptr};
     static const CheckArgs no_args{};
-    const dim3 grid(work + extra, args.n_groups), block(32 * H * (args.W / 2));
+    const dim3 grid(work + extra, args.n_groups), block(threads);
     if (L.final_mode)
-        k_pass_il<true, H, GPW, MAXT><<<grid, block, smem, L.stream>>>(L.tab, args, no_tab, no_args);
+        k_pass_il<true, H, GPW, MAXT, 0><<<grid, block, il_smem_bytes(args.max_dv, args.max_np, args.W), L.stream>>>(
+            L.tab, args, no_tab, no_args);                  // (FINAL reads a buffer per lane: register loads)
     else
-        launch_pdl(k_pass_il<false, H, GPW, MAXT>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
+        launch_pdl(k_pass_il<false, H, GPW, MAXT, AS>, grid, block, smem, L.stream, L.tab, args, with_check ? L.ctab : no_tab,
                    with_check ? *L.check : no_args);
 }
 
 // long columns (four partial sums): two warps per variable; short ones: one warp, one sum
 inline void launch_pass_il(const IlLaunch& L) {
     if (L.args.split == 4) {
-        if (32 * 2 * (L.args.W / 2) <= 320) launch_pass_il_h<2, 2, 320>(L);
-        else launch_pass_il_h<2, 2, 384>(L);
+        const bool narrow = 32 * 2 * (L.args.W / 2) <= 320;
+        if (L.args.as_depth > 0 && 32 * 2 * (L.args.W / 2) <= 256) {   // three CTAs per multiprocessor
+            switch (L.args.as_depth) {
+                case 1: launch_pass_il_h<2, 2, 256, 1>(L); break;
+                case 2: launch_pass_il_h<2, 2, 256, 2>(L); break;
+                case 3: launch_pass_il_h<2, 2, 256, 3>(L); break;
+                default: launch_pass_il_h<2, 2, 256, 4>(L); break;
+            }
+            return;
+        }
+        switch (narrow ? L.args.as_depth : 0) {
+            case 1: launch_pass_il_h<2, 2, 320, 1>(L); break;
+            case 2: launch_pass_il_h<2, 2, 320, 2>(L); break;
+            case 3: launch_pass_il_h<2, 2, 320, 3>(L); break;
+            case 4: launch_pass_il_h<2, 2, 320, 4>(L); break;
+            default:
+                if (narrow) launch_pass_il_h<2, 2, 320, 0>(L);
+                else launch_pass_il_h<2, 2, 384, 0>(L);
+        }
     } else {
-        launch_pass_il_h<1, 1, 384>(L);
+        launch_pass_il_h<1, 1, 384, 0>(L);
     }
 }
 #endif

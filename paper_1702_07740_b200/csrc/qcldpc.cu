@@ -121,6 +121,7 @@ struct qcldpc_code {
     std::vector<uint4> il_blob; uint4* d_il_blob = nullptr; int il_blob16 = 0;   // per-column tables of k_pass_il
     bool il_ok = false;                   // the code fits the family's 32-bit byte offsets
     int il_w = 8;                         // warps per CTA of k_pass_il
+    int il_as = 0;                        // chunks a warp of k_pass_il keeps in flight by asynchronous copies (0: none)
     PassLauncher launcher = nullptr;
     std::vector<char> exact;              // kernel-parameter table of the exact family (empty: generic kernel)
     int n_sm = 148;
@@ -565,12 +566,24 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
     code->il_ok = !exact && code->n_act_cols > 0 && (int64_t)code->n_act_edges * Zp < ((int64_t)1 << 24) &&
                   (int64_t)mb * Zp < ((int64_t)1 << 24) &&
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
+    // long columns (two warps per slot): the asynchronous variant -- messages in tensor memory, loads as asynchronous
+    // copies through a ring, QCLDPC_ILA chunks deep (default 2; 0: register loads) --, eight variables per CTA so that
+    // three CTAs share a multiprocessor; short columns: register loads
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
+    const bool long_cols = code->max_dv > 2 * kIlChunk;
+    int as = long_cols ? env_int("QCLDPC_ILA", 2) : 0;
+    if (as < 0 || as > 4) as = 0;
+    if (as) code->il_w = std::min(8, 2 * ((Z + 1) / 2));
     if (const int wf = env_int("QCLDPC_ILW", 0)) {         // tuning knob: variables per CTA of k_pass_il (even, <= 12)
-        if (wf >= 2 && wf <= (code->max_dv > 2 * kIlChunk ? 12 : 24) && wf % 2 == 0 &&
+        if (wf >= 2 && wf <= (long_cols ? 12 : 24) && wf % 2 == 0 &&
             il_smem_bytes(code->max_dv, max_np, wf) <= (size_t)200 * 1024)
             code->il_w = wf;
     }
+    // (the asynchronous variant: at most 10 warps per CTA -- 64 columns of tensor memory per warp, 256 per CTA)
+    if (as && code->il_w <= 10 && il_smem_bytes(code->max_dv, max_np, code->il_w, as, code->il_w) <= (size_t)200 * 1024)
+        code->il_as = as;
+    else if (as)
+        code->il_w = il_pick_w(Z, code->max_dv, max_np);
     if (code->il_ok) {                                     // one fixed-stride blob per column, in shared-memory layout
         const int mdv = std::max(code->max_dv, 1);
         const size_t stride = il_table_bytes(mdv, max_np);
@@ -982,6 +995,7 @@ static int decode_impl(const qcldpc_code_t* code, const float* d_llr, const uint
         ia.done = w.done; ia.iters = d_iters; ia.topbad = nullptr; ia.unsat = w.unsat;
         ia.Z = Z; ia.Zp = Z + 1; ia.W = code->il_w;
         ia.spc = (Z + 1) / 2; ia.ipc = std::min(code->il_w / 2, ia.spc);
+        ia.as_depth = code->il_as;
         ia.n_frames = n_frames; ia.n_groups = w.n_groups; ia.n_cols = code->n_act_cols; ia.mb = code->mb;
         ia.cand_x = -1; ia.split = code->max_dv > 16 ? 4 : 1; ia.max_dv = std::max(code->max_dv, 1);
         ia.max_np = code->max_np;
