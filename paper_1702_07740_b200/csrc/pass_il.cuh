@@ -563,10 +563,11 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
                 const int blk = c / kPer, rnd = blk / GPW, grp = h * GPW + (blk - rnd * GPW);
                 const int k0 = (rnd * G + ((rnd & 1) ? G - 1 - grp : grp)) * kIlChunk + (c - blk * kPer) * CE;
                 const unsigned e_s = ring_s + (unsigned)(c % AS) * (CE * kIlAsEdgeBytes) + l16;
+                const bool whole = k0 >= ngh && k0 + CE <= dv;
 #pragma unroll
                 for (int j = 0; j < CE; ++j) {
                     const int k = k0 + j;
-                    if (k >= ngh && k < dv) {
+                    if (whole || (k >= ngh && k < dv)) {
                         const int4 d = *reinterpret_cast<const int4*>(s_a + k);     // {t.pre, t.thr, p.pre, p.thr}
                         cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB + off_of(half ? d.z : d.x, half ? d.w : d.y));
                     }
@@ -790,13 +791,14 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
                     if (k >= ke) continue;
                     float m16[kIlChunk * V];
                     il_tmem_ld16(tm_warp + (unsigned)((rnd * GPW + gi) * kIlChunk * V), m16);
-                    if (ke - k == kIlChunk && k >= ng) {      // a whole block without gen edges (no tag)
+                    if (ke - k == kIlChunk && (k >= ng || k + kIlChunk <= ng)) {   // a whole block, all of its edges with or
+                        const unsigned keep = k >= ng ? 0xffffffffu : 0xfffffffeu;   // all without the tag in bit 0
 #pragma unroll
                         for (int j = 0; j < kIlChunk; ++j) {
 #pragma unroll
                             for (int v = 0; v < V; ++v) {
-                                const float wv = w_of(L[v] - m16[j * V + v]);
-                                if (st[v]) il_stg(pk + v * kIlGroup, __float_as_uint(wv));
+                                const unsigned wb = __float_as_uint(w_of(L[v] - m16[j * V + v]));
+                                if (st[v]) il_stg(pk + v * kIlGroup, (wb & keep) | (xh[v] & ~keep));
                             }
                             pk = byte_ptr(pk, step);
                         }
