@@ -60,7 +60,10 @@ typedef struct qcldpc_code qcldpc_code_t;
  * of the exact pass; QCLDPC_FLIP=0 every launch walks the frames forwards; QCLDPC_MERGE_CHECK=0 early-exit check as a
  * separate launch; QCLDPC_CAND_PER_SM=k grid of that launch; QCLDPC_PACK=0 no lane packing and QCLDPC_FV=1|2 frames
  * per thread in the generic pass; QCLDPC_LOOP=stream and QCLDPC_BODY=k (body of 12 k iterations) for the iteration
- * loop (see qcldpc_iterations_issued).  None of them changes any result.
+ * loop (see qcldpc_iterations_issued); QCLDPC_IL=0|2 never / always the frame-interleaved kernel family, QCLDPC_ILW=k
+ * its variables per CTA, QCLDPC_ILA=0..4 the depth of its asynchronous pipeline in chunks of four edges (0: loads
+ * through registers and messages in shared memory; default 2: messages in tensor memory, for columns of more than 16
+ * edges).  None of them changes any result.
  */
 int qcldpc_code_create(const int32_t* base_shifts, int mb, int nb, int Z, qcldpc_code_t** out_code);
 void qcldpc_code_destroy(qcldpc_code_t* code);

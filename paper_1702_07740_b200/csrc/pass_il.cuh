@@ -16,6 +16,11 @@
 // are summed -- is that of the generic pass (pass_kernel.cuh), so a frame's result does not depend on which of the
 // two kernel families decodes it (bit for bit; tests).
 //
+// Long columns (more than 16 edges: two warps per slot) run the ASYNCHRONOUS variant of the pass by default: the
+// messages of a tile wait in TENSOR MEMORY (tcgen05.st / tcgen05.ld; the pass has no tensor-core work, the 256 KB are
+// free) instead of shared memory, and the shared memory so freed is a ring through which every load of a pair, triple-row
+// or static term travels as a 16-byte cp.async, issued chunks ahead and consumed in order (k_pass_il's AS parameter).
+//
 // Kernels: k_il_init_cols / k_il_init_rows (a0; transposes of the frame-major inputs through shared memory),
 // k_pass_il (a1 + a2 + the filter of a3), cand_work_il inside its grid or as k_cand_il (a3), k_pass_il<FINAL> and
 // k_il_check_final (a4; transposes back to the frame-major outputs).
@@ -295,7 +300,8 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 // ipc = min(S, spc): no slot of a CTA idles because Z is not a multiple of the CTA's width (q = 21: 11 slots per column,
 // 5 per CTA), and the slots of a CTA lie in at most two columns, whose tables it loads; grid = (ceil(columns * spc / ipc)
 // [+ check workers], groups).
-// Shared memory: the tables of two columns, the messages m'[2 S][max_dv][32], the partial sums, the handshake counters.
+// Shared memory: the tables of two columns, the messages m'[2 S][max_dv][32] (AS = 0), the partial sums, the handshake
+// counters, the rings (AS > 0).
 // The messages of a column are added as the generic pass adds them: block b = k / 8 of the column's edges belongs to
 // partial sum ((b / G) odd ? G - 1 - b % G : b % G), G = 4 for long columns (max_dv > 16), else 1; inside a partial sum k
 // increases; the partial sums meet in the order 0 .. G-1.  H = 2 (G = 4): warp h of a slot owns the partial sums 2h and
@@ -304,12 +310,16 @@ __global__ void __launch_bounds__(256) k_cand_il(const CheckTables tab, const Ch
 constexpr int kIlV = 2;
 
 // MAXT: threads per CTA the instance is compiled for; 320 (up to five slots with H = 2) leaves 102 registers
-// per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time
-// AS > 0 (H = 2 only): the pair, triple-row and static-term loads do not go through registers: a warp keeps AS chunks of
-// two edges in flight as asynchronous 16-byte copies (lanes 0-15: the edge's pair of t lines into a ring, lanes 16-31: its
-// pair of partner lines straight into the edge's message slot; one more copy per chunk for the second partners of
-// triple-row edges) and consumes them in order, so it never waits for a whole chunk's round trip.  Messages are then
-// stored edge-major (m'[k][v][32]) so that an edge's two lines are contiguous.
+// per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time; 256 (AS > 0)
+// leaves 85 with three CTAs per multiprocessor.
+// AS > 0 (H = 2, not FINAL): the loads of the pair and triple-row edges and of their static terms do not go through
+// registers.  A warp keeps AS chunks of four edges in flight as asynchronous 16-byte copies into its ring (768 bytes per
+// edge: the pairs of t, partner and second-partner lines of the slot's two variables; lanes 0-15 copy an edge's t pair,
+// lanes 16-31 its partner pair, one more copy per two triple-row edges for the second partners) and consumes them in
+// order: it never waits for a whole chunk's round trip.  The messages go to tensor memory: thread = lane of the warp's
+// lane quarter, column (block * 8 + edge of the block) * 2 + variable of the warp's 64 columns; the store phase reads
+// them back a block (16 columns) at a time.  Gen edges of other gen rows keep gen_edge's register loads.  The chunk loop
+// is rolled: unrolled over the blocks, the kernel outgrew the instruction caches (0.211 against 0.193 ms per launch).
 template <bool FINAL, int H, int GPW, int MAXT, int AS>
 __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                     const CheckArgs chk) {
