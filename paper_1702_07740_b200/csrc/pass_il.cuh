@@ -98,10 +98,7 @@ __device__ __forceinline__ T il_pick(T const (&p)[3], int idx) { return idx == 0
 __device__ __forceinline__ const float* il_at(const float* base, int byte_off) {
     return reinterpret_cast<const float*>(reinterpret_cast<const char*>(base) + byte_off);
 }
-// asynchronous 16-byte copy global -> shared; groups of copies; wait until at most N groups of this thread are pending
-__device__ __forceinline__ void il_cp_async16(void* smem_dst, const void* gsrc) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
-}
+// groups of asynchronous copies; wait until at most N groups of this thread are pending
 __device__ __forceinline__ void il_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void il_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }

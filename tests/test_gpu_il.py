@@ -106,6 +106,29 @@ def test_il_frame_independence(B, monkeypatch):
                 np.testing.assert_array_equal(a[f], b[0])
 
 
+@pytest.mark.parametrize("q,F", [(50, 32), (21, 59), (7, 40)])
+def test_il_asynchronous_variant_equals_register_variant(B, monkeypatch, q, F):
+    """Long columns run the asynchronous variant by default (messages in tensor memory, loads as a cp.async ring);
+    QCLDPC_ILA=0 selects the variant with register loads and messages in shared memory, QCLDPC_ILA=1 / 3 other ring
+    depths.  Same outputs bit for bit, fixed count and early stop, ragged last group included."""
+    spec = W.paper_ensemble_spec(400, q)
+    ens = W.make_paper_ensemble(spec)
+    hi = W.make_frames_sparse(*ens, q, W.sigma_for_gap(0.02, 3.0), F // 2, 91)
+    lo = W.make_frames_sparse(*ens, q, W.sigma_for_gap(0.02, 0.3), F - F // 2, 92)
+    llr, syn = np.concatenate([hi.llr, lo.llr]), np.concatenate([hi.syndrome, lo.syndrome])
+    default = B.QCLDPCCode.from_sparse(*ens, q)
+    others = []
+    for depth in ("0", "1", "3"):
+        monkeypatch.setenv("QCLDPC_ILA", depth)
+        others.append(B.QCLDPCCode.from_sparse(*ens, q))
+    monkeypatch.delenv("QCLDPC_ILA")
+    for early, it in ((0, 12), (1, 40)):
+        ref = decode(default, llr, syn, it, early)
+        for other in others:
+            for a, b in zip(ref, decode(other, llr, syn, it, early)):
+                np.testing.assert_array_equal(a, b)
+
+
 def _random_code(rng, mb, nb, Z, density):
     base = np.full((mb, nb), -1, dtype=np.int32)
     mask = rng.random((mb, nb)) < density
