@@ -575,8 +575,8 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
                 for (int j = 0; j < CE; ++j) {
                     const int k = k0 + j;
                     if (whole || (k >= ngh && k < dv)) {
-                        const int4 d = *reinterpret_cast<const int4*>(s_a + k);     // {t.pre, t.thr, p.pre, p.thr}
-                        cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB + off_of(half ? d.z : d.x, half ? d.w : d.y));
+                        const IlRef r = reinterpret_cast<const IlRef*>(s_a + k)[half];   // lanes 0-15: t, lanes 16-31: p
+                        cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB + off_of(r.pre, r.thr));
                     }
                 }
                 if (k0 < ng) {                                // second partners: lanes 0-15 edge 2u, lanes 16-31 edge 2u + 1
