@@ -597,84 +597,80 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
         // one rolled loop over the warp's chunks (the body is large; unrolled, the kernel outgrows the instruction caches)
 #pragma unroll 1
         for (int c = 0; c < n_chunks; ++c) {
-            {
-                {
-                    const int blk = c / kPer, r2 = c - blk * kPer, rnd = blk / GPW, gi = blk - rnd * GPW;
-                    int kb, ke;
-                    block_of(rnd, gi, kb, ke);
-                    const int k0 = kb + r2 * CE;
-                    float acc[V];
+            const int blk = c / kPer, r2 = c - blk * kPer, rnd = blk / GPW, gi = blk - rnd * GPW;
+            int kb, ke;
+            block_of(rnd, gi, kb, ke);
+            const int k0 = kb + r2 * CE;
+            float acc[V];
 #pragma unroll
-                    for (int v = 0; v < V; ++v) acc[v] = gi ? part[1][v] : part[0][v];
-                    if (r2 == 0) {
+            for (int v = 0; v < V; ++v) acc[v] = gi ? part[1][v] : part[0][v];
+            if (r2 == 0) {
 #pragma unroll 1
-                        for (int k = kb; k < min(ke, ngh); ++k) gen_edge(k, acc);
-                    }
-                    il_cp_async_wait<AS - 1>();               // this thread's copies of chunk c have landed ...
-                    __syncwarp();                             // ... and so have the other lanes'
-                    const float* const e = reinterpret_cast<const float*>(ring + (size_t)(c % AS) * CE * kIlAsEdgeBytes) + lane;
-                    constexpr int kE = kIlAsEdgeBytes / 4;    // floats per edge of a ring entry: t at 0, p at 64, p2 at 128
-                    float mk[CE * V];
-                    if (k0 >= ng && k0 + CE <= dv) {          // pair edges only
+                for (int k = kb; k < min(ke, ngh); ++k) gen_edge(k, acc);
+            }
+            il_cp_async_wait<AS - 1>();               // this thread's copies of chunk c have landed ...
+            __syncwarp();                             // ... and so have the other lanes'
+            const float* const e = reinterpret_cast<const float*>(ring + (size_t)(c % AS) * CE * kIlAsEdgeBytes) + lane;
+            constexpr int kE = kIlAsEdgeBytes / 4;    // floats per edge of a ring entry: t at 0, p at 64, p2 at 128
+            float mk[CE * V];
+            if (k0 >= ng && k0 + CE <= dv) {          // pair edges only
 #pragma unroll
-                        for (int j = 0; j < CE; ++j)
-#pragma unroll
-                            for (int v = 0; v < V; ++v) {
-                                mk[j * V + v] = cn_rule(e[j * kE + 64 + v * kIlGroup], e[j * kE + v * kIlGroup]);
-                                acc[v] += mk[j * V + v];
-                            }
-                        il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
-                    } else if (k0 >= ngh && k0 + CE <= ng) {  // edges of triple rows only
-#pragma unroll
-                        for (int j = 0; j < CE; ++j)
-#pragma unroll
-                            for (int v = 0; v < V; ++v) {
-                                const float tv = e[j * kE + v * kIlGroup];
-                                const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
-                                const unsigned ub = __float_as_uint(e[j * kE + 128 + v * kIlGroup]);
-                                const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
-                                float num = qa + qb, den = fmaf(qa, qb, 1.0f);
-                                boxplus_acc(fabsf(tv), num, den);
-                                mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
-                                acc[v] += mk[j * V + v];
-                            }
-                        il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
-                    } else if (k0 + CE > ngh && k0 < dv) {
-#pragma unroll
-                        for (int j = 0; j < CE; ++j) {
-                            const int k = k0 + j;
-                            const bool have = k >= ngh && k < dv;
-                            const bool tri = k < ng;
-                            const unsigned msk = tri ? 0x7ffffffeu : 0x7fffffffu;   // partners of a triple row carry a tag in bit 0
-#pragma unroll
-                            for (int v = 0; v < V; ++v) {
-                                mk[j * V + v] = 0.0f;
-                                if (have) {
-                                    const float tv = e[j * kE + v * kIlGroup];
-                                    const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
-                                    const unsigned ub = tri ? __float_as_uint(e[j * kE + 128 + v * kIlGroup]) : 0u;
-                                    const float qa = __uint_as_float(ua & msk), qb = __uint_as_float(ub & msk);
-                                    float num = qa + qb, den = fmaf(qa, qb, 1.0f);   // (+0.0 is the identity: a pair edge)
-                                    boxplus_acc(fabsf(tv), num, den);
-                                    mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
-                                    acc[v] += mk[j * V + v];
-                                }
-                            }
-                        }
-                        // (the chunk may hold gen edges, whose messages gen_edge has stored: write only the others)
-#pragma unroll
-                        for (int j = 0; j < CE; ++j)
-                            if (k0 + j >= ngh && k0 + j < dv)
-                                il_tmem_st2(tm_warp + (unsigned)((c * CE + j) * V), mk[j * V], mk[j * V + 1]);
-                    }
-                    __syncwarp();                             // every lane has read the ring entry: refill it
-                    issue(c + AS);
+                for (int j = 0; j < CE; ++j)
 #pragma unroll
                     for (int v = 0; v < V; ++v) {
-                        if (gi) part[1][v] = acc[v];
-                        else part[0][v] = acc[v];
+                        mk[j * V + v] = cn_rule(e[j * kE + 64 + v * kIlGroup], e[j * kE + v * kIlGroup]);
+                        acc[v] += mk[j * V + v];
+                    }
+                il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
+            } else if (k0 >= ngh && k0 + CE <= ng) {  // edges of triple rows only
+#pragma unroll
+                for (int j = 0; j < CE; ++j)
+#pragma unroll
+                    for (int v = 0; v < V; ++v) {
+                        const float tv = e[j * kE + v * kIlGroup];
+                        const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
+                        const unsigned ub = __float_as_uint(e[j * kE + 128 + v * kIlGroup]);
+                        const float qa = __uint_as_float(ua & 0x7ffffffeu), qb = __uint_as_float(ub & 0x7ffffffeu);   // bit 0: tag
+                        float num = qa + qb, den = fmaf(qa, qb, 1.0f);
+                        boxplus_acc(fabsf(tv), num, den);
+                        mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
+                        acc[v] += mk[j * V + v];
+                    }
+                il_tmem_st8(tm_warp + (unsigned)(c * CE * V), mk);
+            } else if (k0 + CE > ngh && k0 < dv) {
+#pragma unroll
+                for (int j = 0; j < CE; ++j) {
+                    const int k = k0 + j;
+                    const bool have = k >= ngh && k < dv;
+                    const bool tri = k < ng;
+                    const unsigned msk = tri ? 0x7ffffffeu : 0x7fffffffu;   // partners of a triple row carry a tag in bit 0
+#pragma unroll
+                    for (int v = 0; v < V; ++v) {
+                        mk[j * V + v] = 0.0f;
+                        if (have) {
+                            const float tv = e[j * kE + v * kIlGroup];
+                            const unsigned ua = __float_as_uint(e[j * kE + 64 + v * kIlGroup]);
+                            const unsigned ub = tri ? __float_as_uint(e[j * kE + 128 + v * kIlGroup]) : 0u;
+                            const float qa = __uint_as_float(ua & msk), qb = __uint_as_float(ub & msk);
+                            float num = qa + qb, den = fmaf(qa, qb, 1.0f);   // (+0.0 is the identity: a pair edge)
+                            boxplus_acc(fabsf(tv), num, den);
+                            mk[j * V + v] = with_sign(mag_of(num, den), (ua ^ ub ^ __float_as_uint(tv)) & 0x80000000u);
+                            acc[v] += mk[j * V + v];
+                        }
                     }
                 }
+                // (the chunk may hold gen edges, whose messages gen_edge has stored: write only the others)
+#pragma unroll
+                for (int j = 0; j < CE; ++j)
+                    if (k0 + j >= ngh && k0 + j < dv)
+                        il_tmem_st2(tm_warp + (unsigned)((c * CE + j) * V), mk[j * V], mk[j * V + 1]);
+            }
+            __syncwarp();                             // every lane has read the ring entry: refill it
+            issue(c + AS);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                if (gi) part[1][v] = acc[v];
+                else part[0][v] = acc[v];
             }
         }
         il_cp_async_wait<0>();
