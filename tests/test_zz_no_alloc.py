@@ -73,6 +73,37 @@ def test_decode_static_matches_decode_on_calls_in_a_row(B, cfg_index, Z, n_frame
     assert (out_a.iters == 30).all()
 
 
+def test_decode_static_frame_interleaved_family(B):
+    """A batch of the paper's own ensemble (small: 400 base columns, q = 7, 32 frames) takes the frame-interleaved
+    kernels with their messages in tensor memory; its workspace fits the static array.  Two calls in a row, then one
+    captured into the caller's graph, against the existing path."""
+    spec = W.paper_ensemble_spec(400, 7)
+    ens = W.make_paper_ensemble(spec)
+    code = B.QCLDPCCode.from_sparse(*ens, 7)
+    F = 32
+    assert code.workspace_bytes(F) <= B.qcldpc_static_workspace_bytes()
+    fa = W.make_frames_sparse(*ens, 7, W.sigma_for_gap(0.02, 3.0), F, 4711)
+    fb = W.make_frames_sparse(*ens, 7, W.sigma_for_gap(0.02, 0.3), F, 4712)
+    llr_a, syn_a = torch.from_numpy(fa.llr).cuda(), torch.from_numpy(fa.syndrome).cuda()
+    llr_b, syn_b = torch.from_numpy(fb.llr).cuda(), torch.from_numpy(fb.syndrome).cuda()
+    out_a, out_b = _outputs(B, F, code.n), _outputs(B, F, code.n)
+    code.decode_static(llr_a, syn_a, 40, 1, out_a)
+    code.decode_static(llr_b, syn_b, 15, 0, out_b)
+    torch.cuda.synchronize()
+    ref_a = code.decode(llr_a, syn_a, 40, 1, want_posterior=True)
+    _same(out_a, ref_a)
+    _same(out_b, code.decode(llr_b, syn_b, 15, 0, want_posterior=True))
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        code.decode_static(llr_a, syn_a, 40, 1, out_a)
+    for t in out_a:
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    _same(out_a, ref_a)
+
+
 def test_decode_static_rejects_what_does_not_fit(B):
     cfg, base, Z, fr = W.make_config(1, n_frames=1)
     code = B.QCLDPCCode(base, Z)
