@@ -78,8 +78,8 @@ constexpr int kIlAsEdgeBytes = 768;                           // ring bytes per 
 __host__ __device__ constexpr int il_tmem_cols(int max_threads) { return max_threads <= 256 ? 128 : 256; }
 inline size_t il_smem_bytes(int max_dv, int max_np, int W, int as_depth = 0, int warps = 0) {
     return il_tables_bytes(max_dv, max_np) +
-           (size_t)W * ((as_depth ? 0 : (max_dv > 0 ? max_dv : 1)) + 4) * kIlGroup * sizeof(float) +   // messages (as_depth: in
-                                                                        // tensor memory instead) + 4 partial sums per variable
+           (size_t)W * (as_depth ? 0 : (max_dv > 0 ? max_dv : 1) + 4) * kIlGroup * sizeof(float) +   // messages + 4 partial sums
+                                                     // per variable (as_depth: in tensor memory and in the rings instead)
            128 +                                                                       // handshake flags of the warp pairs
            (size_t)warps * as_depth * kIlAsEdges * kIlAsEdgeBytes;                     // rings of the asynchronous pipeline
 }
@@ -318,7 +318,7 @@ constexpr int kIlV = 2;
 // them back a block (16 columns) at a time.  Gen edges of other gen rows keep gen_edge's register loads.  The chunk loop
 // is rolled: unrolled over the blocks, the kernel outgrew the instruction caches (0.211 against 0.193 ms per launch).
 template <bool FINAL, int H, int GPW, int MAXT, int AS>
-__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const PassTables tab, const IlArgs a, const CheckTables ctab,
                                                     const CheckArgs chk) {
     constexpr int G = H * GPW;
     constexpr int V = kIlV;
@@ -348,7 +348,8 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
     }
     float* const msg_base = reinterpret_cast<float*>(smem_il + il_tables_bytes(mdv, a.max_np));
     const int mdm = AS ? 0 : mdv;                             // message lines per variable in shared memory
-    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * (mdm + 4) * kIlGroup);
+    const int mdx = AS ? 0 : mdv + 4;                         // lines per variable: messages + partial sums
+    int* const s_flag = reinterpret_cast<int*>(msg_base + (size_t)a.W * mdx * kIlGroup);
     if (threadIdx.x < 31) s_flag[threadIdx.x] = 0;
     if constexpr (AS > 0) {                                   // the messages of this CTA live in tensor memory: warp 0 allocates
         if (warp == 0) {
@@ -397,7 +398,16 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
     float* const mm = msg_base + (size_t)slot * V * mdm * kIlGroup + lane;            // m'[v][k][lane] of this slot (AS: none)
     constexpr int kstride = kIlGroup;
     const int vstride = mdv * kIlGroup;
-    float* const xch = msg_base + (size_t)a.W * mdm * kIlGroup + (size_t)slot * 4 * V * kIlGroup + lane;
+    // partial sum gg of variable v of this slot, where the slot's warps exchange them: AS = 0 a region of its own, AS > 0
+    // the head of the owning warp's ring (idle by then)
+    constexpr size_t kRingWarp = (size_t)AS * kIlAsEdges * kIlAsEdgeBytes;
+    auto xch_at = [&](int gg, int v) -> float* {
+        if constexpr (AS > 0)
+            return reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(s_flag) + 128 + (size_t)(slot * H + gg / GPW) * kRingWarp) +
+                   ((gg % GPW) * V + v) * kIlGroup + lane;
+        else
+            return msg_base + (size_t)a.W * mdm * kIlGroup + (size_t)slot * 4 * V * kIlGroup + (gg * V + v) * kIlGroup + lane;
+    };
     // AS: message (block bi of this warp, edge j of the block, variable v) is column (bi * 8 + j) * 2 + v of this warp's
     // 64 columns of tensor memory
     const unsigned tm_warp = tmem0 + ((unsigned)(warp & 3) << 21) + (unsigned)(warp >> 2) * (8 * kIlChunk);
@@ -552,8 +562,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
         // rows (k < ngh) keep their register loads (gen_edge), in order, while the copies of later chunks are in flight.
         static_assert(H == 2 && GPW == 2 && !FINAL, "built for two warps per slot; FINAL reads a buffer per lane");
         constexpr int CE = kIlAsEdges, kPer = kIlChunk / CE;  // edges per chunk, chunks per block
-        unsigned char* const ring = smem_il + il_tables_bytes(mdv, a.max_np) + (size_t)a.W * (mdm + 4) * kIlGroup * sizeof(float) +
-                                    128 + (size_t)warp * AS * CE * kIlAsEdgeBytes;   // this warp's: AS chunks x CE edges x (t | p | p2)
+        unsigned char* const ring = reinterpret_cast<unsigned char*>(s_flag) + 128 + (size_t)warp * kRingWarp;   // this warp's: AS chunks x CE edges x (t | p | p2)
         const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
         const int half = lane >> 4;
         const unsigned l16 = (unsigned)(lane & 15) * 16u;
@@ -718,7 +727,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
 #pragma unroll
         for (int gi = 0; gi < GPW; ++gi)
 #pragma unroll
-            for (int v = 0; v < V; ++v) xch[((h * GPW + gi) * V + v) * kIlGroup] = part[gi][v];
+            for (int v = 0; v < V; ++v) *xch_at(h * GPW + gi, v) = part[gi][v];
         // the two warps of this slot meet here: release / acquire on a counter in shared memory (a named barrier per
         // slot would pin all 16 hardware barriers of the CTA)
         __syncwarp();
@@ -733,7 +742,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 2) k_pass_il(const Pas
         for (int v = 0; v < V; ++v) {
             sum[v] = 0.0f;
 #pragma unroll
-            for (int gg = 0; gg < G; ++gg) sum[v] += xch[(gg * V + v) * kIlGroup];
+            for (int gg = 0; gg < G; ++gg) sum[v] += *xch_at(gg, v);
         }
     }
     float L[V];
