@@ -571,7 +571,9 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
         const char* const hB = half ? qB : tB;                // lanes 0-15 copy the t pair, lanes 16-31 the partner pair
         const int n_chunks = ((dv + G * kIlChunk - 1) / (G * kIlChunk)) * GPW * kPer;
         auto off_of = [&](const int pre, const int thr) { return pre - (i0b >= thr ? Zb : 0); };
-        auto cp16 = [&](unsigned dst_s, const char* src) {
+        auto cp16 = [&](unsigned dst_s, const char* base, int off) {   // (base + off as ONE 32 x 32 + 64 multiply-add)
+            unsigned long long src;
+            asm("mad.wide.s32 %0, %1, 1, %2;" : "=l"(src) : "r"(off), "l"(reinterpret_cast<unsigned long long>(base)));
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_s), "l"(src) : "memory");
         };
         auto issue = [&](int c) {
@@ -585,7 +587,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
                     const int k = k0 + j;
                     if (whole || (k >= ngh && k < dv)) {
                         const IlRef r = reinterpret_cast<const IlRef*>(s_a + k)[half];   // lanes 0-15: t, lanes 16-31: p
-                        cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB + off_of(r.pre, r.thr));
+                        cp16(e_s + j * kIlAsEdgeBytes + half * 256, hB, off_of(r.pre, r.thr));
                     }
                 }
                 if (k0 < ng) {                                // second partners: lanes 0-15 edge 2u, lanes 16-31 edge 2u + 1
@@ -594,7 +596,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
                         const int k2 = k0 + 2 * u + half;
                         if (k2 >= ngh && k2 < ng) {
                             const IlRef r = s_b[k2].p2;
-                            cp16(e_s + (2 * u + half) * kIlAsEdgeBytes + 512, qB + off_of(r.pre, r.thr));
+                            cp16(e_s + (2 * u + half) * kIlAsEdgeBytes + 512, qB, off_of(r.pre, r.thr));
                         }
                     }
                 }
@@ -794,7 +796,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
         const bool st[V] = {live, live && val1 && round == 0};
 #pragma unroll 1
         for (int rnd = 0; rnd * G * kIlChunk < dv; ++rnd) {
-#pragma unroll
+#pragma unroll(AS > 0 ? 1 : GPW)
             for (int gi = 0; gi < GPW; ++gi) {
                 int k, ke;
                 block_of(rnd, gi, k, ke);
