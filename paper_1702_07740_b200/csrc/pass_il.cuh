@@ -738,7 +738,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
         for (;;) {
             asm volatile("ld.acquire.cta.s32 %0, [%1];" : "=r"(seen) : "l"(s_flag + slot * 2 + (1 - h)) : "memory");
             if (seen >= 1) break;
-            __nanosleep(40);                                  // leave the issue slots to the partner
+            __nanosleep(AS > 0 ? 200 : 40);                   // leave the issue slots to the others
         }
 #pragma unroll
         for (int v = 0; v < V; ++v) {
