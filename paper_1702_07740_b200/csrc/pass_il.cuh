@@ -308,7 +308,7 @@ constexpr int kIlV = 2;
 
 // MAXT: threads per CTA the instance is compiled for; 320 (up to five slots with H = 2) leaves 102 registers
 // per thread and takes the edges of triple rows eight at a time, 384 leaves 85 and takes them four at a time; 256 (AS > 0)
-// leaves 85 with three CTAs per multiprocessor.
+// leaves 64 with four CTAs per multiprocessor.
 // AS > 0 (H = 2, not FINAL): the loads of the pair and triple-row edges and of their static terms do not go through
 // registers.  A warp keeps AS chunks of four edges in flight as asynchronous 16-byte copies into its ring (768 bytes per
 // edge: the pairs of t, partner and second-partner lines of the slot's two variables; lanes 0-15 copy an edge's t pair,
@@ -997,7 +997,7 @@ inline void launch_pass_il_h(const IlLaunch& L) {
 inline void launch_pass_il(const IlLaunch& L) {
     if (L.args.split == 4) {
         const bool narrow = 32 * 2 * (L.args.W / 2) <= 320;
-        if (L.args.as_depth > 0 && 32 * 2 * (L.args.W / 2) <= 256) {   // three CTAs per multiprocessor
+        if (L.args.as_depth > 0 && 32 * 2 * (L.args.W / 2) <= 256) {   // four CTAs per multiprocessor
             switch (L.args.as_depth) {
                 case 1: launch_pass_il_h<2, 2, 256, 1>(L); break;
                 case 2: launch_pass_il_h<2, 2, 256, 2>(L); break;

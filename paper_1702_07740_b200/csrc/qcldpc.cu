@@ -566,7 +566,7 @@ static int code_from_lists(const BaseLists& B, int mb, int nb, int Z, qcldpc_cod
                   il_smem_bytes(code->max_dv, max_np, 2) <= (size_t)200 * 1024;
     // long columns (two warps per slot): the asynchronous variant -- messages in tensor memory, loads as asynchronous
     // copies through a ring, QCLDPC_ILA chunks deep (default 2; 0: register loads) --, eight variables per CTA so that
-    // three CTAs share a multiprocessor; short columns: register loads
+    // four CTAs share a multiprocessor; short columns: register loads
     code->il_w = il_pick_w(Z, code->max_dv, max_np);
     const bool long_cols = code->max_dv > 2 * kIlChunk;
     int as = long_cols ? env_int("QCLDPC_ILA", 2) : 0;
