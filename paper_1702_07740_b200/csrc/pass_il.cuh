@@ -607,18 +607,18 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
         for (int c = 0; c < AS; ++c) issue(c);
         // one rolled loop over the warp's chunks (the body is large; unrolled, the kernel outgrows the instruction caches)
 #pragma unroll 1
-        for (int c = 0; c < n_chunks; ++c) {
-            const int blk = c / kPer, r2 = c - blk * kPer, rnd = blk / GPW, gi = blk - rnd * GPW;
+        for (int blk = 0; blk * kPer < n_chunks; ++blk) {
+            const int rnd = blk / GPW, gi = blk - rnd * GPW;
             int kb, ke;
             block_of(rnd, gi, kb, ke);
-            const int k0 = kb + r2 * CE;
             float acc[V];
 #pragma unroll
             for (int v = 0; v < V; ++v) acc[v] = gi ? part[1][v] : part[0][v];
-            if (r2 == 0) {
 #pragma unroll 1
-                for (int k = kb; k < min(ke, ngh); ++k) gen_edge(k, acc);
-            }
+            for (int k = kb; k < min(ke, ngh); ++k) gen_edge(k, acc);
+#pragma unroll
+            for (int r2 = 0; r2 < kPer; ++r2) {
+            const int c = blk * kPer + r2, k0 = kb + r2 * CE;
             il_cp_async_wait<AS - 1>();               // this thread's copies of chunk c have landed ...
             __syncwarp();                             // ... and so have the other lanes'
             const float* const e = reinterpret_cast<const float*>(ring + (size_t)(c % AS) * CE * kIlAsEdgeBytes) + lane;
@@ -678,6 +678,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 4 : 2) k_pass_il(const Pas
             }
             __syncwarp();                             // every lane has read the ring entry: refill it
             issue(c + AS);
+            }
 #pragma unroll
             for (int v = 0; v < V; ++v) {
                 if (gi) part[1][v] = acc[v];
