@@ -129,6 +129,29 @@ def test_il_asynchronous_variant_equals_register_variant(B, monkeypatch, q, F):
                 np.testing.assert_array_equal(a, b)
 
 
+def test_il_two_decodes_at_once_on_two_streams(B):
+    """Two batched decodes in flight at once (two streams, a workspace each): their CTAs share the multiprocessors'
+    tensor memory, registers and shared memory; each must give what it gives alone."""
+    spec = W.paper_ensemble_spec(400, 50)
+    ens = W.make_paper_ensemble(spec)
+    code = B.QCLDPCCode.from_sparse(*ens, 50)
+    fa = W.make_frames_sparse(*ens, 50, W.sigma_for_gap(0.02, 3.0), 32, 1201)
+    fb = W.make_frames_sparse(*ens, 50, W.sigma_for_gap(0.02, 0.3), 64, 1202)
+    ins = [(torch.from_numpy(f.llr).cuda(), torch.from_numpy(f.syndrome).cuda()) for f in (fa, fb)]
+    alone = [code.decode(l, s, 60, 1, want_posterior=True) for l, s in ins]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for _ in range(3):
+        both = []
+        for (l, s), st in zip(ins, streams):
+            with torch.cuda.stream(st):
+                both.append(code.decode(l, s, 60, 1, want_posterior=True, stream=st))
+        torch.cuda.synchronize()
+        for got, ref in zip(both, alone):
+            for a, b in zip(got, ref):
+                assert torch.equal(a, b)
+
+
 def _random_code(rng, mb, nb, Z, density):
     base = np.full((mb, nb), -1, dtype=np.int32)
     mask = rng.random((mb, nb)) < density
